@@ -1,0 +1,213 @@
+/* gp.h — C-ABI of the B200-native null-geodesic tracer (libgp.so).
+ *
+ * The library integrates one null geodesic per image pixel through a stationary,
+ * axisymmetric spacetime in Hamiltonian form,
+ *     H(q,p) = 1/2 g^{mu nu}(q) p_mu p_nu = 0                      (eq 3)
+ *     dq^mu/dlambda = g^{mu nu} p_nu                                (eq 4 / L678, eq 102)
+ *     dp_mu/dlambda = -1/2 (d_mu g^{rho sigma}) p_rho p_sigma       (eq 103; eq 5 at L122 lacks the 1/2)
+ * with explicit Runge-Kutta steps (eq 42-49), from a camera until the
+ * ray is captured or leaves a bounding sphere (section 3.3.2; L404, section 5.1).
+ * Every step of the path runs in hand-written CUDA kernels for sm_100a; there is no CPU
+ * fallback.  All device buffers are owned by the caller; the library allocates nothing
+ * persistent and never synchronises the device (except gp_trace_host, which says so).
+ *
+ * Conventions: G = c = 1; coordinates (t, r, theta, phi) are Schwarzschild /
+ * Boyer-Lindquist (eq 8, L147-159 eq 9-14, L181-230 eq 20-39);
+ * DESIGN.md section 3 lists every reading taken where the paper is silent or garbled.
+ */
+#ifndef GP_H_
+#define GP_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GP_VERSION 100 /* major*10000 + minor*100 + patch */
+
+/* ---- spacetimes (section 2.2) ------------------------------------------- */
+enum {
+  GP_SCHWARZSCHILD = 0, /* PAPER.md L136, eq 8                                          */
+  GP_KERR = 1,          /* PAPER.md L147-159, eq 9-14, Boyer-Lindquist                  */
+  GP_MANKO_NOVIKOV = 2  /* PAPER.md L181-230, eq 20-39, quadrupole deviation only       */
+};
+
+/* M: mass; a = S/M: spin length (eq 14); q: Manko-Novikov quadrupole deviation (eq 25,
+ * beta = q M^3 / k^3).  Schwarzschild ignores a and q; Kerr ignores q.
+ * Valid: M > 0 (M = 0 allowed for GP_SCHWARZSCHILD only: flat space, capture test off);
+ * |a| < M; GP_MANKO_NOVIKOV needs a != 0 (eq 23 divides by S/M). */
+typedef struct gp_metric_params {
+  double M, a, q;
+} gp_metric_params;
+
+/* ---- camera: pinhole at (r_obs, theta_obs, phi_obs), ZAMO orthonormal tetrad --------
+ * Replaces PAPER.md L314-348 (section 3.3.1) per BASELINE.json; see DESIGN.md section 3.
+ * Ray index -> pixel: with S = supersample, Wt = width*S, Ht = height*S,
+ *   ray -> (I, J) = (ray mod Wt, ray div Wt);  J = 0 is the beta_min row.
+ *   X = (I + 0.5)/S + jit_x + shift_x_px,  Y = (J + 0.5)/S + jit_y + shift_y_px   [pixels]
+ *   alpha = alpha_min + X*((alpha_max-alpha_min)/width),  beta likewise with height.
+ * jit = (2u-1)*jitter_amp_px, u from a SplitMix64 hash of (jitter_seed, ray, axis);
+ * the map is evaluated with individually rounded operations and is bit-exact against the
+ * oracle.  Rays traced by a call: ray_begin + k*ray_stride for k in [0, ray_count);
+ * record k is written at slot k of the output buffers.                                 */
+typedef struct gp_camera {
+  double r_obs, theta_obs, phi_obs;
+  double alpha_min, alpha_max, beta_min, beta_max; /* image-plane window, units of length */
+  int32_t width, height;                           /* pixels, > 0                         */
+  int32_t supersample;                             /* S >= 1: S x S sub-rays per pixel    */
+  int32_t projection;                              /* 0 = pinhole in the ZAMO tetrad      */
+  uint64_t jitter_seed;
+  double jitter_amp_px;          /* 0 = sub-pixel centres; 0.5 = uniform in +-0.5 px      */
+  double shift_x_px, shift_y_px; /* rigid shift of the whole grid (chaos companion run)   */
+  int64_t ray_begin, ray_count, ray_stride; /* ray_stride >= 1; all rays < Wt*Ht          */
+} gp_camera;
+
+/* ---- integrator ---------------------------------------------------------------------
+ * scheme 0: classical RK4, fixed step h                     (eq 42-49)
+ * scheme 1: classical RK4, h_n = h_rel * r_n                (BASELINE.json configs[4])
+ * scheme 2: Dormand-Prince 5(4) embedded pair, FSAL, max-norm error over the six evolving
+ *           components, sc = atol + rtol*max(|y|,|y+|), fac = 0.9*err^(-1/5) clamped to
+ *           [0.2, 5], cap h <= h_cap_rel * r, h0 = h_cap_rel * r_obs
+ *           (BASELINE.json configs[1-3], reading R10).
+ * A ray ends: ESCAPED when a step lands at r > r_escape, CAPTURED when it lands at
+ * r < r_H*(1+eps_capture) (both followed by one landing step onto that surface with r as
+ * the independent variable), MAXSTEPS after max_steps attempted steps (or lambda >=
+ * lambda_max when lambda_max > 0), NONFINITE / STEP_UNDERFLOW on numerical failure.     */
+typedef struct gp_integrator_cfg {
+  int32_t scheme;    /* 0, 1, 2 as above                                                 */
+  int32_t precision; /* 0 = FP64 (the only one built); others -> GP_E_UNSUPPORTED        */
+  double h, h_rel, rtol, atol, h_cap_rel;
+  int64_t max_steps; /* attempted steps (accepted + rejected), landing steps not counted */
+  double lambda_max; /* <= 0: off                                                        */
+  double eps_capture, r_escape;
+  double disk_r_in, disk_r_out; /* thin equatorial disk; disk_r_in <= 0 -> prograde ISCO  */
+  int32_t max_crossings;        /* 0..3 recorded disk crossings; 0 = disk off             */
+  int32_t reserved_;
+} gp_integrator_cfg;
+
+/* ---- outputs ------------------------------------------------------------------------ */
+enum {
+  GP_RAY_ESCAPED = 0,
+  GP_RAY_CAPTURED = 1,
+  GP_RAY_MAXSTEPS = 2,
+  GP_RAY_NONFINITE = 3,
+  GP_RAY_STEP_UNDERFLOW = 4
+};
+
+/* One per ray, 128 bytes.  theta and phi are raw (accumulated, not wrapped).  The traced
+ * covector is the time-reversed one: p_t > 0 is the photon energy measured at infinity per
+ * unit locally (ZAMO) measured energy, and L_z = -p_phi (reading R12).        */
+typedef struct gp_ray_record {
+  double t, r, theta, phi, p_r, p_theta; /* state on the exit surface (or last state)    */
+  double lambda;                         /* affine parameter at exit                      */
+  double p_t, p_phi;                     /* constants of the ray                          */
+  double h_max;         /* max |H| over every state a step was attempted from            */
+  double q_drift;       /* Kerr/Schwarzschild: max |Q-Q0| / max(1,|Q0|), Carter constant  */
+  double sin_theta_min; /* min |sin theta| over the same states                           */
+  double err_margin;    /* scheme 2: min |err-1| over attempted steps; else +inf          */
+  uint32_t status;      /* GP_RAY_*                                                       */
+  uint32_t n_accepted, n_rejected;
+  uint32_t n_equator_crossings; /* sign changes of theta - pi/2 over accepted steps       */
+  uint32_t n_disk_recorded;     /* crossings with disk_r_in <= r <= disk_r_out, <= 3      */
+  uint32_t n_rhs;               /* evaluations of Hamilton's equations spent on this ray  */
+} gp_ray_record;
+
+/* One per ray when the disk is on, 48 bytes: crossing radius and redshift factor
+ * g = (p.u_obs)/(p.u_emit) for a prograde circular Keplerian emitter (PAPER.md L356-374,
+ * eq 56-57); unused slots hold NaN.                                                     */
+typedef struct gp_disk_record {
+  double r_cross[3];
+  double g[3];
+} gp_disk_record;
+
+/* Device buffers, caller-owned.  rays: >= ray_count*sizeof(gp_ray_record), 32-byte
+ * aligned.  disk: >= ray_count*sizeof(gp_disk_record) when max_crossings > 0, else may be
+ * NULL.  counters: >= 64 bytes, 8-byte aligned; the library zeroes it on the stream, uses
+ * word 0 as the atomic work counter and leaves totals behind:
+ *   [0] work counter (>= ray_count at exit)  [1] rays finished  [2] attempted steps
+ *   [3] RHS evaluations                      [4..7] reserved                            */
+typedef struct gp_out_buffers {
+  void *rays;
+  size_t rays_bytes;
+  void *disk;
+  size_t disk_bytes;
+  void *counters;
+  size_t counters_bytes;
+} gp_out_buffers;
+
+/* ---- error codes (return values; per-ray failures are data, not errors) ------------- */
+enum {
+  GP_OK = 0,
+  GP_E_BAD_METRIC = -1,
+  GP_E_BAD_PARAM = -2,
+  GP_E_NULL = -3,
+  GP_E_SIZE = -4,
+  GP_E_UNSUPPORTED = -5,
+  GP_E_CUDA = -6
+};
+
+/* ---- entry points -------------------------------------------------------------------
+ * All parameter structs are HOST memory, read before return.  `cuda_stream` is a
+ * cudaStream_t passed as void* (NULL = the legacy default stream).  Unless stated, calls
+ * validate synchronously, enqueue asynchronously on the stream and never synchronise.   */
+
+/* The hot path (BASELINE.json north_star): trace camera->ray_count rays and write one
+ * gp_ray_record (and gp_disk_record) per ray.  out->* are DEVICE pointers.
+ * Returns GP_OK or a GP_E_* code; on error nothing has been enqueued.                   */
+int gp_trace(int metric_id, const gp_metric_params *metric, const gp_camera *camera,
+             const gp_integrator_cfg *cfg, const gp_out_buffers *out, void *cuda_stream);
+
+/* Same computation with HOST output buffers (out->* are host pointers, pinned or
+ * pageable; counters may be NULL).  Allocates device scratch with cudaMallocAsync on the
+ * stream, runs gp_trace, copies the records back and SYNCHRONISES the stream before
+ * returning.  This is the end-to-end call bench.py times.                               */
+int gp_trace_host(int metric_id, const gp_metric_params *metric, const gp_camera *camera,
+                  const gp_integrator_cfg *cfg, const gp_out_buffers *out, void *cuda_stream);
+
+/* Steps a2+a3 alone (pixel -> (alpha,beta) -> initial state), for inspection and parity.
+ * states8: DEVICE, ray_count*8 doubles (t, r, theta, phi, p_t, p_r, p_theta, p_phi).
+ * alpha_beta2: DEVICE, ray_count*2 doubles, or NULL.                                    */
+int gp_init_conditions(int metric_id, const gp_metric_params *metric, const gp_camera *camera,
+                       void *states8, size_t states_bytes, void *alpha_beta2, size_t ab_bytes,
+                       void *cuda_stream);
+
+/* Step a4 alone: inverse metric and its r, theta derivatives at n points.
+ * r_theta2: DEVICE, n*2 doubles (r, theta).  out15: DEVICE, n*15 doubles in the order
+ * g^tt, g^tphi, g^phiphi, g^rr, g^thth, then the same five d/dr, then the same five
+ * d/dtheta.  Closed form for Schwarzschild and Kerr, forward-mode duals for MN.         */
+int gp_eval_metric(int metric_id, const gp_metric_params *metric, const void *r_theta2,
+                   int64_t n, void *out15, size_t out_bytes, void *cuda_stream);
+
+/* One evaluation of Hamilton's equations (steps a4+a5) at n states.
+ * states8: DEVICE n*8 doubles as above.  rhs6: DEVICE n*6 doubles
+ * (dt, dr, dtheta, dphi, dp_r, dp_theta)/dlambda.                                       */
+int gp_eval_rhs(int metric_id, const gp_metric_params *metric, const void *states8, int64_t n,
+                void *rhs6, size_t rhs_bytes, void *cuda_stream);
+
+/* FP64 FMA peak probe used for the roofline denominator: every thread of a full-chip grid
+ * runs `iters` rounds of 8 independent dependent-chain DFMAs; scratch (DEVICE, >= 8 bytes)
+ * receives a value that keeps the chain alive.  *flops_out (HOST) = 2 * DFMAs issued.
+ * Time it with events on the stream.                                                    */
+int gp_probe_fp64_fma(int64_t iters, void *scratch, size_t scratch_bytes, double *flops_out,
+                      void *cuda_stream);
+
+/* Horizon radius r_H and prograde ISCO radius used by the library for these parameters
+ * (r_isco = NaN for GP_MANKO_NOVIKOV).  Host-only helper.                               */
+int gp_metric_radii(int metric_id, const gp_metric_params *metric, double *r_horizon,
+                    double *r_isco);
+
+size_t gp_ray_record_size(void);  /* 128 */
+size_t gp_disk_record_size(void); /* 48  */
+size_t gp_counters_size(void);    /* 64  */
+int gp_version(void);
+/* Static string for a GP_E_* code; for GP_E_CUDA the last CUDA error text seen by this
+ * thread is appended.                                                                   */
+const char *gp_strerror(int code);
+
+#ifdef __cplusplus
+} /* extern "C" */
+#endif
+
+#endif /* GP_H_ */
