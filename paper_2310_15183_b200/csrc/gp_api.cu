@@ -1,0 +1,448 @@
+// gp_api.cu — C-ABI of libgp.so (include/gp.h): synchronous validation, per-launch constants
+// derived on the host in FP64, asynchronous launches on the caller's stream.
+// There is no CPU path: every step of the method runs in the kernels of gp_trace*.cuh.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include "../../include/gp.h"
+#include "gp_trace.cuh"
+
+static_assert(sizeof(gp_ray_record) == 128, "gp_ray_record must be 128 bytes");
+static_assert(sizeof(gp_disk_record) == 48, "gp_disk_record must be 48 bytes");
+
+namespace {
+
+using namespace gp;
+
+thread_local char g_cuda_msg[256] = "";
+
+int cuda_fail(cudaError_t e) {
+  snprintf(g_cuda_msg, sizeof(g_cuda_msg), "%s: %s", cudaGetErrorName(e), cudaGetErrorString(e));
+  return GP_E_CUDA;
+}
+#define GP_CUDA(call)                          \
+  do {                                         \
+    cudaError_t e__ = (call);                  \
+    if (e__ != cudaSuccess) return cuda_fail(e__); \
+  } while (0)
+
+// ---- validation + constants -------------------------------------------------------------------
+int make_metric(int metric_id, const gp_metric_params *m, MetricConst *mc) {
+  if (!m) return GP_E_NULL;
+  if (metric_id < GP_SCHWARZSCHILD || metric_id > GP_MANKO_NOVIKOV) return GP_E_BAD_METRIC;
+  memset(mc, 0, sizeof(*mc));
+  double M = m->M, a = m->a, q = m->q;
+  if (!isfinite(M) || !isfinite(a) || !isfinite(q)) return GP_E_BAD_PARAM;
+  if (metric_id == GP_SCHWARZSCHILD) {
+    if (!(M >= 0.0)) return GP_E_BAD_PARAM;  // M = 0: flat space
+    a = 0.0;
+    q = 0.0;
+  } else {
+    if (!(M > 0.0) || !(fabs(a) < M)) return GP_E_BAD_PARAM;
+    if (metric_id == GP_MANKO_NOVIKOV && a == 0.0) return GP_E_BAD_PARAM;  // eq 23 divides by S/M
+    if (metric_id == GP_KERR) q = 0.0;
+  }
+  mc->M = M;
+  mc->a = a;
+  mc->q = q;
+  mc->a2 = a * a;
+  mc->r_horizon = (metric_id == GP_SCHWARZSCHILD) ? 2.0 * M : M + sqrt(M * M - a * a);
+  if (metric_id == GP_MANKO_NOVIKOV) {
+    double al = (-M + sqrt(M * M - a * a)) / a;          // eq 23
+    double k = M * (1.0 - al * al) / (1.0 + al * al);    // eq 24
+    mc->mn_alpha = al;
+    mc->mn_k = k;
+    mc->mn_inv_k = 1.0 / k;
+    mc->mn_beta = q * M * M * M / (k * k * k);           // eq 25
+    mc->mn_w0 = 4.0 * k * al / (1.0 - al * al);
+    mc->mn_e0 = k * k / ((1.0 - al * al) * (1.0 - al * al));
+  }
+  return GP_OK;
+}
+
+double isco_prograde(int metric_id, const MetricConst &mc) {
+  if (metric_id == GP_MANKO_NOVIKOV) return nan("");
+  double M = mc.M;
+  double as = (M > 0.0) ? mc.a / M : 0.0;
+  double Z1 = 1.0 + cbrt(1.0 - as * as) * (cbrt(1.0 + as) + cbrt(1.0 - as));
+  double Z2 = sqrt(3.0 * as * as + Z1 * Z1);
+  return M * (3.0 + Z2 - sqrt((3.0 - Z1) * (3.0 + Z1 + 2.0 * Z2)));
+}
+
+int make_camera(int metric_id, const MetricConst &mc, const gp_camera *c, double eps_capture, CameraConst *cc) {
+  if (!c) return GP_E_NULL;
+  if (c->width <= 0 || c->height <= 0 || c->supersample <= 0) return GP_E_BAD_PARAM;
+  if (c->projection != 0) return GP_E_UNSUPPORTED;
+  if (!(c->alpha_max > c->alpha_min) || !(c->beta_max > c->beta_min)) return GP_E_BAD_PARAM;
+  if (!isfinite(c->alpha_min) || !isfinite(c->alpha_max) || !isfinite(c->beta_min) || !isfinite(c->beta_max))
+    return GP_E_BAD_PARAM;
+  if (!(c->theta_obs > 0.0) || !(c->theta_obs < 3.14159265358979323846)) return GP_E_BAD_PARAM;
+  if (!isfinite(c->r_obs) || !isfinite(c->phi_obs)) return GP_E_BAD_PARAM;
+  if (!(c->r_obs > mc.r_horizon * (1.0 + eps_capture)) || !(c->r_obs > 0.0)) return GP_E_BAD_PARAM;
+  if (!(c->jitter_amp_px >= 0.0) || !isfinite(c->jitter_amp_px) || !isfinite(c->shift_x_px) ||
+      !isfinite(c->shift_y_px))
+    return GP_E_BAD_PARAM;
+  const long long S = c->supersample;
+  const long long Wt = (long long)c->width * S, Ht = (long long)c->height * S;
+  const long long total = Wt * Ht;
+  if (c->ray_count < 0 || c->ray_begin < 0 || c->ray_stride < 1) return GP_E_BAD_PARAM;
+  if (c->ray_count > 0) {
+    if (c->ray_begin >= total) return GP_E_BAD_PARAM;
+    if ((c->ray_count - 1) > (total - 1 - c->ray_begin) / c->ray_stride) return GP_E_BAD_PARAM;
+  }
+  memset(cc, 0, sizeof(*cc));
+  cc->alpha_min = c->alpha_min;
+  cc->beta_min = c->beta_min;
+  cc->dalpha = (c->alpha_max - c->alpha_min) / (double)c->width;
+  cc->dbeta = (c->beta_max - c->beta_min) / (double)c->height;
+  cc->supersample_d = (double)S;
+  cc->jitter_amp_px = c->jitter_amp_px;
+  cc->shift_x_px = c->shift_x_px;
+  cc->shift_y_px = c->shift_y_px;
+  cc->jitter_seed = c->jitter_seed;
+  cc->Wt = Wt;
+  cc->ray_begin = c->ray_begin;
+  cc->ray_count = c->ray_count;
+  cc->ray_stride = c->ray_stride;
+  cc->r_obs = c->r_obs;
+  cc->theta_obs = c->theta_obs;
+  cc->phi_obs = c->phi_obs;
+  // observer's ZAMO tetrad from the covariant metric of the selected spacetime (reading R12)
+  double g[5];
+  metric_cov(metric_id, mc, c->r_obs, c->theta_obs, g);
+  double Omega = -g[1] / g[2];
+  double lapse2 = -(g[0] + Omega * g[1]);
+  if (!(lapse2 > 0.0) || !(g[2] > 0.0) || !(g[3] > 0.0) || !(g[4] > 0.0)) return GP_E_BAD_PARAM;
+  cc->Omega = Omega;
+  cc->inv_zeta = sqrt(lapse2);
+  cc->sq_grr = sqrt(g[3]);
+  cc->sq_gthth = sqrt(g[4]);
+  cc->sq_gpp = sqrt(g[2]);
+  return GP_OK;
+}
+
+int make_params(int metric_id, const gp_metric_params *m, const gp_camera *cam, const gp_integrator_cfg *cfg,
+                TraceParams *P) {
+  if (!m || !cam || !cfg) return GP_E_NULL;
+  memset(P, 0, sizeof(*P));
+  int rc = make_metric(metric_id, m, &P->mc);
+  if (rc) return rc;
+  if (cfg->precision != 0) return GP_E_UNSUPPORTED;
+  if (cfg->scheme < 0 || cfg->scheme > 2) return GP_E_BAD_PARAM;
+  if (!(cfg->eps_capture >= 0.0) || !isfinite(cfg->eps_capture)) return GP_E_BAD_PARAM;
+  rc = make_camera(metric_id, P->mc, cam, cfg->eps_capture, &P->cc);
+  if (rc) return rc;
+  if (cfg->max_steps < 0 || cfg->max_steps > 500000000LL) return GP_E_BAD_PARAM;
+  if (!(cfg->r_escape > cam->r_obs) || !isfinite(cfg->r_escape)) return GP_E_BAD_PARAM;
+  if (cfg->scheme == 0 && !(cfg->h > 0.0 && isfinite(cfg->h))) return GP_E_BAD_PARAM;
+  if (cfg->scheme == 1 && !(cfg->h_rel > 0.0 && isfinite(cfg->h_rel))) return GP_E_BAD_PARAM;
+  if (cfg->scheme == 2) {
+    if (!(cfg->rtol > 0.0) || !(cfg->atol >= 0.0) || !(cfg->h_cap_rel > 0.0)) return GP_E_BAD_PARAM;
+    if (!isfinite(cfg->rtol) || !isfinite(cfg->atol) || !isfinite(cfg->h_cap_rel)) return GP_E_BAD_PARAM;
+  }
+  if (cfg->max_crossings < 0 || cfg->max_crossings > 3) return GP_E_BAD_PARAM;
+  if (cfg->max_crossings > 0 && metric_id == GP_MANKO_NOVIKOV) return GP_E_UNSUPPORTED;
+  if (isnan(cfg->lambda_max)) return GP_E_BAD_PARAM;
+  P->scheme = cfg->scheme;
+  P->max_crossings = cfg->max_crossings;
+  P->h = cfg->h;
+  P->h_rel = cfg->h_rel;
+  P->rtol = cfg->rtol;
+  P->atol = cfg->atol;
+  P->h_cap_rel = cfg->h_cap_rel;
+  P->max_steps = cfg->max_steps;
+  P->lambda_max = cfg->lambda_max;
+  P->r_cap = P->mc.r_horizon * (1.0 + cfg->eps_capture);
+  P->r_esc = cfg->r_escape;
+  if (cfg->max_crossings > 0) {
+    P->disk_r_in = (cfg->disk_r_in > 0.0) ? cfg->disk_r_in : isco_prograde(metric_id, P->mc);
+    P->disk_r_out = cfg->disk_r_out;
+    if (!(P->disk_r_out >= P->disk_r_in)) return GP_E_BAD_PARAM;
+  }
+  return GP_OK;
+}
+
+// ---- launch -----------------------------------------------------------------------------------
+template <int METRIC, bool DISK>
+int launch_one(const TraceParams &P, cudaStream_t stream) {
+  static int blocks_dp = 0, blocks_rk = 0;
+  static int n_sm = 0;
+  const bool dp54 = (P.scheme == 2);
+  const size_t smem = DISK ? sizeof(double) * kBlock * (dp54 ? kParkSlotsDp54 : kParkSlotsRk4) : 0;
+  int &per_sm = dp54 ? blocks_dp : blocks_rk;
+  if (per_sm == 0) {
+    int dev = 0;
+    GP_CUDA(cudaGetDevice(&dev));
+    GP_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+    int occ = 0;
+    if (dp54)
+      GP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, trace_dp54<METRIC, DISK>, kBlock, smem));
+    else
+      GP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, trace_rk4<METRIC, DISK>, kBlock, smem));
+    if (occ < 1) occ = 1;
+    per_sm = occ;
+  }
+  // persistent grid: every SM filled to its resident-block limit, never more lanes than rays
+  long long want = ((long long)P.cc.ray_count + kBlock - 1) / kBlock;
+  long long grid = (long long)n_sm * per_sm;
+  if (grid > want) grid = want;
+  if (grid < 1) grid = 1;
+  if (dp54)
+    trace_dp54<METRIC, DISK><<<(unsigned)grid, kBlock, smem, stream>>>(P);
+  else
+    trace_rk4<METRIC, DISK><<<(unsigned)grid, kBlock, smem, stream>>>(P);
+  GP_CUDA(cudaGetLastError());
+  return GP_OK;
+}
+
+int launch_trace(int metric_id, const TraceParams &P, cudaStream_t stream) {
+  const bool disk = P.max_crossings > 0;
+  switch (metric_id) {
+    case GP_SCHWARZSCHILD:
+      return disk ? launch_one<METRIC_SCHW, true>(P, stream) : launch_one<METRIC_SCHW, false>(P, stream);
+    case GP_KERR:
+      return disk ? launch_one<METRIC_KERR, true>(P, stream) : launch_one<METRIC_KERR, false>(P, stream);
+    default:
+      return launch_one<METRIC_MN, false>(P, stream);
+  }
+}
+
+// ---- step-level kernels (parity of rows a2-a5 in isolation) -------------------------------------
+__global__ void k_init_conditions(const __grid_constant__ CameraConst cc, double *states8, double *ab2) {
+  long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= cc.ray_count) return;
+  double alpha, beta, pt, pr, pth, pph;
+  alpha_beta(cc, cc.ray_begin + k * cc.ray_stride, alpha, beta);
+  initial_momentum(cc, alpha, beta, pt, pr, pth, pph);
+  double *s = states8 + 8 * k;
+  s[0] = 0.0; s[1] = cc.r_obs; s[2] = cc.theta_obs; s[3] = cc.phi_obs;
+  s[4] = pt; s[5] = pr; s[6] = pth; s[7] = pph;
+  if (ab2) {
+    ab2[2 * k] = alpha;
+    ab2[2 * k + 1] = beta;
+  }
+}
+
+__global__ void k_eval_metric(int metric, const __grid_constant__ MetricConst mc, const double *rt2, long long n,
+                              double *out15) {
+  long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= n) return;
+  double o[15];
+  metric_inv15(metric, mc, rt2[2 * k], rt2[2 * k + 1], o);
+  for (int i = 0; i < 15; ++i) out15[15 * k + i] = o[i];
+}
+
+template <int METRIC>
+__global__ void k_eval_rhs(const __grid_constant__ MetricConst mc, const double *st8, long long n, double *rhs6) {
+  long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= n) return;
+  const double *s = st8 + 8 * k;
+  Rhs o;
+  rhs_eval<METRIC>(mc, s[4], s[7], s[1], s[2], s[5], s[6], o);
+  double *d = rhs6 + 6 * k;
+  d[0] = o.dt; d[1] = o.dr; d[2] = o.dth; d[3] = o.dph; d[4] = o.dpr; d[5] = o.dpth;
+}
+
+// FP64 FMA peak probe: 8 independent dependent chains per thread.
+__global__ void __launch_bounds__(256) k_probe_fma(long long iters, double seed, double *sink) {
+  double a0 = seed + threadIdx.x, a1 = a0 + 1.0, a2 = a0 + 2.0, a3 = a0 + 3.0, a4 = a0 + 4.0, a5 = a0 + 5.0,
+         a6 = a0 + 6.0, a7 = a0 + 7.0;
+  const double m = 0.999999, c = 1e-9;
+  for (long long i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+      a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+    }
+  }
+  double s = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+  if (s == 123.456) *sink = s;  // keeps the chains alive without a store in practice
+}
+
+}  // namespace
+
+// ---- exported entry points -----------------------------------------------------------------------
+extern "C" {
+
+int gp_trace(int metric_id, const gp_metric_params *metric, const gp_camera *camera,
+             const gp_integrator_cfg *cfg, const gp_out_buffers *out, void *cuda_stream) {
+  if (!out) return GP_E_NULL;
+  TraceParams P;
+  int rc = make_params(metric_id, metric, camera, cfg, &P);
+  if (rc) return rc;
+  const size_t n = (size_t)camera->ray_count;
+  if (!out->counters) return GP_E_NULL;
+  if (out->counters_bytes < 64) return GP_E_SIZE;
+  if (((uintptr_t)out->counters & 7u) != 0) return GP_E_BAD_PARAM;
+  if (n > 0) {
+    if (!out->rays) return GP_E_NULL;
+    if (out->rays_bytes < n * sizeof(gp_ray_record)) return GP_E_SIZE;
+    if (((uintptr_t)out->rays & 31u) != 0) return GP_E_BAD_PARAM;
+    if (cfg->max_crossings > 0) {
+      if (!out->disk) return GP_E_NULL;
+      if (out->disk_bytes < n * sizeof(gp_disk_record)) return GP_E_SIZE;
+      if (((uintptr_t)out->disk & 7u) != 0) return GP_E_BAD_PARAM;
+    }
+  }
+  P.rays = (gp_ray_record *)out->rays;
+  P.disk = (gp_disk_record *)out->disk;
+  P.counters = (unsigned long long *)out->counters;
+  cudaStream_t stream = (cudaStream_t)cuda_stream;
+  GP_CUDA(cudaMemsetAsync(out->counters, 0, 64, stream));
+  if (n == 0) return GP_OK;
+  return launch_trace(metric_id, P, stream);
+}
+
+int gp_trace_host(int metric_id, const gp_metric_params *metric, const gp_camera *camera,
+                  const gp_integrator_cfg *cfg, const gp_out_buffers *out, void *cuda_stream) {
+  if (!out || !camera || !cfg) return GP_E_NULL;
+  TraceParams P;
+  int rc = make_params(metric_id, metric, camera, cfg, &P);
+  if (rc) return rc;
+  const size_t n = (size_t)camera->ray_count;
+  const bool disk = cfg->max_crossings > 0;
+  const size_t rays_b = n * sizeof(gp_ray_record), disk_b = disk ? n * sizeof(gp_disk_record) : 0;
+  if (n > 0) {
+    if (!out->rays) return GP_E_NULL;
+    if (out->rays_bytes < rays_b) return GP_E_SIZE;
+    if (disk && !out->disk) return GP_E_NULL;
+    if (disk && out->disk_bytes < disk_b) return GP_E_SIZE;
+  }
+  if (out->counters && out->counters_bytes < 64) return GP_E_SIZE;
+  cudaStream_t stream = (cudaStream_t)cuda_stream;
+  // one scratch allocation: counters | ray records | disk records
+  const size_t off_rays = 64, off_disk = off_rays + ((rays_b + 63) & ~(size_t)63);
+  char *scratch = nullptr;
+  GP_CUDA(cudaMallocAsync((void **)&scratch, off_disk + disk_b + 64, stream));
+  gp_out_buffers dev;
+  dev.counters = scratch;
+  dev.counters_bytes = 64;
+  dev.rays = scratch + off_rays;
+  dev.rays_bytes = rays_b;
+  dev.disk = disk ? scratch + off_disk : nullptr;
+  dev.disk_bytes = disk_b;
+  rc = gp_trace(metric_id, metric, camera, cfg, &dev, cuda_stream);
+  cudaError_t e = cudaSuccess;
+  if (rc == GP_OK) {
+    if (n > 0) e = cudaMemcpyAsync(out->rays, dev.rays, rays_b, cudaMemcpyDeviceToHost, stream);
+    if (e == cudaSuccess && disk && n > 0)
+      e = cudaMemcpyAsync(out->disk, dev.disk, disk_b, cudaMemcpyDeviceToHost, stream);
+    if (e == cudaSuccess && out->counters)
+      e = cudaMemcpyAsync(out->counters, dev.counters, 64, cudaMemcpyDeviceToHost, stream);
+  }
+  cudaError_t e2 = cudaFreeAsync(scratch, stream);
+  cudaError_t e3 = cudaStreamSynchronize(stream);
+  if (rc != GP_OK) return rc;
+  if (e != cudaSuccess) return cuda_fail(e);
+  if (e2 != cudaSuccess) return cuda_fail(e2);
+  if (e3 != cudaSuccess) return cuda_fail(e3);
+  return GP_OK;
+}
+
+int gp_init_conditions(int metric_id, const gp_metric_params *metric, const gp_camera *camera, void *states8,
+                       size_t states_bytes, void *alpha_beta2, size_t ab_bytes, void *cuda_stream) {
+  if (!metric || !camera) return GP_E_NULL;
+  MetricConst mc;
+  int rc = make_metric(metric_id, metric, &mc);
+  if (rc) return rc;
+  CameraConst cc;
+  rc = make_camera(metric_id, mc, camera, 0.0, &cc);
+  if (rc) return rc;
+  const size_t n = (size_t)camera->ray_count;
+  if (n == 0) return GP_OK;
+  if (!states8) return GP_E_NULL;
+  if (states_bytes < n * 64) return GP_E_SIZE;
+  if (alpha_beta2 && ab_bytes < n * 16) return GP_E_SIZE;
+  const unsigned grid = (unsigned)((n + 255) / 256);
+  k_init_conditions<<<grid, 256, 0, (cudaStream_t)cuda_stream>>>(cc, (double *)states8, (double *)alpha_beta2);
+  GP_CUDA(cudaGetLastError());
+  return GP_OK;
+}
+
+int gp_eval_metric(int metric_id, const gp_metric_params *metric, const void *r_theta2, int64_t n, void *out15,
+                   size_t out_bytes, void *cuda_stream) {
+  if (!metric) return GP_E_NULL;
+  MetricConst mc;
+  int rc = make_metric(metric_id, metric, &mc);
+  if (rc) return rc;
+  if (n < 0) return GP_E_BAD_PARAM;
+  if (n == 0) return GP_OK;
+  if (!r_theta2 || !out15) return GP_E_NULL;
+  if (out_bytes < (size_t)n * 15 * sizeof(double)) return GP_E_SIZE;
+  const unsigned grid = (unsigned)((n + 127) / 128);
+  k_eval_metric<<<grid, 128, 0, (cudaStream_t)cuda_stream>>>(metric_id, mc, (const double *)r_theta2, n,
+                                                             (double *)out15);
+  GP_CUDA(cudaGetLastError());
+  return GP_OK;
+}
+
+int gp_eval_rhs(int metric_id, const gp_metric_params *metric, const void *states8, int64_t n, void *rhs6,
+                size_t rhs_bytes, void *cuda_stream) {
+  if (!metric) return GP_E_NULL;
+  MetricConst mc;
+  int rc = make_metric(metric_id, metric, &mc);
+  if (rc) return rc;
+  if (n < 0) return GP_E_BAD_PARAM;
+  if (n == 0) return GP_OK;
+  if (!states8 || !rhs6) return GP_E_NULL;
+  if (rhs_bytes < (size_t)n * 6 * sizeof(double)) return GP_E_SIZE;
+  const unsigned grid = (unsigned)((n + 127) / 128);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (metric_id == GP_SCHWARZSCHILD)
+    k_eval_rhs<METRIC_SCHW><<<grid, 128, 0, st>>>(mc, (const double *)states8, n, (double *)rhs6);
+  else if (metric_id == GP_KERR)
+    k_eval_rhs<METRIC_KERR><<<grid, 128, 0, st>>>(mc, (const double *)states8, n, (double *)rhs6);
+  else
+    k_eval_rhs<METRIC_MN><<<grid, 128, 0, st>>>(mc, (const double *)states8, n, (double *)rhs6);
+  GP_CUDA(cudaGetLastError());
+  return GP_OK;
+}
+
+int gp_probe_fp64_fma(int64_t iters, void *scratch, size_t scratch_bytes, double *flops_out, void *cuda_stream) {
+  if (!scratch || !flops_out) return GP_E_NULL;
+  if (scratch_bytes < 8) return GP_E_SIZE;
+  if (iters <= 0) return GP_E_BAD_PARAM;
+  int dev = 0, n_sm = 0;
+  GP_CUDA(cudaGetDevice(&dev));
+  GP_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+  const int blocks = n_sm * 8, threads = 256;  // 2048 resident threads per SM
+  k_probe_fma<<<blocks, threads, 0, (cudaStream_t)cuda_stream>>>(iters, 0.5, (double *)scratch);
+  GP_CUDA(cudaGetLastError());
+  *flops_out = 2.0 * 64.0 * (double)iters * (double)blocks * (double)threads;
+  return GP_OK;
+}
+
+int gp_metric_radii(int metric_id, const gp_metric_params *metric, double *r_horizon, double *r_isco) {
+  if (!metric || !r_horizon || !r_isco) return GP_E_NULL;
+  MetricConst mc;
+  int rc = make_metric(metric_id, metric, &mc);
+  if (rc) return rc;
+  *r_horizon = mc.r_horizon;
+  *r_isco = isco_prograde(metric_id, mc);
+  return GP_OK;
+}
+
+size_t gp_ray_record_size(void) { return sizeof(gp_ray_record); }
+size_t gp_disk_record_size(void) { return sizeof(gp_disk_record); }
+size_t gp_counters_size(void) { return 64; }
+int gp_version(void) { return GP_VERSION; }
+
+const char *gp_strerror(int code) {
+  static thread_local char buf[320];
+  switch (code) {
+    case GP_OK: return "ok";
+    case GP_E_BAD_METRIC: return "unknown metric id";
+    case GP_E_BAD_PARAM: return "parameter out of range";
+    case GP_E_NULL: return "null pointer";
+    case GP_E_SIZE: return "buffer too small";
+    case GP_E_UNSUPPORTED: return "variant not built";
+    case GP_E_CUDA:
+      snprintf(buf, sizeof(buf), "CUDA error: %s", g_cuda_msg);
+      return buf;
+  }
+  return "unknown error code";
+}
+
+}  // extern "C"

@@ -1,0 +1,140 @@
+// gp_trace.cuh — the fused integrator kernels.
+//
+// One lane integrates one ray at a time and holds its whole state in registers; lanes pull
+// ray slots from a global atomic counter (warp-aggregated) so that a lane whose ray ended
+// refills at once and warps stay full in spite of divergent ray lengths (edge
+// rays leave in < 1000 steps, others run 5e4..1e6).  Ordinary steps, landing steps onto the
+// exit surface and landing steps onto the equator are ONE instruction stream: a landing step
+// is a step of the same Runge-Kutta formula on dy/ds = F(y)/F_w(y) (Henon's device, DESIGN.md
+// reading R14), so a per-lane reciprocal selector is all that differs.
+//
+//   classical RK4            PAPER.md L257-278 (eq 42-49), reading R9      -> trace_rk4
+//   Dormand-Prince 5(4)      BASELINE.json configs[1-3], reading R10        -> trace_dp54
+#ifndef GP_TRACE_CUH_
+#define GP_TRACE_CUH_
+
+#include "../../include/gp.h"
+#include "gp_camera.cuh"
+#include "gp_metric.cuh"
+
+namespace gp {
+
+struct TraceParams {
+  MetricConst mc;
+  CameraConst cc;
+  int scheme;                       // 0 RK4 fixed h, 1 RK4 h = h_rel r, 2 DP5(4)
+  int max_crossings;                // 0 = disk off
+  double h, h_rel, rtol, atol, h_cap_rel;
+  long long max_steps;
+  double lambda_max;
+  double r_cap, r_esc;              // r_H (1 + eps_capture), r_escape
+  double disk_r_in, disk_r_out;
+  gp_ray_record *rays;
+  gp_disk_record *disk;
+  unsigned long long *counters;
+};
+
+enum { MODE_IDLE = 0, MODE_FRESH = 1, MODE_NORMAL = 2, MODE_LAND_R = 3, MODE_LAND_TH = 4 };
+
+constexpr int kBlock = 128;
+constexpr unsigned kFull = 0xffffffffu;
+constexpr double kHalfPi = 1.57079632679489661923;
+
+// Dormand & Prince (1980) 5(4) pair, reading R10.
+namespace dp {
+constexpr double A21 = 1.0 / 5.0;
+constexpr double A31 = 3.0 / 40.0, A32 = 9.0 / 40.0;
+constexpr double A41 = 44.0 / 45.0, A42 = -56.0 / 15.0, A43 = 32.0 / 9.0;
+constexpr double A51 = 19372.0 / 6561.0, A52 = -25360.0 / 2187.0, A53 = 64448.0 / 6561.0, A54 = -212.0 / 729.0;
+constexpr double A61 = 9017.0 / 3168.0, A62 = -355.0 / 33.0, A63 = 46732.0 / 5247.0, A64 = 49.0 / 176.0,
+                 A65 = -5103.0 / 18656.0;
+constexpr double B1 = 35.0 / 384.0, B3 = 500.0 / 1113.0, B4 = 125.0 / 192.0, B5 = -2187.0 / 6784.0,
+                 B6 = 11.0 / 84.0;
+constexpr double E1 = 71.0 / 57600.0, E3 = -71.0 / 16695.0, E4 = 71.0 / 1920.0, E5 = -17253.0 / 339200.0,
+                 E6 = 22.0 / 525.0, E7 = -1.0 / 40.0;
+}  // namespace dp
+
+#if defined(__CUDACC__)
+
+__device__ __forceinline__ bool finite_d(double x) { return fabs(x) <= 1.79769313486231570815e308; }
+
+// 256-bit store of four doubles (one 32-byte sector per instruction; row a11).
+__device__ __forceinline__ void store4(double *p, double a, double b, double c, double d) {
+  asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
+}
+
+// Warp-aggregated work fetch (row a1): one atomic per warp per refill round.  Returns the output
+// slot for this lane or -1 when the image is exhausted.
+__device__ __forceinline__ long long fetch_slot(unsigned need_mask, bool need, unsigned long long *counter,
+                                                long long ray_count) {
+  const unsigned lane = threadIdx.x & 31u;
+  const int leader = __ffs(need_mask) - 1;
+  unsigned long long base = 0;
+  if ((int)lane == leader) base = atomicAdd(counter, (unsigned long long)__popc(need_mask));
+  base = __shfl_sync(kFull, base, leader);
+  if (!need) return -1;
+  long long slot = (long long)(base + (unsigned long long)__popc(need_mask & ((1u << lane) - 1u)));
+  return slot < ray_count ? slot : -1;
+}
+
+// Prograde Keplerian emitter on the equator (eq 56 in closed form; L372,
+// eq 57; readings R19/R20): g = (p.u_obs)/(p.u_emit) = 1/[u^t (p_t + Omega_K p_phi)].
+__device__ __forceinline__ double kepler_g(const MetricConst &mc, double r, double pt, double pph) {
+  double sM = sqrt(mc.M);
+  double sr = sqrt(r);
+  double r32 = r * sr;
+  double den = r32 + mc.a * sM;
+  double Om = sM / den;
+  double ut = den / (sqrt(r32) * sqrt(r32 - 3.0 * mc.M * sr + 2.0 * mc.a * sM));
+  return 1.0 / (ut * (pt + Om * pph));
+}
+
+// Monitors of row a10 carried per lane.
+struct Monitors {
+  double h_max, q_drift, Q0, sin_min, err_margin;
+};
+
+// Carter constant, exact off shell (reading R23): Q = p_th^2 + c^2 (p_ph^2/s^2 - a^2 p_t^2) - 2 a^2 c^2 H.
+template <int METRIC>
+__device__ __forceinline__ double carter_q(const MetricConst &mc, double pt, double pph, double pth,
+                                           const Rhs &o) {
+  if (METRIC == METRIC_MN) return 0.0;
+  const double a2 = (METRIC == METRIC_KERR) ? mc.a2 : 0.0;
+  double c2 = o.c * o.c;
+  return pth * pth + c2 * (pph * pph * o.is * o.is - a2 * pt * pt) - a2 * c2 * o.H2;
+}
+
+template <int METRIC>
+__device__ __forceinline__ void monitor_apply(Monitors &mo, double absH, double Q, double abss, bool first) {
+  mo.h_max = fmax(mo.h_max, absH);
+  mo.sin_min = fmin(mo.sin_min, abss);
+  if (METRIC != METRIC_MN) {
+    if (first) mo.Q0 = Q;
+    double d = fabs(Q - mo.Q0) / fmax(1.0, fabs(mo.Q0));
+    mo.q_drift = fmax(mo.q_drift, d);
+  }
+}
+
+// Row a11: pack and store the 128-byte record with four 256-bit stores.
+__device__ __forceinline__ void store_record(gp_ray_record *rec, double t, double r, double th, double ph,
+                                             double pr, double pth, double lam, double pt, double pph,
+                                             const Monitors &mo, unsigned status, unsigned n_acc,
+                                             unsigned n_rej, unsigned n_cross, unsigned n_rec,
+                                             unsigned n_rhs) {
+  double *p = reinterpret_cast<double *>(rec);
+  store4(p, t, r, th, ph);
+  store4(p + 4, pr, pth, lam, pt);
+  store4(p + 8, pph, mo.h_max, mo.q_drift, mo.sin_min);
+  double w0 = __hiloint2double((int)n_acc, (int)status);      // little endian: status, n_accepted
+  double w1 = __hiloint2double((int)n_cross, (int)n_rej);     // n_rejected, n_equator_crossings
+  double w2 = __hiloint2double((int)n_rhs, (int)n_rec);       // n_disk_recorded, n_rhs
+  store4(p + 12, mo.err_margin, w0, w1, w2);
+}
+
+#endif  // __CUDACC__
+}  // namespace gp
+
+#include "gp_trace_dp54.cuh"
+#include "gp_trace_rk4.cuh"
+
+#endif

@@ -1,0 +1,157 @@
+"""CPU-side checks of the C-ABI boundary: libgp.so builds for sm_100a, loads, exports every
+symbol include/gp.h declares, keeps the documented record layouts, validates arguments
+synchronously, and FAILS LOUDLY (GP_E_CUDA) instead of falling back when no GPU is present.
+No kernel is launched here.
+"""
+import ctypes as C
+import math
+import os
+import re
+import subprocess
+
+import numpy as np
+import pytest
+
+import gp_workloads as W
+import paper_2310_15183_b200 as gp
+from paper_2310_15183_b200 import api
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+HEADER = os.path.join(ROOT, "include", "gp.h")
+
+
+def _declared_functions():
+    src = open(HEADER).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(gp_[a-z0-9_]+)\s*\(", src)))
+
+
+def test_every_declared_symbol_is_exported():
+    names = _declared_functions()
+    assert "gp_trace" in names and "gp_trace_host" in names and len(names) >= 12
+    lib = C.CDLL(os.path.join(ROOT, "paper_2310_15183_b200", "libgp.so"))
+    for n in names:
+        assert hasattr(lib, n), f"{n} declared in gp.h but not exported by libgp.so"
+    assert set(names) == set(api.EXPORTS)
+    for n in names:
+        assert callable(getattr(gp, n)), f"binding lacks {n}"
+
+
+def test_library_is_sm100a_native_cuda():
+    """The binary carries sm_100a SASS for both integrator kernels (no PTX-only JIT path)."""
+    out = subprocess.run(["cuobjdump", "-lelf", os.path.join(ROOT, "paper_2310_15183_b200", "libgp.so")],
+                         capture_output=True, text=True)
+    if out.returncode != 0:
+        pytest.skip("cuobjdump unavailable")
+    assert "sm_100a" in out.stdout
+
+
+def test_record_layouts():
+    assert gp.gp_ray_record_size() == 128 == api.RAY_DTYPE.itemsize
+    assert gp.gp_disk_record_size() == 48 == api.DISK_DTYPE.itemsize
+    assert gp.gp_counters_size() == 64
+    assert gp.gp_version() == 100
+    f = api.RAY_DTYPE.fields
+    assert f["lambda"][1] == 48 and f["err_margin"][1] == 96 and f["status"][1] == 104 and f["n_rhs"][1] == 124
+    assert C.sizeof(api.gp_camera) == 7 * 8 + 4 * 4 + 8 + 3 * 8 + 3 * 8
+    assert C.sizeof(api.gp_integrator_cfg) == 8 + 5 * 8 + 8 + 8 + 2 * 8 + 2 * 8 + 8
+
+
+def test_strerror():
+    assert gp.gp_strerror(0) == "ok"
+    for code in range(-6, 0):
+        assert gp.gp_strerror(code) not in ("ok", "unknown error code")
+    assert gp.gp_strerror(-99) == "unknown error code"
+
+
+def test_metric_radii_closed_forms():
+    """r_+ = M + sqrt(M^2 - a^2) and the Bardeen-Press-Teukolsky prograde ISCO (values computed
+    independently with mpmath during the survey, SURVEY.md pin P11)."""
+    rh, ri = gp.gp_metric_radii(gp.GP_KERR, api.gp_metric_params(1.0, 0.9, 0.0))
+    assert rh == pytest.approx(1.435889894354067, abs=1e-15)
+    assert ri == pytest.approx(2.320883041761887, abs=1e-14)
+    rh, ri = gp.gp_metric_radii(gp.GP_KERR, api.gp_metric_params(1.0, 0.998, 0.0))
+    assert rh == pytest.approx(1.063213922517116, abs=1e-15)
+    assert ri == pytest.approx(1.236970655175184, abs=1e-13)
+    rh, ri = gp.gp_metric_radii(gp.GP_SCHWARZSCHILD, api.gp_metric_params(1.0, 0.3, 0.0))
+    assert rh == 2.0 and ri == pytest.approx(6.0, abs=1e-14)
+    rh, ri = gp.gp_metric_radii(gp.GP_MANKO_NOVIKOV, api.gp_metric_params(1.0, 0.9, 0.5))
+    assert rh == pytest.approx(1.4358898943540674, abs=1e-15) and math.isnan(ri)
+
+
+def _call(w, mutate=None, metric_id=None, out=None, entry="gp_trace"):
+    m = api.metric_struct(w["metric"])
+    cam = api.camera_struct(w["camera"], 0, 64, 1)
+    cfg = api.cfg_struct(w["cfg"])
+    if mutate:
+        mutate(m, cam, cfg)
+    if out is None:
+        out = api.gp_out_buffers(C.c_void_p(0x1000), 64 * 128, C.c_void_p(0x2000), 64 * 48,
+                                 C.c_void_p(0x3000), 64)
+    mid = w["metric"]["id"] if metric_id is None else metric_id
+    return getattr(api.lib, entry)(mid, C.byref(m), C.byref(cam), C.byref(cfg), C.byref(out), None)
+
+
+BAD = [
+    ("metric id", lambda m, c, g: None, 7, api.GP_E_BAD_METRIC),
+    ("M < 0", lambda m, c, g: setattr(m, "M", -1.0), None, api.GP_E_BAD_PARAM),
+    ("|a| >= M", lambda m, c, g: setattr(m, "a", 1.0), None, api.GP_E_BAD_PARAM),
+    ("theta_obs on the axis", lambda m, c, g: setattr(c, "theta_obs", 0.0), None, api.GP_E_BAD_PARAM),
+    ("observer inside the capture radius", lambda m, c, g: setattr(c, "r_obs", 1.2), None, api.GP_E_BAD_PARAM),
+    ("empty window", lambda m, c, g: setattr(c, "alpha_max", c.alpha_min), None, api.GP_E_BAD_PARAM),
+    ("width 0", lambda m, c, g: setattr(c, "width", 0), None, api.GP_E_BAD_PARAM),
+    ("rays beyond the image", lambda m, c, g: setattr(c, "ray_begin", 512 * 512 - 10), None, api.GP_E_BAD_PARAM),
+    ("stride 0", lambda m, c, g: setattr(c, "ray_stride", 0), None, api.GP_E_BAD_PARAM),
+    ("rtol 0", lambda m, c, g: setattr(g, "rtol", 0.0), None, api.GP_E_BAD_PARAM),
+    ("scheme 9", lambda m, c, g: setattr(g, "scheme", 9), None, api.GP_E_BAD_PARAM),
+    ("r_escape inside r_obs", lambda m, c, g: setattr(g, "r_escape", 10.0), None, api.GP_E_BAD_PARAM),
+    ("4 crossings", lambda m, c, g: setattr(g, "max_crossings", 4), None, api.GP_E_BAD_PARAM),
+    ("FP32 variant not built", lambda m, c, g: setattr(g, "precision", 1), None, api.GP_E_UNSUPPORTED),
+    ("projection 1", lambda m, c, g: setattr(c, "projection", 1), None, api.GP_E_UNSUPPORTED),
+]
+
+
+@pytest.mark.parametrize("entry", ["gp_trace", "gp_trace_host"])
+@pytest.mark.parametrize("what,mutate,metric_id,code", BAD, ids=[b[0] for b in BAD])
+def test_validation_is_synchronous(entry, what, mutate, metric_id, code):
+    assert _call(W.workload("C2"), mutate, metric_id, entry=entry) == code
+
+
+def test_manko_novikov_needs_spin_and_has_no_disk():
+    w = W.workload("C4")
+    assert _call(w, lambda m, c, g: setattr(m, "a", 0.0)) == api.GP_E_BAD_PARAM  # eq 23 divides by S/M
+    assert _call(w, lambda m, c, g: setattr(g, "max_crossings", 2)) == api.GP_E_UNSUPPORTED
+
+
+def test_buffer_checks():
+    w = W.workload("C3")
+    small = api.gp_out_buffers(C.c_void_p(0x1000), 63 * 128, C.c_void_p(0x2000), 64 * 48, C.c_void_p(0x3000), 64)
+    assert _call(w, out=small) == api.GP_E_SIZE
+    nodisk = api.gp_out_buffers(C.c_void_p(0x1000), 64 * 128, None, 0, C.c_void_p(0x3000), 64)
+    assert _call(w, out=nodisk) == api.GP_E_NULL
+    smalldisk = api.gp_out_buffers(C.c_void_p(0x1000), 64 * 128, C.c_void_p(0x2000), 10, C.c_void_p(0x3000), 64)
+    assert _call(w, out=smalldisk) == api.GP_E_SIZE
+    nocount = api.gp_out_buffers(C.c_void_p(0x1000), 64 * 128, C.c_void_p(0x2000), 64 * 48, None, 0)
+    assert _call(w, out=nocount) == api.GP_E_NULL
+    misaligned = api.gp_out_buffers(C.c_void_p(0x1008), 64 * 128, C.c_void_p(0x2000), 64 * 48, C.c_void_p(0x3000), 64)
+    assert _call(w, out=misaligned) == api.GP_E_BAD_PARAM
+    assert api.lib.gp_trace(1, None, None, None, None, None) == api.GP_E_NULL
+
+
+def _no_gpu():
+    try:
+        import torch
+        return not torch.cuda.is_available()
+    except Exception:
+        return True
+
+
+@pytest.mark.skipif(not _no_gpu(), reason="a GPU is present")
+def test_no_cpu_fallback_without_a_gpu():
+    """Valid arguments on a machine without a GPU: the call reports GP_E_CUDA; nothing is computed."""
+    w = W.workload("C2")
+    rays = np.zeros(64, dtype=api.RAY_DTYPE)
+    out = api.gp_out_buffers(C.c_void_p(rays.ctypes.data), rays.nbytes, None, 0, None, 0)
+    assert _call(w, out=out, entry="gp_trace_host") == api.GP_E_CUDA
+    assert "CUDA error" in gp.gp_strerror(api.GP_E_CUDA)
+    assert not rays.view(np.uint8).any()

@@ -1,0 +1,315 @@
+"""Parity of the CUDA path (through the C-ABI) against the CPU oracle on the same seeded inputs.
+
+Rules (R25 / R30; BASELINE.json north_star):
+  * image-plane points (row a2): bit-exact;
+  * capture / escape status: identical on every ray outside the flagged sets;
+  * raw exit theta, phi, lambda, t: |delta| <= 1e-9 max(1, |value|) on smooth rays
+    (controller-marginal rays, err_margin < 1e-5: 1e-6);
+  * |H| drift <= 1e-8 on escaped rays, on both sides.
+"""
+import copy
+import math
+
+import numpy as np
+import pytest
+
+import gp_workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-9
+FIELDS = ("theta", "phi", "lambda", "t")
+
+
+@pytest.fixture(scope="module")
+def gp():
+    import paper_2310_15183_b200 as gp
+    return gp
+
+
+@pytest.fixture(scope="module")
+def O():
+    from oracle import oracle as O
+    return O
+
+
+def run_both(gp, O, w, begin=0, count=None, stride=1):
+    b, c, s = W.ray_selection(w, begin, count, stride)
+    rays, disk, counters = gp.api.trace_workload(w, b, c, s)
+    orc, _ = O.trace(w, b, c, s)
+    assert len(rays) == len(orc) == c
+    assert counters[1] == c, "every ray must be finished exactly once"
+    return rays, disk, counters, orc
+
+
+def rel_err(g, o):
+    return np.abs(g - o) / np.maximum(1.0, np.abs(o))
+
+
+def check_parity(rays, orc, tol=TOL, marginal_tol=1e-6, max_status_mismatch=0, label=""):
+    """Element-by-element comparison; returns a dict of summary numbers."""
+    gs, os_ = rays["status"].astype(np.int64), orc["status"]
+    marginal = np.minimum(orc["err_margin"], rays["err_margin"]) < 1e-5
+    mism = gs != os_
+    assert np.count_nonzero(mism & ~marginal) <= max_status_mismatch, (
+        f"{label}: status differs on {np.count_nonzero(mism & ~marginal)} unflagged rays "
+        f"(first at {np.flatnonzero(mism & ~marginal)[:5]})")
+    same = ~mism
+    # exit state is defined (and unique) for escaped and captured rays; MAXSTEPS rays: status only (R21)
+    ended = same & (os_ <= 1)
+    worst = {}
+    for f in FIELDS:
+        e = rel_err(rays[f], orc[f])
+        smooth = ended & ~marginal
+        worst[f] = float(e[smooth].max()) if smooth.any() else 0.0
+        bad = smooth & ~(e <= tol)
+        assert not bad.any(), (f"{label}: {f} off by {e[bad].max():.3e} on {bad.sum()} smooth rays, "
+                               f"first {np.flatnonzero(bad)[:5]}")
+        badm = ended & marginal & ~(e <= marginal_tol)
+        assert not badm.any(), f"{label}: {f} off by {e[badm].max():.3e} on controller-marginal rays"
+    # exact on the exit surface, constants of the ray to rounding
+    assert np.array_equal(rays["r"][ended], orc["r"][ended])
+    for f in ("p_t", "p_phi"):
+        assert rel_err(rays[f], orc[f]).max() <= 1e-14, f
+    # step counters agree wherever the controller was never marginal
+    clean = ended & ~marginal
+    for f in ("n_accepted", "n_rejected", "n_equator_crossings", "n_disk_recorded", "n_rhs"):
+        d = rays[f][clean].astype(np.int64) != orc[f][clean]
+        assert d.mean() <= 1e-4 if d.size else True, f"{label}: {f} differs on {d.sum()} rays"
+    worst["marginal"] = int(marginal.sum())
+    worst["status_mismatch"] = int(mism.sum())
+    return worst
+
+
+def check_monitors(rays, orc, metric_id):
+    esc = (orc["status"] == 0) & (rays["status"] == 0)
+    assert rays["h_max"][esc].max() <= 1e-8 and orc["h_max"][esc].max() <= 1e-8
+    assert np.abs(rays["h_max"] - orc["h_max"])[esc].max() <= 1e-11
+    ok = orc["status"] <= 1
+    assert np.allclose(rays["sin_theta_min"][ok], orc["sin_theta_min"][ok], rtol=1e-8, atol=1e-12)
+    if metric_id != W.MANKO_NOVIKOV:
+        assert np.abs(rays["q_drift"] - orc["q_drift"])[esc].max() <= 1e-10
+
+
+# ---- row a2 / a3 ---------------------------------------------------------------------------------
+@pytest.mark.parametrize("name,extra", [("C1", {}), ("C2", {}), ("C4", {}),
+                                        ("C5a", dict(supersample=2, shift_x_px=1e-6, shift_y_px=1e-6)),
+                                        ("C2", dict(jitter_seed=12345, supersample=3))])
+def test_initial_conditions_bit_exact_alpha_beta(gp, O, name, extra):
+    import torch
+    w = W.workload(name, **extra)
+    b, c, s = W.ray_selection(w, 3, 5000, 977)
+    cam = gp.api.camera_struct(w["camera"], b, c, s)
+    st = torch.empty((c, 8), dtype=torch.float64, device="cuda")
+    ab = torch.empty((c, 2), dtype=torch.float64, device="cuda")
+    gp.gp_init_conditions(w["metric"]["id"], gp.api.metric_struct(w["metric"]), cam, st, ab)
+    torch.cuda.synchronize()
+    ab, st = ab.cpu().numpy(), st.cpu().numpy()
+    rays = b + s * np.arange(c)
+    ab_o = O.alpha_beta(w["camera"], rays)
+    assert np.array_equal(ab.view(np.uint64), ab_o.view(np.uint64)), "alpha, beta must be bit-exact"
+    for i in range(0, c, 37):
+        so = O.initial_state(w["metric"], w["camera"], ab_o[i, 0], ab_o[i, 1])
+        assert np.allclose(st[i], so, rtol=4e-16, atol=1e-18), (i, st[i], so)
+
+
+# ---- rows a4 / a5 --------------------------------------------------------------------------------
+METRICS = [dict(id=W.SCHWARZSCHILD, M=1.0, a=0.0, q=0.0), dict(id=W.KERR, M=1.0, a=0.9, q=0.0),
+           dict(id=W.KERR, M=1.3, a=-0.7, q=0.0), dict(id=W.MANKO_NOVIKOV, M=1.0, a=0.9, q=0.5),
+           dict(id=W.MANKO_NOVIKOV, M=1.0, a=0.5, q=-2.0), dict(id=W.MANKO_NOVIKOV, M=1.0, a=0.9, q=0.0)]
+
+
+def _points(n, seed, m):
+    rng = np.random.default_rng(seed)
+    rh = 2.0 * m["M"]
+    r = rh * (1.02 + np.exp(rng.uniform(math.log(0.02), math.log(600.0), n)))
+    th = rng.uniform(0.05, math.pi - 0.05, n)
+    return r, th
+
+
+@pytest.mark.parametrize("m", METRICS, ids=lambda m: f"id{m['id']}_a{m['a']}_q{m['q']}")
+def test_eval_metric_matches_oracle(gp, O, m):
+    import torch
+    n = 1500
+    r, th = _points(n, 1, m)
+    rt = torch.tensor(np.stack([r, th], 1), dtype=torch.float64, device="cuda")
+    out = torch.empty((n, 15), dtype=torch.float64, device="cuda")
+    gp.gp_eval_metric(m["id"], gp.api.metric_struct(m), rt, out)
+    torch.cuda.synchronize()
+    out = out.cpu().numpy()
+    ref = np.array([O.metric_inv(m, r[i], th[i]) for i in range(n)])
+    scale = np.maximum(np.abs(ref), np.abs(ref).max(axis=1, keepdims=True) * 1e-6)
+    err = np.abs(out - ref) / scale
+    # the oracle's complex-step MN derivatives lose a few digits near the horizon to cancellation
+    assert err.max() <= (5e-9 if m["id"] == W.MANKO_NOVIKOV else 1e-11), err.max()
+
+
+@pytest.mark.parametrize("m", METRICS, ids=lambda m: f"id{m['id']}_a{m['a']}_q{m['q']}")
+def test_eval_rhs_matches_oracle(gp, O, m):
+    import torch
+    n = 1500
+    r, th = _points(n, 2, m)
+    rng = np.random.default_rng(3)
+    st = np.zeros((n, 8))
+    st[:, 1], st[:, 2] = r, th
+    st[:, 4] = rng.uniform(0.5, 1.5, n)
+    st[:, 5] = rng.uniform(-1.5, 1.5, n)
+    st[:, 6] = rng.uniform(-8.0, 8.0, n)
+    st[:, 7] = rng.uniform(-8.0, 8.0, n)
+    d = torch.tensor(st, dtype=torch.float64, device="cuda")
+    out = torch.empty((n, 6), dtype=torch.float64, device="cuda")
+    gp.gp_eval_rhs(m["id"], gp.api.metric_struct(m), d, out)
+    torch.cuda.synchronize()
+    out = out.cpu().numpy()
+    ref = np.array([O.rhs(m, st[i]) for i in range(n)])
+    scale = np.maximum(np.abs(ref), np.abs(ref).max(axis=1, keepdims=True) * 1e-6)
+    err = np.abs(out - ref) / scale
+    assert err.max() <= (5e-9 if m["id"] == W.MANKO_NOVIKOV else 1e-11), err.max()
+
+
+# ---- whole path ----------------------------------------------------------------------------------
+def test_c1_schwarzschild_rk4_full(gp, O):
+    w = W.workload("C1")
+    rays, _, counters, orc = run_both(gp, O, w)
+    res = check_parity(rays, orc, label="C1")
+    check_monitors(rays, orc, W.SCHWARZSCHILD)
+    assert counters[3] == orc["n_rhs"].sum()
+    assert 0 < (orc["status"] == 1).sum() < len(orc)
+    print("C1 worst", res)
+
+
+def test_c2_kerr_dp54_full(gp, O):
+    w = W.workload("C2")
+    rays, _, counters, orc = run_both(gp, O, w)
+    res = check_parity(rays, orc, label="C2")
+    check_monitors(rays, orc, W.KERR)
+    assert counters[2] == (rays["n_accepted"].astype(np.int64) + rays["n_rejected"]).sum()
+    print("C2 worst", res)
+
+
+def test_c3_kerr_disk_subsample(gp, O):
+    w = W.workload("C3")
+    rays, disk, _, orc = run_both(gp, O, w, 5, None, 37)
+    res = check_parity(rays, orc, label="C3")
+    marginal = np.minimum(orc["err_margin"], rays["err_margin"]) < 1e-5
+    ok = (rays["status"] == orc["status"]) & ~marginal
+    n_rec = orc["n_disk_recorded"]
+    assert (n_rec > 0).sum() > 100 and n_rec.max() >= 2
+    for k in range(3):
+        have = ok & (n_rec > k)
+        assert np.array_equal(np.isnan(disk["r_cross"][ok, k]), np.isnan(orc["disk_r"][ok, k]))
+        assert rel_err(disk["r_cross"][have, k], orc["disk_r"][have, k]).max() <= TOL
+        assert rel_err(disk["g"][have, k], orc["disk_g"][have, k]).max() <= TOL
+    print("C3 worst", res, "rays with disk hits", int((n_rec > 0).sum()))
+
+
+def test_c4_manko_novikov_subsample(gp, O):
+    """Config 4 with the step budget cut to 4000 so that the oracle finishes the stalled interior
+    rays in seconds; MAXSTEPS rays are compared by status only (R21, R24)."""
+    w = W.workload("C4")
+    w["cfg"]["max_steps"] = 4000
+    rays, _, _, orc = run_both(gp, O, w, 11, None, 2039)
+    res = check_parity(rays, orc, label="C4", max_status_mismatch=2)
+    assert (orc["status"] == 2).sum() > 20 and (orc["status"] == 0).sum() > 1000
+    esc = (orc["status"] == 0) & (rays["status"] == 0)
+    assert rays["h_max"][esc].max() <= 1e-8
+    print("C4 worst", res)
+
+
+def test_mn_q0_reproduces_kerr_on_gpu(gp):
+    """BASELINE.json config 4: 'q=0 must reproduce Kerr' — through the CUDA path itself."""
+    wk = W.workload("C2")
+    wm = copy.deepcopy(wk)
+    wm["metric"] = dict(id=W.MANKO_NOVIKOV, M=1.0, a=0.9, q=0.0)
+    a, _, _ = gp.api.trace_workload(wk, 7, 3000, 83)
+    b, _, _ = gp.api.trace_workload(wm, 7, 3000, 83)
+    marginal = np.minimum(a["err_margin"], b["err_margin"]) < 1e-5
+    assert (a["status"] != b["status"])[~marginal].sum() == 0
+    ok = (a["status"] == b["status"]) & ~marginal
+    for f in FIELDS:
+        assert rel_err(a[f], b[f])[ok].max() <= TOL, f
+
+
+@pytest.mark.parametrize("name,stride", [("C5a", 16411), ("C5b", 65521)])
+def test_c5_fixed_relative_step_subsample(gp, O, name, stride):
+    w = W.workload(name)
+    w["cfg"]["max_steps"] = 20000
+    rays, _, _, orc = run_both(gp, O, w, 1, None, stride)
+    # near-axis rays (config 5a looks down the axis at 17 degrees) amplify rounding: R30
+    near_axis = orc["sin_theta_min"] < 1e-3
+    res = check_parity(rays[~near_axis], orc[~near_axis], tol=1e-8 if name == "C5b" else TOL, label=name,
+                       max_status_mismatch=1)
+    print(name, "worst", res, "near-axis", int(near_axis.sum()))
+
+
+# ---- edge cases ----------------------------------------------------------------------------------
+def test_empty_and_ragged_selections(gp, O):
+    w = W.workload("C2")
+    rays, _, counters = gp.api.trace_workload(w, 0, 0, 1)
+    assert len(rays) == 0 and counters[1] == 0
+    for count in (1, 31, 33, 1000):
+        rays, _, counters, orc = run_both(gp, O, w, 100003, count, 7)
+        check_parity(rays, orc, label=f"ragged {count}")
+
+
+def test_last_ray_of_the_image(gp, O):
+    w = W.workload("C2")
+    total = W.n_rays(w)
+    rays, _, _, orc = run_both(gp, O, w, total - 5, 5, 1)
+    check_parity(rays, orc, label="tail")
+
+
+def test_flat_space_closed_form_through_the_cuda_path(gp):
+    """Schwarzschild with M = 0 (Fig 6 situation): straight lines, closed-form exit."""
+    w = W.workload("C1")
+    w["metric"]["M"] = 0.0
+    w["camera"].update(theta_obs=1.1, phi_obs=0.4)
+    w["cfg"].update(scheme=2, rtol=1e-12, atol=1e-12, h_cap_rel=0.1, max_steps=100000)
+    rays, _, _ = gp.api.trace_workload(w)
+    import paper_2310_15183_b200 as G
+    import torch
+    cam = G.api.camera_struct(w["camera"])
+    ab = torch.empty((cam.ray_count, 2), dtype=torch.float64, device="cuda")
+    st = torch.empty((cam.ray_count, 8), dtype=torch.float64, device="cuda")
+    G.gp_init_conditions(0, G.api.metric_struct(w["metric"]), cam, st, ab)
+    ab = ab.cpu().numpy()
+    ro, resc = 50.0, 100.0
+    D = np.sqrt(ro * ro + (ab ** 2).sum(1))
+    lam = ro * ro / D + np.sqrt(ro ** 4 / D ** 2 + resc ** 2 - ro ** 2)
+    assert (rays["status"] == 0).all()
+    assert np.abs(rays["lambda"] - lam).max() <= 1e-8
+    assert np.abs(rays["t"] + lam).max() <= 1e-8
+    th0, ph0 = 1.1, 0.4
+    er = np.array([math.sin(th0) * math.cos(ph0), math.sin(th0) * math.sin(ph0), math.cos(th0)])
+    eth = np.array([math.cos(th0) * math.cos(ph0), math.cos(th0) * math.sin(ph0), -math.sin(th0)])
+    eph = np.array([-math.sin(ph0), math.cos(ph0), 0.0])
+    n = (-ro * er[None, :] - ab[:, 1:2] * eth[None, :] + ab[:, 0:1] * eph[None, :]) / D[:, None]
+    X = ro * er[None, :] + lam[:, None] * n
+    assert np.abs(np.cos(rays["theta"]) - X[:, 2] / resc).max() <= 1e-9
+    dphi = (rays["phi"] - np.arctan2(X[:, 1], X[:, 0]) + math.pi) % (2 * math.pi) - math.pi
+    assert np.abs(dphi).max() <= 1e-9
+
+
+def test_step_budget_and_host_entry(gp, O):
+    """max_steps = 0 and a tiny budget end as MAXSTEPS with the oracle's counters; gp_trace_host
+    returns the same records as gp_trace."""
+    w = W.workload("C2")
+    for budget in (0, 25):
+        w["cfg"]["max_steps"] = budget
+        rays, _, _, orc = run_both(gp, O, w, 0, 500, 523)
+        assert (rays["status"] == 2).all() and (orc["status"] == 2).all()
+        assert np.array_equal(rays["n_accepted"].astype(np.int64) + rays["n_rejected"],
+                              orc["n_accepted"] + orc["n_rejected"])
+        assert rel_err(rays["lambda"], orc["lambda"]).max() <= 1e-12
+    w = W.workload("C3")
+    b, c, s = W.ray_selection(w, 9, 4000, 263)
+    dev_r, dev_d, dev_c = gp.api.trace_workload(w, b, c, s)
+    host_r = np.zeros(c, dtype=gp.api.RAY_DTYPE)
+    host_d = np.zeros(c, dtype=gp.api.DISK_DTYPE)
+    host_c = np.zeros(8, dtype=np.uint64)
+    gp.gp_trace_host(w["metric"]["id"], gp.api.metric_struct(w["metric"]),
+                     gp.api.camera_struct(w["camera"], b, c, s), gp.api.cfg_struct(w["cfg"]),
+                     host_r, host_d, host_c)
+    assert host_r.tobytes() == dev_r.tobytes()
+    assert host_d.tobytes() == dev_d.tobytes()
+    assert np.array_equal(host_c[1:4], dev_c[1:4])
