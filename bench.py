@@ -1,0 +1,335 @@
+"""bench.py — throughput of the geodesic-tracing hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--impl reference]
+
+One "step" = one pass of the whole hot path (work fetch,
+pixel map, initial condition, metric + RHS, Runge-Kutta steps with control, termination and
+landing, monitors, record store) over one image of the workload, i.e. ONE launch of the
+persistent trace kernel through the C-ABI call gp_trace.  The default workload is `headline`:
+BASELINE.json configs[1] (Kerr a = 0.9, adaptive Dormand-Prince 5(4), rtol 1e-10) at
+1024 x 1024, the configuration BASELINE.json's `metric` is quoted on.
+
+Printed JSON line (rank 0): geodesics/s over all ranks (`value`), the same through
+gp_trace_host with pinned host buffers (`e2e`), the ALU roofline of the trace kernel
+(`roofline`), the oracle timed on the host cores on a bounded sample (`cpu_baseline`),
+the SM clocks sampled during the timed region (`clocks`).
+
+--impl reference times the CPU oracle as it stands (rank 0 only) on the same metric/config.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import gp_workloads as W  # noqa: E402
+
+# ---- algorithmic FP64 flop model (+,-,x = 1, FMA = 2, 1/x, sqrt, sin, cos,
+# exp, pow = 1 each), counted from the formulas of SURVEY.md appendix A/B as implemented ----------
+F_RHS = {W.SCHWARZSCHILD: 40.0, W.KERR: 81.0, W.MANKO_NOVIKOV: 760.0}
+F_STEP = {0: 56.0, 1: 57.0, 2: 324.0}
+# nominal FP64 FMA peak: 148 SMs x 64 FP64 FMA lanes x 2 flop x 1.965 GHz
+FP64_LANES_PER_SM = 64
+
+
+def _args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="headline")
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--cpu-seconds", type=float, default=12.0,
+                    help="target oracle time for the cpu_baseline sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+# ---- clocks during the timed region (B200_PROFILING.md recipe) ------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+    NAMES = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for ln in self.proc.stdout:
+            self.lines.append(ln)
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        self.thread.join(timeout=2)
+        sm, mx, pw, reasons = [], [], [], set()
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, v in zip(self.NAMES, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": max(mx), "power_w_max": max(pw),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def alg_flops(w, attempts, n_rhs):
+    """Algorithmic FP64 flops of a trace from its step and RHS counts."""
+    return F_RHS[w["metric"]["id"]] * float(n_rhs) + F_STEP[w["cfg"]["scheme"]] * float(attempts)
+
+
+def config_of(w, n_gpus, extra=None):
+    cam, cfg = w["camera"], w["cfg"]
+    c = {"workload": w["name"],
+         "metric_id": {0: "schwarzschild", 1: "kerr", 2: "manko_novikov"}[w["metric"]["id"]],
+         "a": w["metric"]["a"], "q": w["metric"]["q"],
+         "image": f"{cam['width']}x{cam['height']}x{cam['supersample']}^2",
+         "rays_per_step_per_gpu": W.n_rays(w),
+         "scheme": {0: "rk4_fixed", 1: "rk4_h_rel", 2: "dp54_adaptive"}[cfg["scheme"]],
+         "rtol": cfg["rtol"], "r_obs": cam["r_obs"],
+         "parallelism": f"frames{n_gpus}" if n_gpus > 1 else "single",
+         "l2": "each step writes 128 MiB of records (> 126 MB L2); the path reads no input arrays"}
+    if extra:
+        c.update(extra)
+    return c
+
+
+# ---- the oracle, timed (cpu_baseline leg and --impl reference) --------------------------------------
+def oracle_sample(w, seconds):
+    """Time the oracle on a scattered subsample of the workload sized for about `seconds`."""
+    from oracle import oracle as O
+    total = W.n_rays(w)
+    probe = min(total, 4096)
+    stride = max(1, total // probe) | 1
+    b, c, s = W.ray_selection(w, 1, probe, stride)
+    t0 = time.perf_counter()
+    _, used = O.trace(w, b, c, s)
+    rate = c / max(time.perf_counter() - t0, 1e-6)
+    count = int(min(total, max(probe, rate * seconds)))
+    stride = 1 if count >= total else (-(-total // count)) | 1   # odd stride: the sample scatters over the image
+    b, c, s = W.ray_selection(w, 0, None, stride)
+    t0 = time.perf_counter()
+    rec, used = O.trace(w, b, c, s)
+    dt = time.perf_counter() - t0
+    return {"value": c / dt, "unit": "geodesics/s", "cores": int(used), "kind": "oracle",
+            "sample": f"{c} rays of {w['name']} (every {s}th ray from ray {b}), {dt:.2f} s wall, "
+                      f"OpenMP dynamic over rays, g++ -O2 -ffp-contract=off",
+            "rhs_evals_per_s": float(rec["n_rhs"].sum()) / dt, "seconds": dt, "rays": c}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    w = W.workload(args.workload)
+    per_step = max(1.0, min(20.0, 150.0 / max(1, args.steps + args.warmup)))
+    for _ in range(args.warmup):
+        oracle_sample(w, per_step / 4)
+    rates, cpu, t_all = [], None, 0.0
+    rays = 0
+    for _ in range(args.steps):
+        cpu = oracle_sample(w, per_step)
+        rays += cpu["rays"]
+        t_all += cpu["seconds"]
+    value = rays / t_all
+    cpu = {k: cpu[k] for k in ("unit", "cores", "kind", "sample")}
+    cpu["value"] = value
+    print(json.dumps({
+        "impl": "reference", "metric": "geodesics/sec (1024^2 Kerr a=0.9, FP64)", "value": value,
+        "unit": "geodesics/s", "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * t_all / max(1, args.steps), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": config_of(w, 1, {"note": "each step = a bounded scattered sample of the image"}),
+        "cpu_baseline": cpu,
+        "e2e": {"value": value, "unit": "geodesics/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+# ---- the CUDA path ---------------------------------------------------------------------------------
+def run_b200(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    import paper_2310_15183_b200 as gp  # raises if libgp.so cannot be built/loaded: no fallback
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA library is the product, there is no CPU path")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    # weak scaling: every rank traces its own frame of the workload (its own jitter seed); rays are
+    # independent, so there is no exchange step
+    w = W.workload(args.workload)
+    w["camera"]["jitter_seed"] = int(w["camera"].get("jitter_seed", 0)) + rank
+    n = W.n_rays(w)
+    mid = w["metric"]["id"]
+    ms, cs, gs = gp.api.metric_struct(w["metric"]), gp.api.camera_struct(w["camera"]), gp.api.cfg_struct(w["cfg"])
+    disk_on = gs.max_crossings > 0
+    rays = torch.empty(n * 128, dtype=torch.uint8, device=dev)
+    disk = torch.empty(n * 48, dtype=torch.uint8, device=dev) if disk_on else None
+    counters = torch.zeros(64, dtype=torch.uint8, device=dev)
+    scratch = torch.zeros(8, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.Stream(device=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    def step():
+        gp.gp_trace(mid, ms, cs, gs, rays, disk, counters, stream)
+
+    def probe_peak():
+        """DFMA-chain probe (gp_probe_fp64_fma) -> TFLOP/s at the clocks of this moment."""
+        best = 0.0
+        with torch.cuda.stream(stream):
+            gp.gp_probe_fp64_fma(2000, scratch, stream)
+            for _ in range(3):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                fl = gp.gp_probe_fp64_fma(40000, scratch, stream)
+                e1.record(stream)
+                e1.synchronize()
+                best = max(best, fl / (e0.elapsed_time(e1) * 1e-3) / 1e12)
+        return best
+
+    with torch.cuda.stream(stream):
+        for _ in range(max(args.warmup, 3)):
+            step()
+    barrier()
+    peak_probe = probe_peak()
+
+    # ---- device-resident timed region: exactly K steps, CUDA events on the launching stream ----
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.3)
+    barrier()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    with torch.cuda.stream(stream):
+        ev[0].record(stream)
+        for i in range(args.steps):
+            step()
+            ev[i + 1].record(stream)
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    total_ms = ev[0].elapsed_time(ev[-1])
+    per_launch_ms = [ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps)]
+    cnt = counters.cpu().numpy().view("<u8")
+    assert int(cnt[1]) == n, "every ray must finish exactly once"
+    attempts, n_rhs = int(cnt[2]), int(cnt[3])
+    tmax = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    total_ms_max = float(tmax.item())
+
+    # ---- end to end: gp_trace_host into pinned host buffers (alloc + kernel + D2H + sync) ----
+    e2e = None
+    if not args.no_e2e:
+        h_rays = torch.empty(n * 128, dtype=torch.uint8, pin_memory=True).numpy().view(gp.api.RAY_DTYPE)
+        h_disk = (torch.empty(n * 48, dtype=torch.uint8, pin_memory=True).numpy().view(gp.api.DISK_DTYPE)
+                  if disk_on else None)
+        h_cnt = np.zeros(8, dtype=np.uint64)
+        for _ in range(2):
+            gp.gp_trace_host(mid, ms, cs, gs, h_rays, h_disk, h_cnt, stream)
+        barrier()
+        k_e2e = max(3, min(args.steps, 10))
+        t0 = time.perf_counter()
+        for _ in range(k_e2e):
+            gp.gp_trace_host(mid, ms, cs, gs, h_rays, h_disk, h_cnt, stream)  # synchronises the stream
+        torch.cuda.synchronize(dev)
+        dt = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(dt, op=dist.ReduceOp.MAX)
+        assert int(h_cnt[1]) == n and int((h_rays["status"] <= 4).sum()) == n
+        e2e = {"value": world * n * k_e2e / float(dt.item()), "unit": "geodesics/s",
+               "h2d_bytes_per_step": 24 + 120 + 112,  # the three parameter structs, as kernel arguments
+               "d2h_bytes_per_step": n * 128 + (n * 48 if disk_on else 0) + 64,
+               "steps": k_e2e, "call": "gp_trace_host (pinned host records, stream sync inside)"}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    sec = total_ms_max * 1e-3
+    value = world * n * args.steps / sec
+    kern_ms = sum(per_launch_ms) / len(per_launch_ms)
+    flops = alg_flops(w, attempts, n_rhs)
+    achieved = flops / (kern_ms * 1e-3) / 1e12
+    props = torch.cuda.get_device_properties(dev)
+    sm_max = (clocks or {}).get("sm_max_mhz") or 1965.0
+    peak_nominal = props.multi_processor_count * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+    out = {
+        "metric": "geodesics/sec (1024^2 Kerr a=0.9, FP64)" if args.workload == "headline"
+                  else f"geodesics/sec ({args.workload})",
+        "value": value, "unit": "geodesics/s", "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": total_ms_max / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "config": config_of(w, world),
+        "rhs_evals_per_s": world * n_rhs * args.steps / sec,
+        "steps_per_ray": attempts / n, "rhs_per_ray": n_rhs / n,
+        "roofline": {"bound": "alu", "kernel": "trace_dp54" if gs.scheme == 2 else "trace_rk4",
+                     "achieved": achieved, "peak": peak_nominal, "unit": "TFLOP/s",
+                     "frac": achieved / peak_nominal, "traffic": None,
+                     "peak_kind": f"nominal FP64 FMA: {props.multi_processor_count} SMs x "
+                                  f"{FP64_LANES_PER_SM} lanes x 2 x {sm_max:.0f} MHz",
+                     "peak_probe": peak_probe, "frac_of_probe": achieved / peak_probe if peak_probe else None,
+                     "probe_kind": "gp_probe_fp64_fma: register-resident DFMA chains, same process",
+                     "alg_flops_per_launch": flops, "kernel_ms": kern_ms,
+                     "flop_model": f"{F_RHS[mid]:.0f}/RHS + {F_STEP[gs.scheme]:.0f}/step (DESIGN.md 6.2)"},
+        "clocks": clocks, "gpu_launches": args.steps,
+    }
+    if e2e:
+        out["e2e"] = e2e
+    if not args.no_cpu_baseline and world == 1:
+        cpu = oracle_sample(w, args.cpu_seconds)
+        out["cpu_baseline"] = {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample", "rhs_evals_per_s")}
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    a = _args()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_b200(a)
