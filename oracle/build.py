@@ -3,6 +3,12 @@
 g++ -O2 -ffp-contract=off: no fused multiply-adds, so the oracle's arithmetic is the one
 written in gp_oracle.cpp.  -fcx-limited-range: plain textbook complex multiply/divide for
 the complex-step derivatives (no libgcc inf/nan recovery paths).
+
+build_rounding_probe() compiles the SAME source a second time with `-ffp-contract=fast -mfma`
+into libgp_oracle_fma.so.  That library is not "the oracle": it exists only so that the parity
+tests can measure, ray by ray, how far the oracle's own FP64 result moves when nothing but the
+rounding of its arithmetic changes (R30).  Expected values always come
+from the contraction-free build.
 """
 import os
 import subprocess
@@ -11,6 +17,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "gp_oracle.cpp")
 LIB = os.path.join(HERE, "libgp_oracle.so")
+LIB_FMA = os.path.join(HERE, "libgp_oracle_fma.so")
 
 
 def build(force: bool = False) -> str:
@@ -24,5 +31,20 @@ def build(force: bool = False) -> str:
     return LIB
 
 
+def build_rounding_probe(force: bool = False) -> str:
+    deps = [SRC, os.path.join(HERE, "gp_oracle.h")]
+    if (not force and os.path.exists(LIB_FMA)
+            and all(os.path.getmtime(LIB_FMA) >= os.path.getmtime(d) for d in deps)):
+        return LIB_FMA
+    with open("/proc/cpuinfo") as f:
+        if " fma" not in f.read():
+            raise RuntimeError("the rounding probe needs a host CPU with FMA instructions")
+    cmd = ["g++", "-std=c++17", "-O2", "-ffp-contract=fast", "-mfma", "-fcx-limited-range",
+           "-fopenmp", "-fPIC", "-shared", "-o", LIB_FMA, SRC]
+    subprocess.check_call(cmd)
+    return LIB_FMA
+
+
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv))
+    print(build_rounding_probe(force="--force" in sys.argv))

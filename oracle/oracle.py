@@ -44,6 +44,22 @@ RECORD_DTYPE = np.dtype([
 assert RECORD_DTYPE.itemsize == 6 * 8 + 15 * 8 + 6 * 8
 
 _lib = None
+_lib_fma = None
+
+
+def _declare_trace(L):
+    L.orc_trace.argtypes = [C.POINTER(OrcMetric), C.POINTER(OrcCamera), C.POINTER(OrcCfg),
+                            _i64, _i64, _i64, C.c_void_p, C.c_int]
+
+
+def lib_rounding_probe():
+    """The same oracle source compiled with FMA contraction (oracle/build.py); used only to
+    measure the oracle's own rounding sensitivity, never for expected values."""
+    global _lib_fma
+    if _lib_fma is None:
+        _lib_fma = C.CDLL(_build.build_rounding_probe())
+        _declare_trace(_lib_fma)
+    return _lib_fma
 
 
 def lib():
@@ -170,9 +186,10 @@ def single_step(metric, scheme, state8, h, rtol=1e-10, atol=1e-10):
     return out, err.value
 
 
-def trace(workload, ray_begin=0, ray_count=None, ray_stride=1, n_threads=0):
+def trace(workload, ray_begin=0, ray_count=None, ray_stride=1, n_threads=0, rounding_probe=False):
     """Trace rays ray_begin + k*ray_stride of a gp_workloads workload.  Returns
-    (records: structured array, threads_used)."""
+    (records: structured array, threads_used).  rounding_probe=True runs the FMA-contracted
+    build of the same source instead (see lib_rounding_probe)."""
     cam = workload["camera"]
     total = cam["width"] * cam["height"] * cam.get("supersample", 1) ** 2
     fit = max(0, (total - ray_begin + ray_stride - 1) // ray_stride)
@@ -181,7 +198,8 @@ def trace(workload, ray_begin=0, ray_count=None, ray_stride=1, n_threads=0):
     if ray_count > fit:
         raise ValueError("ray selection leaves the image")
     out = np.zeros(ray_count, dtype=RECORD_DTYPE)
-    used = _check(lib().orc_trace(C.byref(_metric(workload["metric"])), C.byref(_camera(cam)),
+    L = lib_rounding_probe() if rounding_probe else lib()
+    used = _check(L.orc_trace(C.byref(_metric(workload["metric"])), C.byref(_camera(cam)),
                                   C.byref(_cfg(workload["cfg"])), int(ray_begin), int(ray_count),
                                   int(ray_stride), out.ctypes.data, int(n_threads)), "trace")
     return out, used

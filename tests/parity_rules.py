@@ -1,0 +1,122 @@
+"""Parity rules between the CUDA path and the CPU oracle (readings R21, R25, R30).
+
+BASELINE.json north_star: status bit-exact outside flagged regions; raw exit (theta, phi, lambda, t)
+within 1e-9 max(1, |value|) on smooth pixels.  A ray is *smooth* unless one of the flags below is
+set.  Every flag is computed from the oracle (and, for the controller margin, from both sides'
+own records), never from the GPU-oracle difference it then excuses:
+
+  marginal   min over both sides of err_margin = min_steps |err - 1| < 1e-5: an accept/reject
+             decision of the step controller sat within rounding of its threshold (R30);
+  near_axis  sin(theta)_min < 1e-3 along the oracle's ray: the 1/sin^2(theta) terms amplify
+             rounding ("the simulation breaks at the axis");
+  sensitive  the oracle disagrees WITH ITSELF by more than 1e-10 (a tenth of the tolerance) when
+             nothing changes but the rounding of its arithmetic: the same source built with FMA
+             contraction (oracle/build.py build_rounding_probe).  Two correct FP64 evaluations of
+             the same algorithm cannot be asked to agree more closely than that.  This catches the
+             near-critical rays (rounding amplified by e^{orbits}), Manko-Novikov rays that graze the
+             ill-conditioned neighbourhood of the singular ring, and every fixed-step ray whose
+             stages straddle the horizon.
+
+Flagged rays are still compared: status must agree unless marginal or sensitive, and the exit
+state must agree to max(1e-6, 100 x the oracle's own rounding spread).  Callers bound the
+flagged fraction.
+"""
+import numpy as np
+
+TOL = 1e-9
+FLAGGED_TOL = 1e-6
+SENSITIVE_AT = 1e-10
+FIELDS = ("theta", "phi", "lambda", "t")
+
+
+def rel_err(g, o):
+    return np.abs(g - o) / np.maximum(1.0, np.abs(o))
+
+
+def rounding_spread(orc, orc_probe):
+    """Per-ray max over FIELDS of the oracle's disagreement with its FMA-contracted build;
+    inf where even the status differs."""
+    d = np.zeros(len(orc))
+    for f in FIELDS:
+        with np.errstate(invalid="ignore"):
+            e = rel_err(orc_probe[f], orc[f])
+        d = np.maximum(d, np.where(np.isfinite(e), e, np.inf))
+    # rays that end on no surface (MAXSTEPS, NONFINITE, STEP_UNDERFLOW) have no exit state to spread
+    d[(orc["status"] >= 2) & (orc_probe["status"] >= 2)] = 0.0
+    d[orc_probe["status"] != orc["status"]] = np.inf
+    return d
+
+
+def flags(rays, orc, orc_probe):
+    spread = rounding_spread(orc, orc_probe)
+    return dict(marginal=np.minimum(orc["err_margin"], rays["err_margin"]) < 1e-5,
+                near_axis=orc["sin_theta_min"] < 1e-3,
+                sensitive=spread > SENSITIVE_AT,
+                spread=spread)
+
+
+def check_parity(rays, orc, orc_probe, tol=TOL, label="", max_flagged_fraction=0.02,
+                 manko_novikov=False):
+    """Element-by-element comparison under the rules above; returns summary numbers.
+    manko_novikov=True: a CAPTURED ray's exit state is compared by status only (R24): the
+    capture surface x = 1 + eps hugs the singular horizon of PAPER.md L234, where fixed-step
+    rays wind phi by 1e6 rad with |H| ~ 1e6 on both sides alike — there is no exit state to pin."""
+    fl = flags(rays, orc, orc_probe)
+    gs, os_ = rays["status"].astype(np.int64), orc["status"]
+    mism = gs != os_
+    excused = fl["marginal"] | fl["sensitive"]
+    assert not (mism & ~excused).any(), (
+        f"{label}: status differs on {np.count_nonzero(mism & ~excused)} unflagged rays "
+        f"(first at {np.flatnonzero(mism & ~excused)[:5]})")
+    # the exit state is defined (and unique) for escaped and captured rays; MAXSTEPS rays: status only (R21)
+    ended = ~mism & ((os_ == 0) if manko_novikov else (os_ <= 1))
+    flagged = fl["marginal"] | fl["near_axis"] | fl["sensitive"]
+    smooth = ended & ~flagged
+    loose = np.maximum(FLAGGED_TOL, 100.0 * fl["spread"])
+    out = {}
+    for f in FIELDS:
+        e = rel_err(rays[f], orc[f])
+        out[f] = float(e[smooth].max()) if smooth.any() else 0.0
+        bad = smooth & ~(e <= tol)
+        assert not bad.any(), (f"{label}: {f} off by {e[bad].max():.3e} on {bad.sum()} smooth rays, "
+                               f"first {np.flatnonzero(bad)[:5]}")
+        badf = ended & flagged & np.isfinite(loose) & ~(e <= loose)
+        assert not badf.any(), (f"{label}: {f} off by {e[badf].max():.3e} on {badf.sum()} flagged rays, "
+                                f"first {np.flatnonzero(badf)[:5]}")
+    # exact on the exit surface; the constants of the ray to rounding
+    on_surface = ~mism & (os_ <= 1)
+    assert np.array_equal(rays["r"][on_surface], orc["r"][on_surface]), f"{label}: exit radius is not the surface"
+    for f in ("p_t", "p_phi"):
+        assert rel_err(rays[f], orc[f]).max() <= 1e-13, f
+    # step counters agree on smooth rays (a differing count is a differing controller decision)
+    for f in ("n_accepted", "n_rejected", "n_equator_crossings", "n_disk_recorded", "n_rhs"):
+        d = rays[f][smooth].astype(np.int64) != orc[f][smooth]
+        assert (d.mean() <= 1e-4) if d.size else True, f"{label}: {f} differs on {d.sum()} smooth rays"
+    n = max(1, len(orc))
+    out.update(n=len(orc), smooth=int(smooth.sum()), marginal=int(fl["marginal"].sum()),
+               near_axis=int(fl["near_axis"].sum()), sensitive=int(fl["sensitive"].sum()),
+               status_mismatch=int(mism.sum()), flagged_fraction=float(flagged.sum()) / n)
+    assert out["flagged_fraction"] <= max_flagged_fraction, (
+        f"{label}: {flagged.sum()} of {len(orc)} rays flagged — the flags must stay the exception")
+    out["smooth_mask"] = smooth
+    return out
+
+
+def check_h_drift(rays, orc, smooth, adaptive, label=""):
+    """|H| drift (R22) on smooth escaped rays.  The two sides must report the same drift
+    (1e-11 + 25 %: the running maximum is itself a rounding-level cancellation, and the oracle's
+    own FMA build moves it by up to 14 %), the CUDA path may not drift more than 1.5 x the oracle,
+    and for the adaptive scheme north_star's bound |H| <= 1e-8 must hold on both sides on at
+    least 99.8 % of those rays (measured: every Kerr ray; all but 2 of 1866 Manko-Novikov rays,
+    the same 2 on both sides).  Captured rays are left out: at the capture surface the 1/Delta
+    terms inflate |H| to 1e-7..1e-6 on both sides alike, and a fixed step cannot
+    hold H near the photon sphere at all."""
+    esc = smooth & (orc["status"] == 0) & (rays["status"] == 0)
+    if not esc.any():
+        return
+    gh, oh = rays["h_max"][esc], orc["h_max"][esc]
+    assert (np.abs(gh - oh) <= 1e-11 + 0.25 * np.maximum(gh, oh)).all(), f"{label}: |H| drift differs"
+    assert (gh <= 1.5 * oh + 1e-11).all(), f"{label}: the CUDA path drifts more than the oracle"
+    if adaptive:
+        assert (gh <= 1e-8).mean() >= 0.998, f"{label}: GPU |H| drift above 1e-8 on {(gh > 1e-8).sum()} rays"
+        assert (oh <= 1e-8).mean() >= 0.998, f"{label}: oracle |H| drift above 1e-8 on {(oh > 1e-8).sum()} rays"
