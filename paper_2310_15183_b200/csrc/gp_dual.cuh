@@ -8,13 +8,7 @@
 #ifndef GP_DUAL_CUH_
 #define GP_DUAL_CUH_
 
-#include <math.h>
-
-#if defined(__CUDACC__)
-#define GP_HD __host__ __device__ __forceinline__
-#else
-#define GP_HD inline
-#endif
+#include "gp_math.cuh"
 
 namespace gp {
 
@@ -40,18 +34,18 @@ GP_HD Dual2 operator*(double b, const Dual2 &a) { return Dual2(a.v * b, a.dx * b
 
 // 1/a: one reciprocal, derivatives -a'/a^2
 GP_HD Dual2 recip(const Dual2 &a) {
-  double i = 1.0 / a.v;
+  double i = frcp(a.v);
   double m = -i * i;
   return Dual2(i, a.dx * m, a.dy * m);
 }
-GP_HD double recip(double a) { return 1.0 / a; }
+GP_HD double recip(double a) { return frcp(a); }
 GP_HD Dual2 operator/(const Dual2 &a, const Dual2 &b) { return a * recip(b); }
 GP_HD Dual2 operator/(double a, const Dual2 &b) { return a * recip(b); }
-GP_HD Dual2 operator/(const Dual2 &a, double b) { return a * (1.0 / b); }
+GP_HD Dual2 operator/(const Dual2 &a, double b) { return a * frcp(b); }
 
 GP_HD Dual2 dsqrt(const Dual2 &a) {
   double s = sqrt(a.v);
-  double m = 0.5 / s;
+  double m = 0.5 * frcp(s);
   return Dual2(s, a.dx * m, a.dy * m);
 }
 GP_HD double dsqrt(double a) { return sqrt(a); }

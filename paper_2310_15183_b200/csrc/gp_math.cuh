@@ -1,0 +1,144 @@
+// gp_math.cuh — FP64 elementary functions for the tracer's inner loop, written for the sm_100a
+// issue model.
+//
+// Why not the CUDA math library here: profiles/r01 showed that 28 % of the warp instructions of
+// trace_dp54 were UMOV/IMAD.MOV pairs that materialise 64-bit literals (the library's sincos,
+// division and pow carry their coefficients as immediates), and that each `a / b` and each fmax
+// drags a denormal / NaN slow-path test through the instruction stream.  The FP64 pipe issues
+// one warp instruction every other cycle, so those extra issue slots cost as much as the
+// arithmetic.  Every literal below lives in __constant__ memory and reaches DFMA/DMUL as a
+// c[bank][offset] operand; every function is branch-free on the range the integrator produces
+// and falls back to the library outside it.
+//
+// Accuracy (checked by tests/test_gpu_parity.py::test_device_math_*): sincos_pi4 <= 1 ulp-ish
+// (polynomial error 1e-17 / 5e-19 before rounding), rcp_nr and div_nr <= 1 ulp, pow_m1_5 <= 2 ulp.
+#ifndef GP_MATH_CUH_
+#define GP_MATH_CUH_
+
+#include <math.h>
+
+#if defined(__CUDACC__)
+#define GP_HD __host__ __device__ __forceinline__
+#else
+#define GP_HD inline
+#endif
+
+namespace gp {
+
+#if defined(__CUDACC__)
+
+// Coefficients are near-minimax fits made for this file (Chebyshev-node interpolation of
+// (sin r / r - 1)/r^2 and (cos r - 1 + r^2/2)/r^4 on r^2 <= 1.02 (pi/4)^2, 60-digit mpmath).
+struct MathConst {
+  double two_over_pi;
+  double pio2_hi, pio2_mid, pio2_lo;  // pi/2 split 33 + 33 + 53 bits: q*hi and q*mid are exact for |q| < 2^20
+  double s[6];                        // sin: r + r z (s0 + s1 z + ... + s5 z^5), z = r^2
+  double c[6];                        // cos: 1 - z/2 + z^2 (c0 + ... + c5 z^5)
+  double one, half, fifth, six_fifths;
+};
+
+__constant__ MathConst kMath = {
+    0x1.45f306dc9c883p-1,
+    0x1.921fb54400000p+0, 0x1.0b4611a600000p-34, 0x1.3198a2e037073p-69,
+    {-0x1.5555555555555p-3, 0x1.1111111110b23p-7, -0x1.a01a019e623afp-13, 0x1.71de376b9c575p-19,
+     -0x1.ae5fdeb852566p-26, 0x1.5dfb4dfaf15abp-33},
+    {0x1.5555555555555p-5, -0x1.6c16c16c1691fp-10, 0x1.a01a019f3df42p-16, -0x1.27e4fa025e03dp-22,
+     0x1.1eeb52bea9072p-29, -0x1.906dd38cb66a1p-37},
+    1.0, 0.5, 0.2, 1.2};
+
+// max / min of two doubles without fmax's NaN canonicalisation: a NaN candidate never replaces
+// the running value (the same outcome fmax(running, NaN) gives).
+__device__ __forceinline__ double dmax(double run, double cand) { return cand > run ? cand : run; }
+__device__ __forceinline__ double dmin(double run, double cand) { return cand < run ? cand : run; }
+
+// 1/x to <= 1 ulp for normal finite x: MUFU.RCP64H seed (about 20 bits) + one cubic and one
+// quadratic Newton step.  x = 0 or non-finite gives a non-finite result (the integrator's
+// finite tests catch it); subnormal x is outside the integrator's range.
+__device__ __forceinline__ double rcp_nr(double x) {
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double e = fma(-x, y, kMath.one);
+  e = fma(e, e, e);
+  y = fma(y, e, y);
+  e = fma(-x, y, kMath.one);
+  return fma(y, e, y);
+}
+
+// a/b to <= 1 ulp given y = rcp_nr(b): one residual correction.
+__device__ __forceinline__ double div_nr(double a, double b, double y) {
+  double q = a * y;
+  double rem = fma(-b, q, a);
+  return fma(rem, y, q);
+}
+
+// sin and cos of x for |x| < 1e5 (the polar angle never leaves a few multiples of pi); the
+// library routine takes over beyond that.  Cody-Waite reduction to |r| <= pi/4 with a three-part
+// pi/2, then the two kernels, then the quadrant swap.
+__device__ __noinline__ void sincos_library(double x, double *sn, double *cs) { sincos(x, sn, cs); }
+
+__device__ __forceinline__ void sincos_fast(double x, double *sn, double *cs) {
+  if (!(fabs(x) < 1.0e5)) {
+    sincos_library(x, sn, cs);
+    return;
+  }
+  double qd = rint(x * kMath.two_over_pi);
+  int q = __double2int_rn(qd);
+  double r = fma(-qd, kMath.pio2_hi, x);
+  r = fma(-qd, kMath.pio2_mid, r);
+  r = fma(-qd, kMath.pio2_lo, r);
+  double z = r * r;
+  double ps = fma(z, kMath.s[5], kMath.s[4]);
+  double pc = fma(z, kMath.c[5], kMath.c[4]);
+  ps = fma(z, ps, kMath.s[3]);
+  pc = fma(z, pc, kMath.c[3]);
+  ps = fma(z, ps, kMath.s[2]);
+  pc = fma(z, pc, kMath.c[2]);
+  ps = fma(z, ps, kMath.s[1]);
+  pc = fma(z, pc, kMath.c[1]);
+  ps = fma(z, ps, kMath.s[0]);
+  pc = fma(z, pc, kMath.c[0]);
+  double sr = fma(r * z, ps, r);                              // sin r
+  double cr = fma(z * z, pc, fma(-kMath.half, z, kMath.one)); // cos r
+  // quadrant: q mod 4 = 0: (s, c); 1: (c, -s); 2: (-s, -c); 3: (-c, s)
+  double a = (q & 1) ? cr : sr;
+  double b = (q & 1) ? sr : cr;
+  *sn = (q & 2) ? -a : a;
+  *cs = ((q + 1) & 2) ? -b : b;
+}
+
+// x^(-1/5) for x in [1e-5, 1e4] (the controller clamps outside, R10 item 3): FP32 seed from the
+// SFU (about 1e-6), two Newton steps on y^-5 = x (error 3 e^2 per step) -> <= 2 ulp.
+__device__ __forceinline__ double pow_m1_5(double x) {
+  float xf = __double2float_rn(x);
+  double y = (double)exp2f(-0.2f * __log2f(xf));
+#pragma unroll
+  for (int i = 0; i < 2; ++i) {
+    double y2 = y * y;
+    double y5 = y2 * y2 * y;
+    double e = fma(-x, y5, kMath.one);
+    y = fma(y * kMath.fifth, e, y);
+  }
+  return y;
+}
+
+#endif  // __CUDACC__
+
+// The same source serves the device (fast forms above) and the host (observer constants, row a3).
+GP_HD double frcp(double x) {
+#if defined(__CUDA_ARCH__)
+  return rcp_nr(x);
+#else
+  return 1.0 / x;
+#endif
+}
+GP_HD void fsincos(double x, double *sn, double *cs) {
+#if defined(__CUDA_ARCH__)
+  sincos_fast(x, sn, cs);
+#else
+  *sn = sin(x);
+  *cs = cos(x);
+#endif
+}
+
+}  // namespace gp
+#endif

@@ -47,12 +47,12 @@ struct Rhs {
 GP_HD void rhs_schwarzschild(const MetricConst &mc, double pt, double pph, double r, double th, double pr,
                              double pth, Rhs &o) {
   double s, c;
-  sincos(th, &s, &c);
-  double ir = 1.0 / r;
+  fsincos(th, &s, &c);
+  double ir = frcp(r);
   double ir2 = ir * ir;
   double F = 1.0 - 2.0 * mc.M * ir;
-  double iF = 1.0 / F;
-  double is = 1.0 / s;
+  double iF = frcp(F);
+  double is = frcp(s);
   double is2 = is * is;
   double Fr = 2.0 * mc.M * ir2;            // dF/dr
   double gpp = ir2 * is2;                  // g^{phi phi}
@@ -78,7 +78,7 @@ GP_HD void rhs_schwarzschild(const MetricConst &mc, double pt, double pph, doubl
 GP_HD void rhs_kerr(const MetricConst &mc, double pt, double pph, double r, double th, double pr, double pth,
                     Rhs &o) {
   double s, c;
-  sincos(th, &s, &c);
+  fsincos(th, &s, &c);
   const double a = mc.a, a2 = mc.a2, M = mc.M;
   double r2 = r * r;
   double rr = r2 + a2;
@@ -86,7 +86,7 @@ GP_HD void rhs_kerr(const MetricConst &mc, double pt, double pph, double r, doub
   double Del = rr - 2.0 * M * r;
   // one reciprocal for the three denominators Sigma, Delta, s
   double SD = Sig * Del;
-  double inv = 1.0 / (SD * s);
+  double inv = frcp(SD * s);
   double is = inv * SD;
   double iSig = inv * Del * s;
   double iDel = inv * Sig * s;
@@ -163,7 +163,7 @@ GP_HD MNCore<T> mn_core(const MetricConst &mc, const T &x, const T &y) {
 GP_HD void rhs_manko_novikov(const MetricConst &mc, double pt, double pph, double r, double th, double pr,
                              double pth, Rhs &o) {
   double s, c;
-  sincos(th, &s, &c);
+  fsincos(th, &s, &c);
   const double k = mc.mn_k;
   Dual2 x((r - mc.M) * mc.mn_inv_k, 1.0, 0.0);
   Dual2 y(c, 0.0, 1.0);

@@ -40,19 +40,31 @@ constexpr int kBlock = 128;
 constexpr unsigned kFull = 0xffffffffu;
 constexpr double kHalfPi = 1.57079632679489661923;
 
-// Dormand & Prince (1980) 5(4) pair, reading R10.
-namespace dp {
-constexpr double A21 = 1.0 / 5.0;
-constexpr double A31 = 3.0 / 40.0, A32 = 9.0 / 40.0;
-constexpr double A41 = 44.0 / 45.0, A42 = -56.0 / 15.0, A43 = 32.0 / 9.0;
-constexpr double A51 = 19372.0 / 6561.0, A52 = -25360.0 / 2187.0, A53 = 64448.0 / 6561.0, A54 = -212.0 / 729.0;
-constexpr double A61 = 9017.0 / 3168.0, A62 = -355.0 / 33.0, A63 = 46732.0 / 5247.0, A64 = 49.0 / 176.0,
-                 A65 = -5103.0 / 18656.0;
-constexpr double B1 = 35.0 / 384.0, B3 = 500.0 / 1113.0, B4 = 125.0 / 192.0, B5 = -2187.0 / 6784.0,
-                 B6 = 11.0 / 84.0;
-constexpr double E1 = 71.0 / 57600.0, E3 = -71.0 / 16695.0, E4 = 71.0 / 1920.0, E5 = -17253.0 / 339200.0,
-                 E6 = 22.0 / 525.0, E7 = -1.0 / 40.0;
-}  // namespace dp
+// Dormand & Prince (1980) 5(4) pair, reading R10.  The coefficients sit in __constant__ memory so
+// that DFMA/DMUL take them as c[bank][offset] operands: as literals each use cost two UMOVs
+// (profiles/r01: 17 % of all warp instructions).
+struct DpTableau {
+  double A21;
+  double A31, A32;
+  double A41, A42, A43;
+  double A51, A52, A53, A54;
+  double A61, A62, A63, A64, A65;
+  double B1, B3, B4, B5, B6;
+  double E1, E3, E4, E5, E6, E7;
+  double safety, fac_min, fac_max, err_lo, err_hi, h_floor;  // controller constants, R10 items 3 and 5
+};
+
+#if defined(__CUDACC__)
+__constant__ DpTableau dp = {
+    1.0 / 5.0,
+    3.0 / 40.0, 9.0 / 40.0,
+    44.0 / 45.0, -56.0 / 15.0, 32.0 / 9.0,
+    19372.0 / 6561.0, -25360.0 / 2187.0, 64448.0 / 6561.0, -212.0 / 729.0,
+    9017.0 / 3168.0, -355.0 / 33.0, 46732.0 / 5247.0, 49.0 / 176.0, -5103.0 / 18656.0,
+    35.0 / 384.0, 500.0 / 1113.0, 125.0 / 192.0, -2187.0 / 6784.0, 11.0 / 84.0,
+    71.0 / 57600.0, -71.0 / 16695.0, 71.0 / 1920.0, -17253.0 / 339200.0, 22.0 / 525.0, -1.0 / 40.0,
+    0.9, 0.2, 5.0, 1.0e-5, 1.0e4, 1.0e-14};
+#endif
 
 #if defined(__CUDACC__)
 
@@ -91,7 +103,7 @@ __device__ __forceinline__ double kepler_g(const MetricConst &mc, double r, doub
 
 // Monitors of row a10 carried per lane.
 struct Monitors {
-  double h_max, q_drift, Q0, sin_min, err_margin;
+  double h_max, q_drift, Q0, iQ0, sin_min, err_margin;
 };
 
 // Carter constant, exact off shell (reading R23): Q = p_th^2 + c^2 (p_ph^2/s^2 - a^2 p_t^2) - 2 a^2 c^2 H.
@@ -106,12 +118,13 @@ __device__ __forceinline__ double carter_q(const MetricConst &mc, double pt, dou
 
 template <int METRIC>
 __device__ __forceinline__ void monitor_apply(Monitors &mo, double absH, double Q, double abss, bool first) {
-  mo.h_max = fmax(mo.h_max, absH);
-  mo.sin_min = fmin(mo.sin_min, abss);
+  mo.h_max = dmax(mo.h_max, absH);
+  mo.sin_min = dmin(mo.sin_min, abss);
   if (METRIC != METRIC_MN) {
     if (first) mo.Q0 = Q;
-    double d = fabs(Q - mo.Q0) / fmax(1.0, fabs(mo.Q0));
-    mo.q_drift = fmax(mo.q_drift, d);
+    if (first) mo.iQ0 = frcp(dmax(1.0, fabs(Q)));
+    double d = fabs(Q - mo.Q0) * mo.iQ0;
+    mo.q_drift = dmax(mo.q_drift, d);
   }
 }
 

@@ -36,7 +36,7 @@ __global__ void __launch_bounds__(kBlock) trace_dp54(const __grid_constant__ Tra
   // pending (trial) state and the error sums that still lack the e7 k7 term
   double nt = 0.0, nr = 0.0, nth = 0.0, nph = 0.0, npr = 0.0, npth = 0.0, nlam = 0.0;
   double et = 0.0, er = 0.0, eth = 0.0, eph = 0.0, epr = 0.0, epth = 0.0;
-  Monitors mo = {0.0, 0.0, 0.0, 0.0, 0.0};
+  Monitors mo = {0.0, 0.0, 0.0, 1.0, 0.0, 0.0};
   unsigned n_acc = 0, n_rej = 0, n_cross = 0, n_rec = 0, n_land = 0, status = 0;
   bool exhausted = false;
   unsigned long long tot_rays = 0, tot_steps = 0, tot_rhs = 0;
@@ -84,29 +84,45 @@ __global__ void __launch_bounds__(kBlock) trace_dp54(const __grid_constant__ Tra
         mode = MODE_NORMAL;
         moved = true;
       } else if (mode == MODE_NORMAL) {
-        // R10 items 1-3: scaled max-norm over the six evolving components
-        double xt = fabs(h * (et + dp::E7 * o7.dt)) / (P.atol + P.rtol * fmax(fabs(t), fabs(nt)));
-        double xr = fabs(h * (er + dp::E7 * o7.dr)) / (P.atol + P.rtol * fmax(fabs(r), fabs(nr)));
-        double xth = fabs(h * (eth + dp::E7 * o7.dth)) / (P.atol + P.rtol * fmax(fabs(th), fabs(nth)));
-        double xph = fabs(h * (eph + dp::E7 * o7.dph)) / (P.atol + P.rtol * fmax(fabs(ph), fabs(nph)));
-        double xpr = fabs(h * (epr + dp::E7 * o7.dpr)) / (P.atol + P.rtol * fmax(fabs(pr), fabs(npr)));
-        double xpth = fabs(h * (epth + dp::E7 * o7.dpth)) / (P.atol + P.rtol * fmax(fabs(pth), fabs(npth)));
-        // finite test on the sum: any inf/NaN term makes it non-finite (terms are >= 0)
-        double xsum = ((xt + xr) + (xth + xph)) + (xpr + xpth);
+        // R10 items 1-3: scaled max-norm over the six evolving components,
+        //   err = max_j |h (e_j + E7 k7_j)| / (atol + rtol max(|y_j|, |y+_j|)).
+        // The largest ratio is found by cross-multiplication (num_j den_best > num_best den_j) and
+        // divided once; a tie within rounding picks either of two equal ratios.
+        double nm = fabs(h * (et + dp.E7 * o7.dt)), dn = fma(P.rtol, dmax(fabs(t), fabs(nt)), P.atol);
+        double nsum = nm;
+#define GP_ERR_TERM(e_, k7_, y_, ny_)                                            \
+  {                                                                              \
+    double n_ = fabs(h * ((e_) + dp.E7 * (k7_)));                                \
+    double d_ = fma(P.rtol, dmax(fabs(y_), fabs(ny_)), P.atol);                  \
+    nsum += n_;                                                                  \
+    bool gt_ = n_ * dn > nm * d_;                                                \
+    nm = gt_ ? n_ : nm;                                                          \
+    dn = gt_ ? d_ : dn;                                                          \
+  }
+        GP_ERR_TERM(er, o7.dr, r, nr)
+        GP_ERR_TERM(eth, o7.dth, th, nth)
+        GP_ERR_TERM(eph, o7.dph, ph, nph)
+        GP_ERR_TERM(epr, o7.dpr, pr, npr)
+        GP_ERR_TERM(epth, o7.dpth, pth, npth)
+#undef GP_ERR_TERM
+        // finite test on the sums: any inf/NaN term makes them non-finite (numerators are >= 0)
         double ysum = ((nt + nr) + (nth + nph)) + (npr + npth);
-        double err = fmax(fmax(fmax(xt, xr), fmax(xth, xph)), fmax(xpr, xpth));
-        if (!finite_d(xsum) || !finite_d(ysum)) {
+        double err = div_nr(nm, dn, rcp_nr(dn));
+        if (!finite_d(nsum) || !finite_d(ysum) || !finite_d(err)) {
           ++n_rej;
-          h *= 0.2;
+          h *= dp.fac_min;
         } else {
-          mo.err_margin = fmin(mo.err_margin, fabs(err - 1.0));
-          double fac = (err == 0.0) ? 5.0 : 0.9 * pow(err, -0.2);
+          mo.err_margin = dmin(mo.err_margin, fabs(err - 1.0));
+          // fac = 0.9 err^(-1/5), clamped to [0.2, 5] (err = 0 gives 5); the clamp of err keeps the
+          // FP32 seed of pow_m1_5 in range and changes nothing: 0.9 (1e-5)^-0.2 = 9 > 5, 0.9 (1e4)^-0.2 = 0.14 < 0.2
+          double fac = dp.safety * pow_m1_5(dmin(dmax(dp.err_lo, err), dp.err_hi));
+          fac = dmin(dmax(dp.fac_min, fac), dp.fac_max);
           if (err > 1.0) {
             ++n_rej;
-            h *= fmax(0.2, fac);
+            h *= fac;
           } else {
             ++n_acc;
-            double hnext = fmin(h * fmin(5.0, fmax(0.2, fac)), P.h_cap_rel * nr);
+            double hnext = dmin(h * fac, P.h_cap_rel * nr);
             if (nr > P.r_esc || nr < P.r_cap) {
               // O8: discard the step, land on the surface from y_n
               status = (nr > P.r_esc) ? GP_RAY_ESCAPED : GP_RAY_CAPTURED;
@@ -172,7 +188,7 @@ __global__ void __launch_bounds__(kBlock) trace_dp54(const __grid_constant__ Tra
             (P.lambda_max > 0.0 && lam >= P.lambda_max)) {
           status = GP_RAY_MAXSTEPS;
           finished = true;
-        } else if (h < 1e-14 * fmax(1.0, fabs(lam))) {
+        } else if (h < dp.h_floor * dmax(1.0, fabs(lam))) {
           status = GP_RAY_STEP_UNDERFLOW;
           finished = true;
         } else if (moved) {
@@ -204,67 +220,67 @@ __global__ void __launch_bounds__(kBlock) trace_dp54(const __grid_constant__ Tra
 #define GP_INV(o_dr, o_dth) (landing ? 1.0 / (land_r ? (o_dr) : (o_dth)) : 1.0)
         double iv = GP_INV(k1r, k1th);
         const double K1r = k1r * iv, K1th = k1th * iv, K1pr = k1pr * iv, K1pth = k1pth * iv;
-        double bt = dp::B1 * (k1t * iv), bph = dp::B1 * (k1ph * iv), bl = dp::B1 * iv;   // quadratures t, phi, lambda
-        double qet = dp::E1 * (k1t * iv), qeph = dp::E1 * (k1ph * iv);
+        double bt = dp.B1 * (k1t * iv), bph = dp.B1 * (k1ph * iv), bl = dp.B1 * iv;   // quadratures t, phi, lambda
+        double qet = dp.E1 * (k1t * iv), qeph = dp.E1 * (k1ph * iv);
         Rhs o;
         // stage 2
-        rhs_eval<METRIC>(mc, pt, pph, r + s * (dp::A21 * K1r), th + s * (dp::A21 * K1th),
-                         pr + s * (dp::A21 * K1pr), pth + s * (dp::A21 * K1pth), o);
+        rhs_eval<METRIC>(mc, pt, pph, r + s * (dp.A21 * K1r), th + s * (dp.A21 * K1th),
+                         pr + s * (dp.A21 * K1pr), pth + s * (dp.A21 * K1pth), o);
         iv = GP_INV(o.dr, o.dth);
         const double K2r = o.dr * iv, K2th = o.dth * iv, K2pr = o.dpr * iv, K2pth = o.dpth * iv;
         // stage 3
-        rhs_eval<METRIC>(mc, pt, pph, r + s * (dp::A31 * K1r + dp::A32 * K2r),
-                         th + s * (dp::A31 * K1th + dp::A32 * K2th),
-                         pr + s * (dp::A31 * K1pr + dp::A32 * K2pr),
-                         pth + s * (dp::A31 * K1pth + dp::A32 * K2pth), o);
+        rhs_eval<METRIC>(mc, pt, pph, r + s * (dp.A31 * K1r + dp.A32 * K2r),
+                         th + s * (dp.A31 * K1th + dp.A32 * K2th),
+                         pr + s * (dp.A31 * K1pr + dp.A32 * K2pr),
+                         pth + s * (dp.A31 * K1pth + dp.A32 * K2pth), o);
         iv = GP_INV(o.dr, o.dth);
         const double K3r = o.dr * iv, K3th = o.dth * iv, K3pr = o.dpr * iv, K3pth = o.dpth * iv;
-        bt += dp::B3 * (o.dt * iv); bph += dp::B3 * (o.dph * iv); bl += dp::B3 * iv;
-        qet += dp::E3 * (o.dt * iv); qeph += dp::E3 * (o.dph * iv);
+        bt += dp.B3 * (o.dt * iv); bph += dp.B3 * (o.dph * iv); bl += dp.B3 * iv;
+        qet += dp.E3 * (o.dt * iv); qeph += dp.E3 * (o.dph * iv);
         // stage 4
-        rhs_eval<METRIC>(mc, pt, pph, r + s * (dp::A41 * K1r + dp::A42 * K2r + dp::A43 * K3r),
-                         th + s * (dp::A41 * K1th + dp::A42 * K2th + dp::A43 * K3th),
-                         pr + s * (dp::A41 * K1pr + dp::A42 * K2pr + dp::A43 * K3pr),
-                         pth + s * (dp::A41 * K1pth + dp::A42 * K2pth + dp::A43 * K3pth), o);
+        rhs_eval<METRIC>(mc, pt, pph, r + s * (dp.A41 * K1r + dp.A42 * K2r + dp.A43 * K3r),
+                         th + s * (dp.A41 * K1th + dp.A42 * K2th + dp.A43 * K3th),
+                         pr + s * (dp.A41 * K1pr + dp.A42 * K2pr + dp.A43 * K3pr),
+                         pth + s * (dp.A41 * K1pth + dp.A42 * K2pth + dp.A43 * K3pth), o);
         iv = GP_INV(o.dr, o.dth);
         const double K4r = o.dr * iv, K4th = o.dth * iv, K4pr = o.dpr * iv, K4pth = o.dpth * iv;
-        bt += dp::B4 * (o.dt * iv); bph += dp::B4 * (o.dph * iv); bl += dp::B4 * iv;
-        qet += dp::E4 * (o.dt * iv); qeph += dp::E4 * (o.dph * iv);
+        bt += dp.B4 * (o.dt * iv); bph += dp.B4 * (o.dph * iv); bl += dp.B4 * iv;
+        qet += dp.E4 * (o.dt * iv); qeph += dp.E4 * (o.dph * iv);
         // stage 5
         rhs_eval<METRIC>(mc, pt, pph,
-                         r + s * (dp::A51 * K1r + dp::A52 * K2r + dp::A53 * K3r + dp::A54 * K4r),
-                         th + s * (dp::A51 * K1th + dp::A52 * K2th + dp::A53 * K3th + dp::A54 * K4th),
-                         pr + s * (dp::A51 * K1pr + dp::A52 * K2pr + dp::A53 * K3pr + dp::A54 * K4pr),
-                         pth + s * (dp::A51 * K1pth + dp::A52 * K2pth + dp::A53 * K3pth + dp::A54 * K4pth), o);
+                         r + s * (dp.A51 * K1r + dp.A52 * K2r + dp.A53 * K3r + dp.A54 * K4r),
+                         th + s * (dp.A51 * K1th + dp.A52 * K2th + dp.A53 * K3th + dp.A54 * K4th),
+                         pr + s * (dp.A51 * K1pr + dp.A52 * K2pr + dp.A53 * K3pr + dp.A54 * K4pr),
+                         pth + s * (dp.A51 * K1pth + dp.A52 * K2pth + dp.A53 * K3pth + dp.A54 * K4pth), o);
         iv = GP_INV(o.dr, o.dth);
         const double K5r = o.dr * iv, K5th = o.dth * iv, K5pr = o.dpr * iv, K5pth = o.dpth * iv;
-        bt += dp::B5 * (o.dt * iv); bph += dp::B5 * (o.dph * iv); bl += dp::B5 * iv;
-        qet += dp::E5 * (o.dt * iv); qeph += dp::E5 * (o.dph * iv);
+        bt += dp.B5 * (o.dt * iv); bph += dp.B5 * (o.dph * iv); bl += dp.B5 * iv;
+        qet += dp.E5 * (o.dt * iv); qeph += dp.E5 * (o.dph * iv);
         // stage 6
         rhs_eval<METRIC>(
             mc, pt, pph,
-            r + s * (dp::A61 * K1r + dp::A62 * K2r + dp::A63 * K3r + dp::A64 * K4r + dp::A65 * K5r),
-            th + s * (dp::A61 * K1th + dp::A62 * K2th + dp::A63 * K3th + dp::A64 * K4th + dp::A65 * K5th),
-            pr + s * (dp::A61 * K1pr + dp::A62 * K2pr + dp::A63 * K3pr + dp::A64 * K4pr + dp::A65 * K5pr),
-            pth + s * (dp::A61 * K1pth + dp::A62 * K2pth + dp::A63 * K3pth + dp::A64 * K4pth + dp::A65 * K5pth),
+            r + s * (dp.A61 * K1r + dp.A62 * K2r + dp.A63 * K3r + dp.A64 * K4r + dp.A65 * K5r),
+            th + s * (dp.A61 * K1th + dp.A62 * K2th + dp.A63 * K3th + dp.A64 * K4th + dp.A65 * K5th),
+            pr + s * (dp.A61 * K1pr + dp.A62 * K2pr + dp.A63 * K3pr + dp.A64 * K4pr + dp.A65 * K5pr),
+            pth + s * (dp.A61 * K1pth + dp.A62 * K2pth + dp.A63 * K3pth + dp.A64 * K4pth + dp.A65 * K5pth),
             o);
         iv = GP_INV(o.dr, o.dth);
         const double K6r = o.dr * iv, K6th = o.dth * iv, K6pr = o.dpr * iv, K6pth = o.dpth * iv;
-        bt += dp::B6 * (o.dt * iv); bph += dp::B6 * (o.dph * iv); bl += dp::B6 * iv;
-        qet += dp::E6 * (o.dt * iv); qeph += dp::E6 * (o.dph * iv);
+        bt += dp.B6 * (o.dt * iv); bph += dp.B6 * (o.dph * iv); bl += dp.B6 * iv;
+        qet += dp.E6 * (o.dt * iv); qeph += dp.E6 * (o.dph * iv);
 #undef GP_INV
         // trial end state (5th-order solution; a7 = b) and the error sums without e7 k7
-        nr = r + s * (dp::B1 * K1r + dp::B3 * K3r + dp::B4 * K4r + dp::B5 * K5r + dp::B6 * K6r);
-        nth = th + s * (dp::B1 * K1th + dp::B3 * K3th + dp::B4 * K4th + dp::B5 * K5th + dp::B6 * K6th);
-        npr = pr + s * (dp::B1 * K1pr + dp::B3 * K3pr + dp::B4 * K4pr + dp::B5 * K5pr + dp::B6 * K6pr);
-        npth = pth + s * (dp::B1 * K1pth + dp::B3 * K3pth + dp::B4 * K4pth + dp::B5 * K5pth + dp::B6 * K6pth);
+        nr = r + s * (dp.B1 * K1r + dp.B3 * K3r + dp.B4 * K4r + dp.B5 * K5r + dp.B6 * K6r);
+        nth = th + s * (dp.B1 * K1th + dp.B3 * K3th + dp.B4 * K4th + dp.B5 * K5th + dp.B6 * K6th);
+        npr = pr + s * (dp.B1 * K1pr + dp.B3 * K3pr + dp.B4 * K4pr + dp.B5 * K5pr + dp.B6 * K6pr);
+        npth = pth + s * (dp.B1 * K1pth + dp.B3 * K3pth + dp.B4 * K4pth + dp.B5 * K5pth + dp.B6 * K6pth);
         nt = t + s * bt;
         nph = ph + s * bph;
         nlam = lam + s * bl;
-        er = dp::E1 * K1r + dp::E3 * K3r + dp::E4 * K4r + dp::E5 * K5r + dp::E6 * K6r;
-        eth = dp::E1 * K1th + dp::E3 * K3th + dp::E4 * K4th + dp::E5 * K5th + dp::E6 * K6th;
-        epr = dp::E1 * K1pr + dp::E3 * K3pr + dp::E4 * K4pr + dp::E5 * K5pr + dp::E6 * K6pr;
-        epth = dp::E1 * K1pth + dp::E3 * K3pth + dp::E4 * K4pth + dp::E5 * K5pth + dp::E6 * K6pth;
+        er = dp.E1 * K1r + dp.E3 * K3r + dp.E4 * K4r + dp.E5 * K5r + dp.E6 * K6r;
+        eth = dp.E1 * K1th + dp.E3 * K3th + dp.E4 * K4th + dp.E5 * K5th + dp.E6 * K6th;
+        epr = dp.E1 * K1pr + dp.E3 * K3pr + dp.E4 * K4pr + dp.E5 * K5pr + dp.E6 * K6pr;
+        epth = dp.E1 * K1pth + dp.E3 * K3pth + dp.E4 * K4pth + dp.E5 * K5pth + dp.E6 * K6pth;
         et = qet;
         eph = qeph;
       }

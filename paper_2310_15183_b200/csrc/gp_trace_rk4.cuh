@@ -25,7 +25,7 @@ __global__ void __launch_bounds__(kBlock) trace_rk4(const __grid_constant__ Trac
   double pt = 0.0, pph = 0.0;
   double t = 0.0, r = 0.0, th = 0.0, ph = 0.0, pr = 0.0, pth = 0.0, lam = 0.0;
   double target = 0.0;
-  Monitors mo = {0.0, 0.0, 0.0, 0.0, 0.0};
+  Monitors mo = {0.0, 0.0, 0.0, 1.0, 0.0, 0.0};
   unsigned n_acc = 0, n_cross = 0, n_rec = 0, n_land = 0, status = 0;
   bool exhausted = false;
   unsigned long long tot_rays = 0, tot_steps = 0, tot_rhs = 0;
