@@ -48,6 +48,7 @@ int make_metric(int metric_id, const gp_metric_params *m, MetricConst *mc) {
   mc->a = a;
   mc->q = q;
   mc->a2 = a * a;
+  mc->m2M = -2.0 * M;
   mc->r_horizon = (metric_id == GP_SCHWARZSCHILD) ? 2.0 * M : M + sqrt(M * M - a * a);
   if (metric_id == GP_MANKO_NOVIKOV) {
     double al = (-M + sqrt(M * M - a * a)) / a;          // eq 23
@@ -170,7 +171,7 @@ int launch_one(const TraceParams &P, cudaStream_t stream) {
   static int blocks_dp = 0, blocks_rk = 0;
   static int n_sm = 0;
   const bool dp54 = (P.scheme == 2);
-  const size_t smem = DISK ? sizeof(double) * kBlock * (dp54 ? kParkSlotsDp54 : kParkSlotsRk4) : 0;
+  const size_t smem = dp54 ? dp54_smem_bytes(DISK) : (DISK ? sizeof(double) * kBlock * kParkSlotsRk4 : 0);
   int &per_sm = dp54 ? blocks_dp : blocks_rk;
   if (per_sm == 0) {
     int dev = 0;
@@ -182,6 +183,11 @@ int launch_one(const TraceParams &P, cudaStream_t stream) {
     else
       GP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, trace_rk4<METRIC, DISK>, kBlock, smem));
     if (occ < 1) occ = 1;
+    // tuning aid: GP_BLOCKS_PER_SM caps the resident blocks per SM (never raises them)
+    if (const char *cap = getenv("GP_BLOCKS_PER_SM")) {
+      int c = atoi(cap);
+      if (c >= 1 && c < occ) occ = c;
+    }
     per_sm = occ;
   }
   // persistent grid: every SM filled to its resident-block limit, never more lanes than rays

@@ -24,6 +24,7 @@ enum { METRIC_SCHW = 0, METRIC_KERR = 1, METRIC_MN = 2 };
 struct MetricConst {
   double M, a, q;
   double a2;        // a^2
+  double m2M;       // -2M
   double r_horizon; // 2M | M + sqrt(M^2-a^2) | M + k
   // Manko-Novikov, PAPER.md L192-196 (eq 23-25), reading R7
   double mn_alpha;  // (-M + sqrt(M^2-a^2))/a
@@ -75,35 +76,43 @@ GP_HD void rhs_schwarzschild(const MetricConst &mc, double pt, double pph, doubl
 //   Sigma = r^2 + a^2 c^2, Delta = r^2 - 2Mr + a^2,
 //   P = (r^2+a^2) p_t + a p_ph,  W = p_ph/s + a s p_t,
 //   N = Delta p_r^2 + p_th^2 + W^2 - P^2/Delta,   2H = N/Sigma.
+// Written out operation by operation (half-derivatives, shared products, explicit fma): 53 FP64
+// instructions beside the sincos and the reciprocal, against 61 for the textbook arrangement — the
+// FP64 pipe is the bound, so the operation count is the run time.
 GP_HD void rhs_kerr(const MetricConst &mc, double pt, double pph, double r, double th, double pr, double pth,
                     Rhs &o) {
   double s, c;
   fsincos(th, &s, &c);
-  const double a = mc.a, a2 = mc.a2, M = mc.M;
+  const double a = mc.a, a2 = mc.a2;
   double r2 = r * r;
   double rr = r2 + a2;
-  double Sig = r2 + a2 * c * c;
-  double Del = rr - 2.0 * M * r;
+  double a2c = a2 * c;
+  double Sig = fma(a2c, c, r2);
+  double Del = fma(mc.m2M, r, rr);
   // one reciprocal for the three denominators Sigma, Delta, s
   double SD = Sig * Del;
   double inv = frcp(SD * s);
   double is = inv * SD;
-  double iSig = inv * Del * s;
-  double iDel = inv * Sig * s;
-  double P = rr * pt + a * pph;
-  double W = pph * is + a * s * pt;
+  double t1 = inv * s;
+  double iSig = t1 * Del;
+  double iDel = t1 * Sig;
+  double as = a * s;
+  double W = fma(pph, is, as * pt);
+  double P = fma(rr, pt, a * pph);
   double PiD = P * iDel;
-  double N = Del * pr * pr + pth * pth + W * W - P * PiD;
+  double pr2 = pr * pr;
+  double N = fma(-P, PiD, fma(W, W, fma(pth, pth, Del * pr2)));
   double H2 = N * iSig;
-  o.dt = (a * s * W - rr * PiD) * iSig;
-  o.dph = (W * is - a * PiD) * iSig;
-  o.dr = Del * pr * iSig;
+  o.dt = fma(-rr, PiD, as * W) * iSig;
+  o.dph = fma(-a, PiD, W * is) * iSig;
+  o.dr = (pr * iSig) * Del;
   o.dth = pth * iSig;
-  double rm = r - M;
-  double dNr = 2.0 * (rm * (pr * pr + PiD * PiD) - 2.0 * r * pt * PiD);
-  o.dpr = -0.5 * iSig * (dNr - 2.0 * r * H2);
-  double dNth = 2.0 * W * c * (a * pt - pph * is * is);
-  o.dpth = -0.5 * iSig * (dNth + 2.0 * a2 * s * c * H2);
+  // dp_r = -(1/2 d_r N - r 2H)/Sigma,  1/2 d_r N = (r-M)(p_r^2 + (P/Delta)^2) - 2 r p_t P/Delta
+  double halfNr = fma(-2.0, (r * pt) * PiD, (r - mc.M) * fma(PiD, PiD, pr2));
+  o.dpr = fma(r, H2, -halfNr) * iSig;
+  // dp_th = -(1/2 d_th N + a^2 s c 2H)/Sigma,  1/2 d_th N = W c (a p_t - p_ph/s^2)
+  double halfNth = (W * c) * fma(-(pph * is), is, a * pt);
+  o.dpth = -fma(a2c * s, H2, halfNth) * iSig;
   o.H2 = H2;
   o.s = s;
   o.c = c;

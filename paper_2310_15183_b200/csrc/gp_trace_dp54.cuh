@@ -15,31 +15,75 @@
 namespace gp {
 #if defined(__CUDACC__)
 
-// Shared-memory parking lot for the state a ray resumes from after an equator landing step:
-// trial state (r, th, pr, pth, t, ph, lambda), next step, raw k7 (6) and its monitor triple.
+// Shared-memory plan, per lane.  Registers hold only what every stage
+// touches; the rest lives in shared memory so that five blocks (20 warps) fit per SM:
+//   K area   8 x double2   stage slopes K2..K5 of (r, th) and (p_r, p_th); K1 and the newest K stay
+//                          in registers.  128-bit accesses, [slot][lane] layout: conflict-free.
+//   cold     kColdSlots x double   state the stages never read: t, phi, lambda, the monitors, the
+//                          landing target, k1 of the two quadratures, the per-lane totals.
+//   park     17 x double   (DISK only) what a ray resumes from after an equator landing step:
+//                          trial state (r, th, pr, pth, t, ph, lambda), next step, raw k7 (6) and
+//                          its monitor triple.
+enum { C_T = 0, C_PH, C_LAM, C_HMAX, C_QDRIFT, C_Q0, C_IQ0, C_SINMIN, C_MARGIN, C_TARGET, C_K1T, C_K1PH,
+       C_TOT_RAYS, C_TOT_STEPS, C_TOT_RHS, kColdSlots };
+constexpr int kKSlots2 = 8;
 constexpr int kParkSlotsDp54 = 17;
+constexpr size_t dp54_smem_bytes(bool disk) {
+  return sizeof(double) * kBlock * (2 * kKSlots2 + kColdSlots + (disk ? kParkSlotsDp54 : 0));
+}
+// Resident blocks per SM the register allocation is held to (4 -> <= 128 registers, no spills for
+// Schwarzschild and Kerr; the Manko-Novikov duals need 2 -> <= 255).  Measured on B200 (headline):
+// 3 blocks 48.7, 4 blocks 51.6, 5 blocks (70 B of spills) 49.6 M geodesics/s.
+#ifndef GP_DP54_MIN_BLOCKS
+#define GP_DP54_MIN_BLOCKS 4
+#endif
+#ifndef GP_DP54_MIN_BLOCKS_MN
+#define GP_DP54_MIN_BLOCKS_MN 2
+#endif
+
+// Shared-memory accessors by 32-bit shared-window address.  asm volatile keeps every access (the
+// compiler would otherwise forward the stored K's back into registers and spill) and their order.
+__device__ __forceinline__ void sts1(unsigned a, double x) {
+  asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(x));
+}
+__device__ __forceinline__ double lds1(unsigned a) {
+  double x;
+  asm volatile("ld.shared.f64 %0, [%1];" : "=d"(x) : "r"(a));
+  return x;
+}
+__device__ __forceinline__ void sts2(unsigned a, double x, double y) {
+  asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(a), "d"(x), "d"(y));
+}
+__device__ __forceinline__ void lds2(unsigned a, double &x, double &y) {
+  asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(x), "=d"(y) : "r"(a));
+}
 
 template <int METRIC, bool DISK>
-__global__ void __launch_bounds__(kBlock) trace_dp54(const __grid_constant__ TraceParams P) {
-  extern __shared__ double park[];  // [kParkSlotsDp54][kBlock] when DISK
+__global__ void __launch_bounds__(kBlock, METRIC == METRIC_MN ? GP_DP54_MIN_BLOCKS_MN : GP_DP54_MIN_BLOCKS)
+trace_dp54(const __grid_constant__ TraceParams P) {
+  extern __shared__ double2 smem2[];
   const MetricConst &mc = P.mc;
   const int tid = threadIdx.x;
+  const unsigned sm_k = (unsigned)__cvta_generic_to_shared(smem2) + 16u * tid;                  // + 16 kBlock slot
+  const unsigned sm_c = (unsigned)__cvta_generic_to_shared(smem2 + kKSlots2 * kBlock) + 8u * tid;  // + 8 kBlock slot
+  const unsigned sm_p = sm_c + 8u * kBlock * kColdSlots;
+#define KS(slot) (sm_k + 16u * kBlock * (slot))
+#define CS(slot) (sm_c + 8u * kBlock * (slot))
+#define PS(slot) (sm_p + 8u * kBlock * (slot))
 
   // ---- per-lane ray state (registers) ----
   int mode = MODE_IDLE;
   long long slot = -1;
   double pt = 0.0, pph = 0.0;                         // constants of the ray
-  double t = 0.0, r = 0.0, th = 0.0, ph = 0.0, pr = 0.0, pth = 0.0, lam = 0.0;  // y_n
-  double k1t = 0.0, k1r = 0.0, k1th = 0.0, k1ph = 0.0, k1pr = 0.0, k1pth = 0.0;  // raw F(y_n)
+  double r = 0.0, th = 0.0, pr = 0.0, pth = 0.0;      // y_n, the part Hamilton's equations read
+  double k1r = 0.0, k1th = 0.0, k1pr = 0.0, k1pth = 0.0;  // raw F(y_n), same part
   double h = 0.0;                                     // step of the attempt in flight / next attempt
-  double target = 0.0;                                // landing target
   // pending (trial) state and the error sums that still lack the e7 k7 term
   double nt = 0.0, nr = 0.0, nth = 0.0, nph = 0.0, npr = 0.0, npth = 0.0, nlam = 0.0;
   double et = 0.0, er = 0.0, eth = 0.0, eph = 0.0, epr = 0.0, epth = 0.0;
-  Monitors mo = {0.0, 0.0, 0.0, 1.0, 0.0, 0.0};
   unsigned n_acc = 0, n_rej = 0, n_cross = 0, n_rec = 0, n_land = 0, status = 0;
   bool exhausted = false;
-  unsigned long long tot_rays = 0, tot_steps = 0, tot_rhs = 0;
+  sts1(CS(C_TOT_RAYS), 0.0); sts1(CS(C_TOT_STEPS), 0.0); sts1(CS(C_TOT_RHS), 0.0);
 
   for (;;) {
     // ---- a1: refill idle lanes ----
@@ -59,9 +103,9 @@ __global__ void __launch_bounds__(kBlock) trace_dp54(const __grid_constant__ Tra
           nt = 0.0; nr = P.cc.r_obs; nth = P.cc.theta_obs; nph = P.cc.phi_obs; nlam = 0.0;
           mode = MODE_FRESH;
           n_acc = n_rej = n_cross = n_rec = n_land = 0;
-          mo.h_max = 0.0; mo.q_drift = 0.0; mo.Q0 = 0.0;
-          mo.sin_min = __longlong_as_double(0x7ff0000000000000LL);
-          mo.err_margin = __longlong_as_double(0x7ff0000000000000LL);
+          const double inf = __longlong_as_double(0x7ff0000000000000LL);
+          sts1(CS(C_HMAX), 0.0); sts1(CS(C_QDRIFT), 0.0); sts1(CS(C_Q0), 0.0); sts1(CS(C_IQ0), 1.0);
+          sts1(CS(C_SINMIN), inf); sts1(CS(C_MARGIN), inf);
         }
       }
     }
@@ -76,14 +120,19 @@ __global__ void __launch_bounds__(kBlock) trace_dp54(const __grid_constant__ Tra
       bool finished = false;
       bool moved = false;   // y_n changed: run the stop tests' monitor on the new state
       double monH = 0.0, monQ = 0.0, monS = 0.0;
+      double lam = 0.0;     // lambda of y_n, valid after this block when mode == MODE_NORMAL
       if (mode == MODE_FRESH) {
-        t = nt; r = nr; th = nth; ph = nph; pr = npr; pth = npth; lam = nlam;
-        k1t = o7.dt; k1r = o7.dr; k1th = o7.dth; k1ph = o7.dph; k1pr = o7.dpr; k1pth = o7.dpth;
+        r = nr; th = nth; pr = npr; pth = npth; lam = nlam;
+        sts1(CS(C_T), nt); sts1(CS(C_PH), nph); sts1(CS(C_LAM), nlam);
+        k1r = o7.dr; k1th = o7.dth; k1pr = o7.dpr; k1pth = o7.dpth;
+        sts1(CS(C_K1T), o7.dt); sts1(CS(C_K1PH), o7.dph);
         h = P.h_cap_rel * P.cc.r_obs;       // R10 item 4
         monH = fabs(0.5 * o7.H2); monQ = carter_q<METRIC>(mc, pt, pph, npth, o7); monS = fabs(o7.s);
         mode = MODE_NORMAL;
         moved = true;
       } else if (mode == MODE_NORMAL) {
+        const double t = lds1(CS(C_T)), ph = lds1(CS(C_PH));
+        lam = lds1(CS(C_LAM));
         // R10 items 1-3: scaled max-norm over the six evolving components,
         //   err = max_j |h (e_j + E7 k7_j)| / (atol + rtol max(|y_j|, |y+_j|)).
         // The largest ratio is found by cross-multiplication (num_j den_best > num_best den_j) and
@@ -112,7 +161,7 @@ __global__ void __launch_bounds__(kBlock) trace_dp54(const __grid_constant__ Tra
           ++n_rej;
           h *= dp.fac_min;
         } else {
-          mo.err_margin = dmin(mo.err_margin, fabs(err - 1.0));
+          sts1(CS(C_MARGIN), dmin(lds1(CS(C_MARGIN)), fabs(err - 1.0)));
           // fac = 0.9 err^(-1/5), clamped to [0.2, 5] (err = 0 gives 5); the clamp of err keeps the
           // FP32 seed of pow_m1_5 in range and changes nothing: 0.9 (1e-5)^-0.2 = 9 > 5, 0.9 (1e4)^-0.2 = 0.14 < 0.2
           double fac = dp.safety * pow_m1_5(dmin(dmax(dp.err_lo, err), dp.err_hi));
@@ -126,7 +175,7 @@ __global__ void __launch_bounds__(kBlock) trace_dp54(const __grid_constant__ Tra
             if (nr > P.r_esc || nr < P.r_cap) {
               // O8: discard the step, land on the surface from y_n
               status = (nr > P.r_esc) ? GP_RAY_ESCAPED : GP_RAY_CAPTURED;
-              target = (nr > P.r_esc) ? P.r_esc : P.r_cap;
+              sts1(CS(C_TARGET), (nr > P.r_esc) ? P.r_esc : P.r_cap);
               mode = MODE_LAND_R;
             } else {
               bool commit = true;
@@ -134,23 +183,24 @@ __global__ void __launch_bounds__(kBlock) trace_dp54(const __grid_constant__ Tra
                 ++n_cross;
                 if (DISK && n_rec < (unsigned)P.max_crossings) {
                   // O7: locate the crossing from y_n; resume from the parked trial state afterwards
-                  double *pk = park + tid;
-                  pk[0 * kBlock] = nr; pk[1 * kBlock] = nth; pk[2 * kBlock] = npr; pk[3 * kBlock] = npth;
-                  pk[4 * kBlock] = nt; pk[5 * kBlock] = nph; pk[6 * kBlock] = lam + h; pk[7 * kBlock] = hnext;
-                  pk[8 * kBlock] = o7.dt; pk[9 * kBlock] = o7.dr; pk[10 * kBlock] = o7.dth;
-                  pk[11 * kBlock] = o7.dph; pk[12 * kBlock] = o7.dpr; pk[13 * kBlock] = o7.dpth;
-                  pk[14 * kBlock] = fabs(0.5 * o7.H2);
-                  pk[15 * kBlock] = carter_q<METRIC>(mc, pt, pph, npth, o7);
-                  pk[16 * kBlock] = fabs(o7.s);
-                  target = kHalfPi;
+                  sts1(PS(0), nr); sts1(PS(1), nth); sts1(PS(2), npr); sts1(PS(3), npth);
+                  sts1(PS(4), nt); sts1(PS(5), nph); sts1(PS(6), lam + h); sts1(PS(7), hnext);
+                  sts1(PS(8), o7.dt); sts1(PS(9), o7.dr); sts1(PS(10), o7.dth);
+                  sts1(PS(11), o7.dph); sts1(PS(12), o7.dpr); sts1(PS(13), o7.dpth);
+                  sts1(PS(14), fabs(0.5 * o7.H2));
+                  sts1(PS(15), carter_q<METRIC>(mc, pt, pph, npth, o7));
+                  sts1(PS(16), fabs(o7.s));
+                  sts1(CS(C_TARGET), kHalfPi);
                   mode = MODE_LAND_TH;
                   commit = false;
                 }
               }
               if (commit) {
                 monH = fabs(0.5 * o7.H2); monQ = carter_q<METRIC>(mc, pt, pph, npth, o7); monS = fabs(o7.s);
-                t = nt; r = nr; th = nth; ph = nph; pr = npr; pth = npth; lam += h;
-                k1t = o7.dt; k1r = o7.dr; k1th = o7.dth; k1ph = o7.dph; k1pr = o7.dpr; k1pth = o7.dpth;
+                r = nr; th = nth; pr = npr; pth = npth; lam += h;
+                sts1(CS(C_T), nt); sts1(CS(C_PH), nph); sts1(CS(C_LAM), lam);
+                k1r = o7.dr; k1th = o7.dth; k1pr = o7.dpr; k1pth = o7.dpth;
+                sts1(CS(C_K1T), o7.dt); sts1(CS(C_K1PH), o7.dph);
                 h = hnext;
                 moved = true;
               }
@@ -159,7 +209,8 @@ __global__ void __launch_bounds__(kBlock) trace_dp54(const __grid_constant__ Tra
         }
       } else if (mode == MODE_LAND_R) {
         // landed on the exit surface: the record is the landed state (R14)
-        t = nt; r = target; th = nth; ph = nph; pr = npr; pth = npth; lam = nlam;
+        r = lds1(CS(C_TARGET)); th = nth; pr = npr; pth = npth;
+        sts1(CS(C_T), nt); sts1(CS(C_PH), nph); sts1(CS(C_LAM), nlam);
         ++n_land;
         finished = true;
       } else {  // MODE_LAND_TH
@@ -171,12 +222,12 @@ __global__ void __launch_bounds__(kBlock) trace_dp54(const __grid_constant__ Tra
             P.disk[slot].g[n_rec] = kepler_g(mc, rc, pt, pph);
             ++n_rec;
           }
-          const double *pk = park + tid;
-          r = pk[0 * kBlock]; th = pk[1 * kBlock]; pr = pk[2 * kBlock]; pth = pk[3 * kBlock];
-          t = pk[4 * kBlock]; ph = pk[5 * kBlock]; lam = pk[6 * kBlock]; h = pk[7 * kBlock];
-          k1t = pk[8 * kBlock]; k1r = pk[9 * kBlock]; k1th = pk[10 * kBlock];
-          k1ph = pk[11 * kBlock]; k1pr = pk[12 * kBlock]; k1pth = pk[13 * kBlock];
-          monH = pk[14 * kBlock]; monQ = pk[15 * kBlock]; monS = pk[16 * kBlock];
+          r = lds1(PS(0)); th = lds1(PS(1)); pr = lds1(PS(2)); pth = lds1(PS(3));
+          lam = lds1(PS(6)); h = lds1(PS(7));
+          sts1(CS(C_T), lds1(PS(4))); sts1(CS(C_PH), lds1(PS(5))); sts1(CS(C_LAM), lam);
+          sts1(CS(C_K1T), lds1(PS(8))); sts1(CS(C_K1PH), lds1(PS(11)));
+          k1r = lds1(PS(9)); k1th = lds1(PS(10)); k1pr = lds1(PS(12)); k1pth = lds1(PS(13));
+          monH = lds1(PS(14)); monQ = lds1(PS(15)); monS = lds1(PS(16));
         }
         mode = MODE_NORMAL;
         moved = true;
@@ -192,15 +243,25 @@ __global__ void __launch_bounds__(kBlock) trace_dp54(const __grid_constant__ Tra
           status = GP_RAY_STEP_UNDERFLOW;
           finished = true;
         } else if (moved) {
+          Monitors mo;
+          mo.h_max = lds1(CS(C_HMAX)); mo.q_drift = lds1(CS(C_QDRIFT)); mo.Q0 = lds1(CS(C_Q0));
+          mo.iQ0 = lds1(CS(C_IQ0)); mo.sin_min = lds1(CS(C_SINMIN)); mo.err_margin = 0.0;
           monitor_apply<METRIC>(mo, monH, monQ, monS, n_acc == 0 && n_rej == 0);
+          sts1(CS(C_HMAX), mo.h_max); sts1(CS(C_SINMIN), mo.sin_min);
+          if (METRIC != METRIC_MN) {
+            sts1(CS(C_QDRIFT), mo.q_drift); sts1(CS(C_Q0), mo.Q0); sts1(CS(C_IQ0), mo.iQ0);
+          }
         }
       }
 
       if (finished) {
         unsigned attempts = n_acc + n_rej;
         unsigned n_rhs = 1u + 6u * attempts + 5u * n_land;
-        store_record(P.rays + slot, t, r, th, ph, pr, pth, lam, pt, pph, mo, status, n_acc, n_rej, n_cross,
-                     n_rec, n_rhs);
+        Monitors mo;
+        mo.h_max = lds1(CS(C_HMAX)); mo.q_drift = lds1(CS(C_QDRIFT)); mo.Q0 = 0.0; mo.iQ0 = 0.0;
+        mo.sin_min = lds1(CS(C_SINMIN)); mo.err_margin = lds1(CS(C_MARGIN));
+        store_record(P.rays + slot, lds1(CS(C_T)), r, th, lds1(CS(C_PH)), pr, pth, lds1(CS(C_LAM)), pt, pph, mo,
+                     status, n_acc, n_rej, n_cross, n_rec, n_rhs);
         if (DISK) {
           const double qnan = __longlong_as_double(0x7ff8000000000000LL);
           for (unsigned i = n_rec; i < 3u; ++i) {
@@ -208,79 +269,126 @@ __global__ void __launch_bounds__(kBlock) trace_dp54(const __grid_constant__ Tra
             P.disk[slot].g[i] = qnan;
           }
         }
-        tot_rays += 1; tot_steps += attempts; tot_rhs += n_rhs;
+        sts1(CS(C_TOT_RAYS), lds1(CS(C_TOT_RAYS)) + 1.0);
+        sts1(CS(C_TOT_STEPS), lds1(CS(C_TOT_STEPS)) + (double)attempts);
+        sts1(CS(C_TOT_RHS), lds1(CS(C_TOT_RHS)) + (double)n_rhs);
         mode = MODE_IDLE;
       } else {
         // ---- C: stages 2..6 of the next attempt from (y_n, k1) ----
         // step and reciprocal selector: ordinary step s = h, divisor 1; landing s = target - y_w,
-        // divisor F_w (w = r or theta)
+        // divisor F_w (w = r or theta).  A landing step never returns to (y_n, k1) — the ray ends
+        // (r) or resumes from the parked state (theta) — so k1 is scaled in place.
         const bool land_r = (mode == MODE_LAND_R), land_th = (mode == MODE_LAND_TH);
         const bool landing = land_r || land_th;
-        const double s = land_r ? (target - r) : (land_th ? (target - th) : h);
-#define GP_INV(o_dr, o_dth) (landing ? 1.0 / (land_r ? (o_dr) : (o_dth)) : 1.0)
-        double iv = GP_INV(k1r, k1th);
-        const double K1r = k1r * iv, K1th = k1th * iv, K1pr = k1pr * iv, K1pth = k1pth * iv;
-        double bt = dp.B1 * (k1t * iv), bph = dp.B1 * (k1ph * iv), bl = dp.B1 * iv;   // quadratures t, phi, lambda
-        double qet = dp.E1 * (k1t * iv), qeph = dp.E1 * (k1ph * iv);
+        // Landing steps are 1 in ~300; the divisor work below is skipped by a warp-uniform branch
+        // unless some lane of this convergence group is landing.
+        const bool any_land = __any_sync(__activemask(), landing);
+        double s = h;
+        double bl = 1.0;             // sum of b_i / F_w: d(lambda)/ds of the step, 1 for an ordinary step
+        double k1t = lds1(CS(C_K1T)), k1ph = lds1(CS(C_K1PH));
+        if (any_land) {
+          double iv = 1.0;
+          if (landing) {
+            s = lds1(CS(C_TARGET)) - (land_r ? r : th);
+            iv = rcp_nr(land_r ? k1r : k1th);
+          }
+          k1r *= iv; k1th *= iv; k1pr *= iv; k1pth *= iv; k1t *= iv; k1ph *= iv;
+          bl = dp.B1 * iv;
+        }
+        // divide the stage slopes of a landing lane by F_w and add its b_i / F_w to bl
+#define GP_HENON(b_i)                                                           \
+  if (any_land) {                                                               \
+    double iv = landing ? rcp_nr(land_r ? o.dr : o.dth) : 1.0;                  \
+    o.dr *= iv; o.dth *= iv; o.dpr *= iv; o.dpth *= iv; o.dt *= iv; o.dph *= iv; \
+    bl += (b_i) * iv;                                                           \
+  }
+        // quadratures t, phi: running 5th-order sums and the two error sums
+        double bt = dp.B1 * k1t, bph = dp.B1 * k1ph;
+        double qet = dp.E1 * k1t, qeph = dp.E1 * k1ph;
         Rhs o;
+        double ar, ath, apr, apth;   // K_j of the stage just evaluated
+        double br, bth, bpr, bpth;   // K's streamed back from shared memory
         // stage 2
-        rhs_eval<METRIC>(mc, pt, pph, r + s * (dp.A21 * K1r), th + s * (dp.A21 * K1th),
-                         pr + s * (dp.A21 * K1pr), pth + s * (dp.A21 * K1pth), o);
-        iv = GP_INV(o.dr, o.dth);
-        const double K2r = o.dr * iv, K2th = o.dth * iv, K2pr = o.dpr * iv, K2pth = o.dpth * iv;
+        rhs_eval<METRIC>(mc, pt, pph, r + s * (dp.A21 * k1r), th + s * (dp.A21 * k1th),
+                         pr + s * (dp.A21 * k1pr), pth + s * (dp.A21 * k1pth), o);
+        GP_HENON(0.0)
+        ar = o.dr; ath = o.dth; apr = o.dpr; apth = o.dpth;                         // K2
+        sts2(KS(0), ar, ath); sts2(KS(1), apr, apth);
         // stage 3
-        rhs_eval<METRIC>(mc, pt, pph, r + s * (dp.A31 * K1r + dp.A32 * K2r),
-                         th + s * (dp.A31 * K1th + dp.A32 * K2th),
-                         pr + s * (dp.A31 * K1pr + dp.A32 * K2pr),
-                         pth + s * (dp.A31 * K1pth + dp.A32 * K2pth), o);
-        iv = GP_INV(o.dr, o.dth);
-        const double K3r = o.dr * iv, K3th = o.dth * iv, K3pr = o.dpr * iv, K3pth = o.dpth * iv;
-        bt += dp.B3 * (o.dt * iv); bph += dp.B3 * (o.dph * iv); bl += dp.B3 * iv;
-        qet += dp.E3 * (o.dt * iv); qeph += dp.E3 * (o.dph * iv);
+        rhs_eval<METRIC>(mc, pt, pph, r + s * (dp.A31 * k1r + dp.A32 * ar),
+                         th + s * (dp.A31 * k1th + dp.A32 * ath),
+                         pr + s * (dp.A31 * k1pr + dp.A32 * apr),
+                         pth + s * (dp.A31 * k1pth + dp.A32 * apth), o);
+        GP_HENON(dp.B3)
+        ar = o.dr; ath = o.dth; apr = o.dpr; apth = o.dpth;                         // K3
+        sts2(KS(2), ar, ath); sts2(KS(3), apr, apth);
+        bt += dp.B3 * o.dt; bph += dp.B3 * o.dph;
+        qet += dp.E3 * o.dt; qeph += dp.E3 * o.dph;
         // stage 4
-        rhs_eval<METRIC>(mc, pt, pph, r + s * (dp.A41 * K1r + dp.A42 * K2r + dp.A43 * K3r),
-                         th + s * (dp.A41 * K1th + dp.A42 * K2th + dp.A43 * K3th),
-                         pr + s * (dp.A41 * K1pr + dp.A42 * K2pr + dp.A43 * K3pr),
-                         pth + s * (dp.A41 * K1pth + dp.A42 * K2pth + dp.A43 * K3pth), o);
-        iv = GP_INV(o.dr, o.dth);
-        const double K4r = o.dr * iv, K4th = o.dth * iv, K4pr = o.dpr * iv, K4pth = o.dpth * iv;
-        bt += dp.B4 * (o.dt * iv); bph += dp.B4 * (o.dph * iv); bl += dp.B4 * iv;
-        qet += dp.E4 * (o.dt * iv); qeph += dp.E4 * (o.dph * iv);
+        {
+          double xr = dp.A41 * k1r + dp.A43 * ar, xth = dp.A41 * k1th + dp.A43 * ath;
+          double xpr = dp.A41 * k1pr + dp.A43 * apr, xpth = dp.A41 * k1pth + dp.A43 * apth;
+          lds2(KS(0), br, bth); lds2(KS(1), bpr, bpth);                             // K2
+          xr += dp.A42 * br; xth += dp.A42 * bth; xpr += dp.A42 * bpr; xpth += dp.A42 * bpth;
+          rhs_eval<METRIC>(mc, pt, pph, r + s * xr, th + s * xth, pr + s * xpr, pth + s * xpth, o);
+        }
+        GP_HENON(dp.B4)
+        ar = o.dr; ath = o.dth; apr = o.dpr; apth = o.dpth;                         // K4
+        sts2(KS(4), ar, ath); sts2(KS(5), apr, apth);
+        bt += dp.B4 * o.dt; bph += dp.B4 * o.dph;
+        qet += dp.E4 * o.dt; qeph += dp.E4 * o.dph;
         // stage 5
-        rhs_eval<METRIC>(mc, pt, pph,
-                         r + s * (dp.A51 * K1r + dp.A52 * K2r + dp.A53 * K3r + dp.A54 * K4r),
-                         th + s * (dp.A51 * K1th + dp.A52 * K2th + dp.A53 * K3th + dp.A54 * K4th),
-                         pr + s * (dp.A51 * K1pr + dp.A52 * K2pr + dp.A53 * K3pr + dp.A54 * K4pr),
-                         pth + s * (dp.A51 * K1pth + dp.A52 * K2pth + dp.A53 * K3pth + dp.A54 * K4pth), o);
-        iv = GP_INV(o.dr, o.dth);
-        const double K5r = o.dr * iv, K5th = o.dth * iv, K5pr = o.dpr * iv, K5pth = o.dpth * iv;
-        bt += dp.B5 * (o.dt * iv); bph += dp.B5 * (o.dph * iv); bl += dp.B5 * iv;
-        qet += dp.E5 * (o.dt * iv); qeph += dp.E5 * (o.dph * iv);
+        {
+          double xr = dp.A51 * k1r + dp.A54 * ar, xth = dp.A51 * k1th + dp.A54 * ath;
+          double xpr = dp.A51 * k1pr + dp.A54 * apr, xpth = dp.A51 * k1pth + dp.A54 * apth;
+          lds2(KS(0), br, bth); lds2(KS(1), bpr, bpth);                             // K2
+          xr += dp.A52 * br; xth += dp.A52 * bth; xpr += dp.A52 * bpr; xpth += dp.A52 * bpth;
+          lds2(KS(2), br, bth); lds2(KS(3), bpr, bpth);                             // K3
+          xr += dp.A53 * br; xth += dp.A53 * bth; xpr += dp.A53 * bpr; xpth += dp.A53 * bpth;
+          rhs_eval<METRIC>(mc, pt, pph, r + s * xr, th + s * xth, pr + s * xpr, pth + s * xpth, o);
+        }
+        GP_HENON(dp.B5)
+        ar = o.dr; ath = o.dth; apr = o.dpr; apth = o.dpth;                         // K5
+        sts2(KS(6), ar, ath); sts2(KS(7), apr, apth);
+        bt += dp.B5 * o.dt; bph += dp.B5 * o.dph;
+        qet += dp.E5 * o.dt; qeph += dp.E5 * o.dph;
         // stage 6
-        rhs_eval<METRIC>(
-            mc, pt, pph,
-            r + s * (dp.A61 * K1r + dp.A62 * K2r + dp.A63 * K3r + dp.A64 * K4r + dp.A65 * K5r),
-            th + s * (dp.A61 * K1th + dp.A62 * K2th + dp.A63 * K3th + dp.A64 * K4th + dp.A65 * K5th),
-            pr + s * (dp.A61 * K1pr + dp.A62 * K2pr + dp.A63 * K3pr + dp.A64 * K4pr + dp.A65 * K5pr),
-            pth + s * (dp.A61 * K1pth + dp.A62 * K2pth + dp.A63 * K3pth + dp.A64 * K4pth + dp.A65 * K5pth),
-            o);
-        iv = GP_INV(o.dr, o.dth);
-        const double K6r = o.dr * iv, K6th = o.dth * iv, K6pr = o.dpr * iv, K6pth = o.dpth * iv;
-        bt += dp.B6 * (o.dt * iv); bph += dp.B6 * (o.dph * iv); bl += dp.B6 * iv;
-        qet += dp.E6 * (o.dt * iv); qeph += dp.E6 * (o.dph * iv);
-#undef GP_INV
+        {
+          double xr = dp.A61 * k1r + dp.A65 * ar, xth = dp.A61 * k1th + dp.A65 * ath;
+          double xpr = dp.A61 * k1pr + dp.A65 * apr, xpth = dp.A61 * k1pth + dp.A65 * apth;
+          lds2(KS(0), br, bth); lds2(KS(1), bpr, bpth);                             // K2
+          xr += dp.A62 * br; xth += dp.A62 * bth; xpr += dp.A62 * bpr; xpth += dp.A62 * bpth;
+          lds2(KS(2), br, bth); lds2(KS(3), bpr, bpth);                             // K3
+          xr += dp.A63 * br; xth += dp.A63 * bth; xpr += dp.A63 * bpr; xpth += dp.A63 * bpth;
+          lds2(KS(4), br, bth); lds2(KS(5), bpr, bpth);                             // K4
+          xr += dp.A64 * br; xth += dp.A64 * bth; xpr += dp.A64 * bpr; xpth += dp.A64 * bpth;
+          rhs_eval<METRIC>(mc, pt, pph, r + s * xr, th + s * xth, pr + s * xpr, pth + s * xpth, o);
+        }
+        GP_HENON(dp.B6)
+        ar = o.dr; ath = o.dth; apr = o.dpr; apth = o.dpth;                         // K6
+        bt += dp.B6 * o.dt; bph += dp.B6 * o.dph;
+        qet += dp.E6 * o.dt; qeph += dp.E6 * o.dph;
+#undef GP_HENON
         // trial end state (5th-order solution; a7 = b) and the error sums without e7 k7
-        nr = r + s * (dp.B1 * K1r + dp.B3 * K3r + dp.B4 * K4r + dp.B5 * K5r + dp.B6 * K6r);
-        nth = th + s * (dp.B1 * K1th + dp.B3 * K3th + dp.B4 * K4th + dp.B5 * K5th + dp.B6 * K6th);
-        npr = pr + s * (dp.B1 * K1pr + dp.B3 * K3pr + dp.B4 * K4pr + dp.B5 * K5pr + dp.B6 * K6pr);
-        npth = pth + s * (dp.B1 * K1pth + dp.B3 * K3pth + dp.B4 * K4pth + dp.B5 * K5pth + dp.B6 * K6pth);
-        nt = t + s * bt;
-        nph = ph + s * bph;
-        nlam = lam + s * bl;
-        er = dp.E1 * K1r + dp.E3 * K3r + dp.E4 * K4r + dp.E5 * K5r + dp.E6 * K6r;
-        eth = dp.E1 * K1th + dp.E3 * K3th + dp.E4 * K4th + dp.E5 * K5th + dp.E6 * K6th;
-        epr = dp.E1 * K1pr + dp.E3 * K3pr + dp.E4 * K4pr + dp.E5 * K5pr + dp.E6 * K6pr;
-        epth = dp.E1 * K1pth + dp.E3 * K3pth + dp.E4 * K4pth + dp.E5 * K5pth + dp.E6 * K6pth;
+        {
+          double xr = dp.B1 * k1r + dp.B6 * ar, xth = dp.B1 * k1th + dp.B6 * ath;
+          double xpr = dp.B1 * k1pr + dp.B6 * apr, xpth = dp.B1 * k1pth + dp.B6 * apth;
+          er = dp.E1 * k1r + dp.E6 * ar; eth = dp.E1 * k1th + dp.E6 * ath;
+          epr = dp.E1 * k1pr + dp.E6 * apr; epth = dp.E1 * k1pth + dp.E6 * apth;
+          lds2(KS(2), br, bth); lds2(KS(3), bpr, bpth);                             // K3
+          xr += dp.B3 * br; xth += dp.B3 * bth; xpr += dp.B3 * bpr; xpth += dp.B3 * bpth;
+          er += dp.E3 * br; eth += dp.E3 * bth; epr += dp.E3 * bpr; epth += dp.E3 * bpth;
+          lds2(KS(4), br, bth); lds2(KS(5), bpr, bpth);                             // K4
+          xr += dp.B4 * br; xth += dp.B4 * bth; xpr += dp.B4 * bpr; xpth += dp.B4 * bpth;
+          er += dp.E4 * br; eth += dp.E4 * bth; epr += dp.E4 * bpr; epth += dp.E4 * bpth;
+          lds2(KS(6), br, bth); lds2(KS(7), bpr, bpth);                             // K5
+          xr += dp.B5 * br; xth += dp.B5 * bth; xpr += dp.B5 * bpr; xpth += dp.B5 * bpth;
+          er += dp.E5 * br; eth += dp.E5 * bth; epr += dp.E5 * bpr; epth += dp.E5 * bpth;
+          nr = r + s * xr; nth = th + s * xth; npr = pr + s * xpr; npth = pth + s * xpth;
+        }
+        nt = lds1(CS(C_T)) + s * bt;
+        nph = lds1(CS(C_PH)) + s * bph;
+        nlam = lds1(CS(C_LAM)) + s * bl;
         et = qet;
         eph = qeph;
       }
@@ -288,11 +396,17 @@ __global__ void __launch_bounds__(kBlock) trace_dp54(const __grid_constant__ Tra
   }
 
   // totals (gp.h: counters[1] rays finished, [2] attempted steps, [3] RHS evaluations)
-  if (tot_rays) {
-    atomicAdd(P.counters + 1, tot_rays);
-    atomicAdd(P.counters + 2, tot_steps);
-    atomicAdd(P.counters + 3, tot_rhs);
+  {
+    const double tr = lds1(CS(C_TOT_RAYS));
+    if (tr > 0.0) {
+      atomicAdd(P.counters + 1, (unsigned long long)tr);
+      atomicAdd(P.counters + 2, (unsigned long long)lds1(CS(C_TOT_STEPS)));
+      atomicAdd(P.counters + 3, (unsigned long long)lds1(CS(C_TOT_RHS)));
+    }
   }
+#undef KS
+#undef CS
+#undef PS
 }
 
 #endif  // __CUDACC__
