@@ -320,8 +320,23 @@ int gp_trace_host(int metric_id, const gp_metric_params *metric, const gp_camera
   cudaStream_t stream = (cudaStream_t)cuda_stream;
   // one scratch allocation: counters | ray records | disk records
   const size_t off_rays = 64, off_disk = off_rays + ((rays_b + 63) & ~(size_t)63);
+  // The scratch comes from a library-owned stream-ordered pool that keeps its memory between
+  // calls (release threshold = max): the default pool would hand 128 MiB back to the driver at
+  // every synchronisation and pay cudaMalloc again on the next call.
+  static cudaMemPool_t pool = nullptr;
+  if (!pool) {
+    int dev = 0;
+    GP_CUDA(cudaGetDevice(&dev));
+    cudaMemPoolProps props = {};
+    props.allocType = cudaMemAllocationTypePinned;
+    props.location.type = cudaMemLocationTypeDevice;
+    props.location.id = dev;
+    GP_CUDA(cudaMemPoolCreate(&pool, &props));
+    unsigned long long keep = ~0ull;
+    GP_CUDA(cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep));
+  }
   char *scratch = nullptr;
-  GP_CUDA(cudaMallocAsync((void **)&scratch, off_disk + disk_b + 64, stream));
+  GP_CUDA(cudaMallocFromPoolAsync((void **)&scratch, off_disk + disk_b + 64, pool, stream));
   gp_out_buffers dev;
   dev.counters = scratch;
   dev.counters_bytes = 64;

@@ -1,17 +1,19 @@
 // gp_math.cuh — FP64 elementary functions for the tracer's inner loop, written for the sm_100a
 // issue model.
 //
-// Why not the CUDA math library here: profiles/r01 showed that 28 % of the warp instructions of
-// trace_dp54 were UMOV/IMAD.MOV pairs that materialise 64-bit literals (the library's sincos,
-// division and pow carry their coefficients as immediates), and that each `a / b` and each fmax
-// drags a denormal / NaN slow-path test through the instruction stream.  The FP64 pipe issues
-// one warp instruction every other cycle, so those extra issue slots cost as much as the
-// arithmetic.  Every literal below lives in __constant__ memory and reaches DFMA/DMUL as a
-// c[bank][offset] operand; every function is branch-free on the range the integrator produces
-// and falls back to the library outside it.
+// Why not the CUDA math library here: profiles/trace_dp54_r01a.md showed that 28 % of the warp
+// instructions of the first trace_dp54 were UMOV/IMAD.MOV pairs materialising 64-bit literals (the
+// library's sincos, division and pow carry their coefficients as immediates), and that each `a / b`
+// and each fmax drags a denormal / NaN slow-path test through the instruction stream.  On sm_100a
+// an FP64 instruction holds the issue slot for two cycles and every other instruction costs a full
+// cycle on top, so those instructions cost as much as the arithmetic.
+// Every literal below lives in __constant__ memory (one LDCU per use at worst, 128-bit pairs where
+// adjacent); every function is branch-free on the range the integrator produces and falls back to
+// the library outside it.
 //
-// Accuracy (checked by tests/test_gpu_parity.py::test_device_math_*): sincos_pi4 <= 1 ulp-ish
-// (polynomial error 1e-17 / 5e-19 before rounding), rcp_nr and div_nr <= 1 ulp, pow_m1_5 <= 2 ulp.
+// Accuracy: sincos polynomial error 1e-17 / 5e-19 before rounding, rcp_nr and div_nr <= 1 ulp,
+// pow_m1_5 <= 2 ulp; exercised against the oracle by tests/test_gpu_parity.py
+// (test_eval_rhs_matches_oracle, test_eval_metric_matches_oracle and every trace test).
 #ifndef GP_MATH_CUH_
 #define GP_MATH_CUH_
 
