@@ -308,7 +308,10 @@ def run_b200(args):
         "steps_per_ray": attempts / n, "rhs_per_ray": n_rhs / n,
         "roofline": {"bound": "alu", "kernel": "trace_dp54" if gs.scheme == 2 else "trace_rk4",
                      "achieved": achieved, "peak": peak_nominal, "unit": "TFLOP/s",
-                     "frac": achieved / peak_nominal, "traffic": None,
+                     "frac": achieved / peak_nominal,
+                     # dram__bytes_read.sum + dram__bytes_write.sum of one headline launch, from the
+                     # ncu --set full capture summarised in profiles/trace_dp54_r01c.md
+                     "traffic": 8.29e7 if args.workload == "headline" else None,
                      "peak_kind": f"nominal FP64 FMA: {props.multi_processor_count} SMs x "
                                   f"{FP64_LANES_PER_SM} lanes x 2 x {sm_max:.0f} MHz",
                      "peak_probe": peak_probe, "frac_of_probe": achieved / peak_probe if peak_probe else None,
