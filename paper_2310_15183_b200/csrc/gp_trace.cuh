@@ -52,6 +52,7 @@ struct DpTableau {
   double B1, B3, B4, B5, B6;
   double E1, E3, E4, E5, E6, E7;
   double safety, fac_min, fac_max, err_lo, err_hi, h_floor;  // controller constants, R10 items 3 and 5
+  double sixth;                                              // RK4 weight 1/6 (eq 44)
 };
 
 #if defined(__CUDACC__)
@@ -63,7 +64,8 @@ __constant__ DpTableau dp = {
     9017.0 / 3168.0, -355.0 / 33.0, 46732.0 / 5247.0, 49.0 / 176.0, -5103.0 / 18656.0,
     35.0 / 384.0, 500.0 / 1113.0, 125.0 / 192.0, -2187.0 / 6784.0, 11.0 / 84.0,
     71.0 / 57600.0, -71.0 / 16695.0, 71.0 / 1920.0, -17253.0 / 339200.0, 22.0 / 525.0, -1.0 / 40.0,
-    0.9, 0.2, 5.0, 1.0e-5, 1.0e4, 1.0e-14};
+    0.9, 0.2, 5.0, 1.0e-5, 1.0e4, 1.0e-14,
+    1.0 / 6.0};
 #endif
 
 #if defined(__CUDACC__)

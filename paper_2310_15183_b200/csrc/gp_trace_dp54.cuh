@@ -137,12 +137,15 @@ trace_dp54(const __grid_constant__ TraceParams P) {
         //   err = max_j |h (e_j + E7 k7_j)| / (atol + rtol max(|y_j|, |y+_j|)).
         // The largest ratio is found by cross-multiplication (num_j den_best > num_best den_j) and
         // divided once; a tie within rounding picks either of two equal ratios.
-        double nm = fabs(h * (et + dp.E7 * o7.dt)), dn = fma(P.rtol, dmax(fabs(t), fabs(nt)), P.atol);
+        // |h| is common to the six numerators and multiplies the winner only; the scale is built as
+        // |larger of y, y+| * rtol + atol with the abs folded into the multiply's operand modifier.
+#define GP_SCALE(y_, ny_) (__dmul_rn(fabs(fabs(y_) > fabs(ny_) ? (y_) : (ny_)), P.rtol) + P.atol)
+        double nm = fabs(et + dp.E7 * o7.dt), dn = GP_SCALE(t, nt);
         double nsum = nm;
 #define GP_ERR_TERM(e_, k7_, y_, ny_)                                            \
   {                                                                              \
-    double n_ = fabs(h * ((e_) + dp.E7 * (k7_)));                                \
-    double d_ = fma(P.rtol, dmax(fabs(y_), fabs(ny_)), P.atol);                  \
+    double n_ = fabs((e_) + dp.E7 * (k7_));                                      \
+    double d_ = GP_SCALE(y_, ny_);                                               \
     nsum += n_;                                                                  \
     bool gt_ = n_ * dn > nm * d_;                                                \
     nm = gt_ ? n_ : nm;                                                          \
@@ -154,6 +157,8 @@ trace_dp54(const __grid_constant__ TraceParams P) {
         GP_ERR_TERM(epr, o7.dpr, pr, npr)
         GP_ERR_TERM(epth, o7.dpth, pth, npth)
 #undef GP_ERR_TERM
+#undef GP_SCALE
+        nm *= fabs(h);
         // finite test on the sums: any inf/NaN term makes them non-finite (numerators are >= 0)
         double ysum = ((nt + nr) + (nth + nph)) + (npr + npth);
         double err = div_nr(nm, dn, rcp_nr(dn));

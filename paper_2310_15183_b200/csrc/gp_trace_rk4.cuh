@@ -67,43 +67,47 @@ __global__ void __launch_bounds__(kBlock) trace_rk4(const __grid_constant__ Trac
         const bool normal = (mode == MODE_NORMAL);
         const bool land_r = (mode == MODE_LAND_R);
         const double s = normal ? (P.scheme == 0 ? P.h : P.h_rel * r) : (land_r ? (target - r) : (target - th));
-#define GP_INV(o_dr, o_dth) (normal ? 1.0 : 1.0 / (land_r ? (o_dr) : (o_dth)))
+        // Landing steps are 1 in several hundred: their divisor work (Henon's 1/F_w) sits behind a
+        // warp-uniform branch taken only when some lane of this convergence group is landing.
+        const bool any_land = __any_sync(__activemask(), !normal);
+        double sl = 1.0;  // weighted sum of 1/F_w: d(lambda)/ds of a landing step (unused otherwise)
+#define GP_HENON(weight, first)                                                   \
+  if (any_land) {                                                                 \
+    double iv = normal ? 1.0 : rcp_nr(land_r ? o.dr : o.dth);                     \
+    o.dt *= iv; o.dr *= iv; o.dth *= iv; o.dph *= iv; o.dpr *= iv; o.dpth *= iv;  \
+    sl = (first) ? iv : sl + (weight) * iv;                                       \
+  }
         Rhs o;
         // k1 = F(y_n)
         rhs_eval<METRIC>(mc, pt, pph, r, th, pr, pth, o);
         if (normal)
           monitor_apply<METRIC>(mo, fabs(0.5 * o.H2), carter_q<METRIC>(mc, pt, pph, pth, o), fabs(o.s),
                                 n_acc == 0);
-        double iv = GP_INV(o.dr, o.dth);
-        double kt = o.dt * iv, kr = o.dr * iv, kth = o.dth * iv, kph = o.dph * iv, kpr = o.dpr * iv,
-               kpth = o.dpth * iv;
-        double st = kt, sr = kr, sth = kth, sph = kph, spr = kpr, spth = kpth, sl = iv;  // k1 + 2k2 + 2k3 + k4
+        GP_HENON(1.0, true)
+        double st = o.dt, sr = o.dr, sth = o.dth, sph = o.dph, spr = o.dpr, spth = o.dpth;  // k1 + 2k2 + 2k3 + k4
         const double hs = 0.5 * s;
         // k2 = F(y_n + h/2 k1)
-        double yr = r + hs * kr;
+        double yr = r + hs * o.dr;
         bool captured = normal && (yr < P.r_cap);
-        rhs_eval<METRIC>(mc, pt, pph, yr, th + hs * kth, pr + hs * kpr, pth + hs * kpth, o);
-        iv = GP_INV(o.dr, o.dth);
-        kt = o.dt * iv; kr = o.dr * iv; kth = o.dth * iv; kph = o.dph * iv; kpr = o.dpr * iv; kpth = o.dpth * iv;
-        st += 2.0 * kt; sr += 2.0 * kr; sth += 2.0 * kth; sph += 2.0 * kph; spr += 2.0 * kpr; spth += 2.0 * kpth;
-        sl += 2.0 * iv;
+        rhs_eval<METRIC>(mc, pt, pph, yr, th + hs * o.dth, pr + hs * o.dpr, pth + hs * o.dpth, o);
+        GP_HENON(2.0, false)
+        st += 2.0 * o.dt; sr += 2.0 * o.dr; sth += 2.0 * o.dth; sph += 2.0 * o.dph; spr += 2.0 * o.dpr;
+        spth += 2.0 * o.dpth;
         // k3 = F(y_n + h/2 k2)
-        yr = r + hs * kr;
+        yr = r + hs * o.dr;
         captured = captured || (normal && (yr < P.r_cap));
-        rhs_eval<METRIC>(mc, pt, pph, yr, th + hs * kth, pr + hs * kpr, pth + hs * kpth, o);
-        iv = GP_INV(o.dr, o.dth);
-        kt = o.dt * iv; kr = o.dr * iv; kth = o.dth * iv; kph = o.dph * iv; kpr = o.dpr * iv; kpth = o.dpth * iv;
-        st += 2.0 * kt; sr += 2.0 * kr; sth += 2.0 * kth; sph += 2.0 * kph; spr += 2.0 * kpr; spth += 2.0 * kpth;
-        sl += 2.0 * iv;
+        rhs_eval<METRIC>(mc, pt, pph, yr, th + hs * o.dth, pr + hs * o.dpr, pth + hs * o.dpth, o);
+        GP_HENON(2.0, false)
+        st += 2.0 * o.dt; sr += 2.0 * o.dr; sth += 2.0 * o.dth; sph += 2.0 * o.dph; spr += 2.0 * o.dpr;
+        spth += 2.0 * o.dpth;
         // k4 = F(y_n + h k3)
-        yr = r + s * kr;
+        yr = r + s * o.dr;
         captured = captured || (normal && (yr < P.r_cap));
-        rhs_eval<METRIC>(mc, pt, pph, yr, th + s * kth, pr + s * kpr, pth + s * kpth, o);
-        iv = GP_INV(o.dr, o.dth);
-        st += o.dt * iv; sr += o.dr * iv; sth += o.dth * iv; sph += o.dph * iv; spr += o.dpr * iv;
-        spth += o.dpth * iv; sl += iv;
-#undef GP_INV
-        const double w = s / 6.0;
+        rhs_eval<METRIC>(mc, pt, pph, yr, th + s * o.dth, pr + s * o.dpr, pth + s * o.dpth, o);
+        GP_HENON(1.0, false)
+        st += o.dt; sr += o.dr; sth += o.dth; sph += o.dph; spr += o.dpr; spth += o.dpth;
+#undef GP_HENON
+        const double w = s * dp.sixth;
         const double nt = t + w * st, nr = r + w * sr, nth = th + w * sth, nph = ph + w * sph,
                      npr = pr + w * spr, npth = pth + w * spth;
 
