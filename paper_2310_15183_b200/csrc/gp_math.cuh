@@ -109,10 +109,12 @@ __device__ __forceinline__ void sincos_fast(double x, double *sn, double *cs) {
 }
 
 // x^(-1/5) for x in [1e-5, 1e4] (the controller clamps outside, R10 item 3): FP32 seed from the
-// SFU (about 1e-6), two Newton steps on y^-5 = x (error 3 e^2 per step) -> <= 2 ulp.
+// SFU (lg2/ex2, about 1e-6 relative), two Newton steps on y^-5 = x (error 3 e^2 per step) -> <= 2 ulp.
 __device__ __forceinline__ double pow_m1_5(double x) {
-  float xf = __double2float_rn(x);
-  double y = (double)exp2f(-0.2f * __log2f(xf));
+  float xf = __double2float_rn(x), lg, yf;
+  asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(lg) : "f"(xf));
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(yf) : "f"(-0.2f * lg));
+  double y = (double)yf;
 #pragma unroll
   for (int i = 0; i < 2; ++i) {
     double y2 = y * y;

@@ -290,3 +290,50 @@ def test_step_budget_and_host_entry(gp, O):
     assert host_r.tobytes() == dev_r.tobytes()
     assert host_d.tobytes() == dev_d.tobytes()
     assert np.array_equal(host_c[1:4], dev_c[1:4])
+
+
+# ---- full size, in the launch configuration bench.py times ------------------------------------
+def test_headline_full_image_sampled_parity_and_closed_form_shadow(gp, O):
+    """The headline launch (1024 x 1024, every ray, one persistent launch) compared (a) record by
+    record with the oracle on a scattered sample the oracle traces one by one, and (b) on a larger
+    sample with the closed-form Kerr classifier: a ray that starts inward is captured iff the radial
+    potential R(r) = ((r^2+a^2) p_t + a p_phi)^2 - Delta (Q + (p_phi + a p_t)^2) has no root in
+    (r_+, r_obs) (Carter 1968; pin P3 of the oracle, here applied to the GPU's own records)."""
+    import torch
+    w = W.workload("headline")
+    n = W.n_rays(w)
+    rays, _, counters = gp.api.trace_workload(w)
+    assert len(rays) == n and counters[1] == n
+    assert set(np.unique(rays["status"])) <= {0, 1}
+    # (a) sampled parity
+    b, c, s = W.ray_selection(w, 7, None, 257)
+    orc, _ = O.trace(w, b, c, s)
+    probe, _ = O.trace(w, b, c, s, rounding_probe=True)
+    check_parity(w, rays[b::s][:c], orc, probe, "headline sample", max_flagged_fraction=0.01)
+    # (b) closed-form classifier on every 53rd ray
+    sel = np.arange(11, n, 53)
+    cam = gp.api.camera_struct(w["camera"], 11, len(sel), 53)
+    st = torch.empty((len(sel), 8), dtype=torch.float64, device="cuda")
+    ab = torch.empty((len(sel), 2), dtype=torch.float64, device="cuda")
+    gp.gp_init_conditions(w["metric"]["id"], gp.api.metric_struct(w["metric"]), cam, st, ab)
+    st = st.cpu().numpy()
+    M, a, ro = 1.0, 0.9, 1000.0
+    rp = M + math.sqrt(M * M - a * a)
+    pt, th, pth, pph = st[:, 4], st[:, 2], st[:, 6], st[:, 7]
+    K = pth ** 2 + np.cos(th) ** 2 * (pph ** 2 / np.sin(th) ** 2 - a * a * pt * pt) + (pph + a * pt) ** 2
+    checked = wrong = 0
+    for i in range(len(sel)):
+        P = np.poly1d([pt[i], 0.0, a * a * pt[i] + a * pph[i]])
+        R = P * P - np.poly1d([1.0, -2 * M, a * a]) * K[i]
+        crit = [z.real for z in R.deriv().roots if abs(z.imag) < 1e-12 and z.real > rp]
+        if any(abs(R(cr)) < 1e-6 * pt[i] ** 2 * cr ** 4 for cr in crit):
+            continue  # within 1e-6 of the shadow edge (double root)
+        roots = [z.real for z in R.roots if abs(z.imag) < 1e-9 * max(1.0, abs(z.real)) and rp < z.real < ro]
+        checked += 1
+        wrong += int((rays["status"][sel[i]] == 1) != (len(roots) == 0))
+    assert checked > 15000 and wrong == 0, (checked, wrong)
+    # exit surface and invariants on the whole image
+    esc = rays["status"] == 0
+    assert np.all(rays["r"][esc] == 1100.0) and np.all(rays["r"][~esc] == rp * (1.0 + 1e-3))
+    assert np.percentile(rays["h_max"][esc], 99.9) <= 1e-8
+    assert np.percentile(rays["q_drift"][esc], 99.9) <= 1e-8
