@@ -337,3 +337,25 @@ def test_headline_full_image_sampled_parity_and_closed_form_shadow(gp, O):
     assert np.all(rays["r"][esc] == 1100.0) and np.all(rays["r"][~esc] == rp * (1.0 + 1e-3))
     assert np.percentile(rays["h_max"][esc], 99.9) <= 1e-8
     assert np.percentile(rays["q_drift"][esc], 99.9) <= 1e-8
+
+
+def test_manko_novikov_equatorial_mirror_symmetry_on_the_gpu(gp):
+    """the Manko-Novikov spacetime is reflection-symmetric about the equator, so
+    an equatorial observer's image is mirror-symmetric: the rays through (alpha, beta) and
+    (alpha, -beta) end with the same status, theta' = pi - theta, phi' = phi, lambda' = lambda.
+    A property that holds at any size; checked on a jitter-free 160 x 160 frame of config 4
+    (step budget 3000: interior rays end as MAXSTEPS on both sides of the mirror)."""
+    w = W.workload("C4", width=160, height=160, jitter_amp_px=0.0)
+    w["cfg"]["max_steps"] = 3000
+    rays, _, _ = gp.api.trace_workload(w)
+    img = rays.reshape(160, 160)
+    up, dn = img[80:, :], img[:80, :][::-1, :]      # row j <-> row H-1-j
+    same = up["status"] == dn["status"]
+    assert same.mean() >= 0.995, same.mean()
+    # smooth pairs: both escaped after an ordinary number of steps (the chaotic band takes more)
+    ok = same & (up["status"] == 0) & (up["n_accepted"] < 500) & (dn["n_accepted"] < 500)
+    assert ok.mean() > 0.6
+    assert np.abs(up["theta"] + dn["theta"] - math.pi)[ok].max() <= 1e-8
+    assert rel_err(up["phi"], dn["phi"])[ok].max() <= 1e-8
+    assert rel_err(up["lambda"], dn["lambda"])[ok].max() <= 1e-9
+    assert (img["status"] == 2).sum() > 100 and (img["status"] == 0).sum() > 15000
