@@ -36,6 +36,7 @@ F_RHS = {W.SCHWARZSCHILD: 40.0, W.KERR: 81.0, W.MANKO_NOVIKOV: 760.0}
 F_STEP = {0: 56.0, 1: 57.0, 2: 324.0}
 # nominal FP64 FMA peak: 148 SMs x 64 FP64 FMA lanes x 2 flop x 1.965 GHz
 FP64_LANES_PER_SM = 64
+FP32_LANES_PER_SM = 128
 
 
 def _args():
@@ -47,6 +48,8 @@ def _args():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--cpu-seconds", type=float, default=12.0,
                     help="target oracle time for the cpu_baseline sample")
+    ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32"],
+                    help="fp32: the single-precision variant (fixed-step RK4 workloads only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -198,6 +201,11 @@ def run_b200(args):
     # independent, so there is no exchange step
     w = W.workload(args.workload)
     w["camera"]["jitter_seed"] = int(w["camera"].get("jitter_seed", 0)) + rank
+    fp32 = args.precision == "fp32"
+    if fp32:
+        if w["cfg"]["scheme"] == 2:
+            raise SystemExit("bench.py: --precision fp32 exists for the fixed-step RK4 workloads only")
+        w["cfg"]["precision"] = 1
     n = W.n_rays(w)
     mid = w["metric"]["id"]
     ms, cs, gs = gp.api.metric_struct(w["metric"]), gp.api.camera_struct(w["camera"]), gp.api.cfg_struct(w["cfg"])
@@ -296,13 +304,14 @@ def run_b200(args):
     achieved = flops / (kern_ms * 1e-3) / 1e12
     props = torch.cuda.get_device_properties(dev)
     sm_max = (clocks or {}).get("sm_max_mhz") or 1965.0
-    peak_nominal = props.multi_processor_count * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+    lanes = FP32_LANES_PER_SM if fp32 else FP64_LANES_PER_SM
+    peak_nominal = props.multi_processor_count * lanes * 2 * sm_max * 1e6 / 1e12
     out = {
         "metric": "geodesics/sec (1024^2 Kerr a=0.9, FP64)" if args.workload == "headline"
                   else f"geodesics/sec ({args.workload})",
         "value": value, "unit": "geodesics/s", "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": total_ms_max / args.steps,
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32" if fp32 else "f64",
         "data": "synthetic", "config": config_of(w, world),
         "rhs_evals_per_s": world * n_rhs * args.steps / sec,
         "steps_per_ray": attempts / n, "rhs_per_ray": n_rhs / n,
@@ -312,9 +321,10 @@ def run_b200(args):
                      # dram__bytes_read.sum + dram__bytes_write.sum of one headline launch, from the
                      # ncu --set full capture summarised in profiles/trace_dp54_r01c.md
                      "traffic": 8.29e7 if args.workload == "headline" else None,
-                     "peak_kind": f"nominal FP64 FMA: {props.multi_processor_count} SMs x "
-                                  f"{FP64_LANES_PER_SM} lanes x 2 x {sm_max:.0f} MHz",
-                     "peak_probe": peak_probe, "frac_of_probe": achieved / peak_probe if peak_probe else None,
+                     "peak_kind": f"nominal {'FP32' if fp32 else 'FP64'} FMA: {props.multi_processor_count} SMs x "
+                                  f"{lanes} lanes x 2 x {sm_max:.0f} MHz",
+                     "peak_probe": None if fp32 else peak_probe,
+                     "frac_of_probe": None if fp32 else (achieved / peak_probe if peak_probe else None),
                      "probe_kind": "gp_probe_fp64_fma: register-resident DFMA chains, same process",
                      "alg_flops_per_launch": flops, "kernel_ms": kern_ms,
                      "flop_model": f"{F_RHS[mid]:.0f}/RHS + {F_STEP[gs.scheme]:.0f}/step (DESIGN.md 6.2)"},

@@ -77,7 +77,9 @@ typedef struct gp_camera {
  * lambda_max when lambda_max > 0), NONFINITE / STEP_UNDERFLOW on numerical failure.     */
 typedef struct gp_integrator_cfg {
   int32_t scheme;    /* 0, 1, 2 as above                                                 */
-  int32_t precision; /* 0 = FP64 (the only one built); others -> GP_E_UNSUPPORTED        */
+  int32_t precision; /* 0 = FP64; 1 = FP32 state and equations, schemes 0 and 1 only (with
+                        scheme 2 -> GP_E_UNSUPPORTED); the ray is born and the record written in
+                        FP64 either way; others -> GP_E_UNSUPPORTED                             */
   double h, h_rel, rtol, atol, h_cap_rel;
   int64_t max_steps; /* attempted steps (accepted + rejected), landing steps not counted */
   double lambda_max; /* <= 0: off                                                        */

@@ -130,8 +130,11 @@ int make_params(int metric_id, const gp_metric_params *m, const gp_camera *cam, 
   memset(P, 0, sizeof(*P));
   int rc = make_metric(metric_id, m, &P->mc);
   if (rc) return rc;
-  if (cfg->precision != 0) return GP_E_UNSUPPORTED;
+  if (cfg->precision != 0 && cfg->precision != 1) return GP_E_UNSUPPORTED;
   if (cfg->scheme < 0 || cfg->scheme > 2) return GP_E_BAD_PARAM;
+  // the single-precision variant exists for the fixed-step schemes only: a 1e-10 tolerance has no
+  // meaning in FP32 arithmetic
+  if (cfg->precision == 1 && cfg->scheme == 2) return GP_E_UNSUPPORTED;
   if (!(cfg->eps_capture >= 0.0) || !isfinite(cfg->eps_capture)) return GP_E_BAD_PARAM;
   rc = make_camera(metric_id, P->mc, cam, cfg->eps_capture, &P->cc);
   if (rc) return rc;
@@ -147,6 +150,7 @@ int make_params(int metric_id, const gp_metric_params *m, const gp_camera *cam, 
   if (cfg->max_crossings > 0 && metric_id == GP_MANKO_NOVIKOV) return GP_E_UNSUPPORTED;
   if (isnan(cfg->lambda_max)) return GP_E_BAD_PARAM;
   P->scheme = cfg->scheme;
+  P->precision = cfg->precision;
   P->max_crossings = cfg->max_crossings;
   P->h = cfg->h;
   P->h_rel = cfg->h_rel;
@@ -168,11 +172,13 @@ int make_params(int metric_id, const gp_metric_params *m, const gp_camera *cam, 
 // ---- launch -----------------------------------------------------------------------------------
 template <int METRIC, bool DISK>
 int launch_one(const TraceParams &P, cudaStream_t stream) {
-  static int blocks_dp = 0, blocks_rk = 0;
+  static int blocks[3] = {0, 0, 0};  // resident blocks per SM: dp54, rk4 FP64, rk4 FP32
   static int n_sm = 0;
   const bool dp54 = (P.scheme == 2);
-  const size_t smem = dp54 ? dp54_smem_bytes(DISK) : (DISK ? sizeof(double) * kBlock * kParkSlotsRk4 : 0);
-  int &per_sm = dp54 ? blocks_dp : blocks_rk;
+  const bool fp32 = (P.precision == 1);
+  const size_t smem = dp54 ? dp54_smem_bytes(DISK)
+                           : (DISK ? (fp32 ? sizeof(float) : sizeof(double)) * kBlock * kParkSlotsRk4 : 0);
+  int &per_sm = blocks[dp54 ? 0 : (fp32 ? 2 : 1)];
   if (per_sm == 0) {
     int dev = 0;
     GP_CUDA(cudaGetDevice(&dev));
@@ -180,8 +186,10 @@ int launch_one(const TraceParams &P, cudaStream_t stream) {
     int occ = 0;
     if (dp54)
       GP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, trace_dp54<METRIC, DISK>, kBlock, smem));
+    else if (fp32)
+      GP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, trace_rk4<METRIC, DISK, float>, kBlock, smem));
     else
-      GP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, trace_rk4<METRIC, DISK>, kBlock, smem));
+      GP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, trace_rk4<METRIC, DISK, double>, kBlock, smem));
     if (occ < 1) occ = 1;
     // tuning aid: GP_BLOCKS_PER_SM caps the resident blocks per SM (never raises them)
     if (const char *cap = getenv("GP_BLOCKS_PER_SM")) {
@@ -197,8 +205,10 @@ int launch_one(const TraceParams &P, cudaStream_t stream) {
   if (grid < 1) grid = 1;
   if (dp54)
     trace_dp54<METRIC, DISK><<<(unsigned)grid, kBlock, smem, stream>>>(P);
+  else if (fp32)
+    trace_rk4<METRIC, DISK, float><<<(unsigned)grid, kBlock, smem, stream>>>(P);
   else
-    trace_rk4<METRIC, DISK><<<(unsigned)grid, kBlock, smem, stream>>>(P);
+    trace_rk4<METRIC, DISK, double><<<(unsigned)grid, kBlock, smem, stream>>>(P);
   GP_CUDA(cudaGetLastError());
   return GP_OK;
 }

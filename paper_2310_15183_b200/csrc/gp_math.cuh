@@ -144,5 +144,59 @@ GP_HD void fsincos(double x, double *sn, double *cs) {
 #endif
 }
 
+// FP32 forms for the single-precision variant (cfg.precision = 1): the
+// correctly rounded reciprocal and the library's full-range sincosf / expf / sqrtf.
+GP_HD float frcp(float x) {
+#if defined(__CUDA_ARCH__)
+  return __frcp_rn(x);
+#else
+  return 1.0f / x;
+#endif
+}
+#if defined(__CUDACC__)
+__device__ __noinline__ void sincosf_library(float x, float *sn, float *cs) { sincosf(x, sn, cs); }
+// FP32 sincos for |x| < 1e4: two-term Cody-Waite (the FMA keeps q*hi exact), Taylor kernels through
+// r^9 / r^10 on |r| <= pi/4 (truncation 2e-9 / 1e-10, below half an FP32 ulp), quadrant swap.
+__device__ __forceinline__ void sincosf_fast(float x, float *sn, float *cs) {
+  if (!(fabsf(x) < 1.0e4f)) {
+    sincosf_library(x, sn, cs);
+    return;
+  }
+  float qf = rintf(x * 0.636619772367581343f);
+  int q = __float2int_rn(qf);
+  float r = fmaf(-qf, 1.57079637050628662109375f, x);
+  r = fmaf(-qf, -4.37113882867379116e-8f, r);
+  float z = r * r;
+  float ps = fmaf(z, 2.75573192e-6f, -1.98412698e-4f);
+  float pc = fmaf(z, -2.75573192e-7f, 2.48015873e-5f);
+  ps = fmaf(z, ps, 8.33333333e-3f);
+  pc = fmaf(z, pc, -1.38888889e-3f);
+  ps = fmaf(z, ps, -1.66666667e-1f);
+  pc = fmaf(z, pc, 4.16666667e-2f);
+  float sr = fmaf(r * z, ps, r);
+  float cr = fmaf(z * z, pc, fmaf(-0.5f, z, 1.0f));
+  float a = (q & 1) ? cr : sr;
+  float b = (q & 1) ? sr : cr;
+  *sn = (q & 2) ? -a : a;
+  *cs = ((q + 1) & 2) ? -b : b;
+}
+#endif
+GP_HD void fsincos(float x, float *sn, float *cs) {
+#if defined(__CUDA_ARCH__)
+  sincosf_fast(x, sn, cs);
+#else
+  *sn = sinf(x);
+  *cs = cosf(x);
+#endif
+}
+GP_HD double fexp(double x) { return exp(x); }
+GP_HD float fexp(float x) { return expf(x); }
+GP_HD double fsqrt(double x) { return sqrt(x); }
+GP_HD float fsqrt(float x) { return sqrtf(x); }
+GP_HD double ffma(double a, double b, double c) { return fma(a, b, c); }
+GP_HD float ffma(float a, float b, float c) { return fmaf(a, b, c); }
+
+template <class T> struct identity_of { typedef T type; };
+
 }  // namespace gp
 #endif

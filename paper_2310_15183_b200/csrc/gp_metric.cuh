@@ -36,34 +36,38 @@ struct MetricConst {
 };
 
 // Derivatives of (t, r, theta, phi, p_r, p_theta) with respect to the affine parameter, plus the
-// by-products the monitors want: sin, cos of theta and 2H.
-struct Rhs {
-  double dt, dr, dth, dph, dpr, dpth;
-  double s, c, H2;
-  double is;  // 1/sin(theta) (Schwarzschild, Kerr; 0 for Manko-Novikov)
+// by-products the monitors want: sin, cos of theta and 2H.  T is the
+// arithmetic type: double (required), float (the cfg.precision = 1 variant).
+template <class T>
+struct RhsT {
+  T dt, dr, dth, dph, dpr, dpth;
+  T s, c, H2;
+  T is;  // 1/sin(theta) (Schwarzschild, Kerr; 0 for Manko-Novikov)
 };
+typedef RhsT<double> Rhs;
 
 // ---- Schwarzschild --------------------------------------------------------------------------
 // 2H = -p_t^2/F + F p_r^2 + p_th^2/r^2 + p_ph^2/(r^2 s^2),  F = 1 - 2M/r   (eq 8 inverted)
-GP_HD void rhs_schwarzschild(const MetricConst &mc, double pt, double pph, double r, double th, double pr,
-                             double pth, Rhs &o) {
-  double s, c;
+template <class T>
+GP_HD void rhs_schwarzschild(const MetricConst &mc, T pt, T pph, T r, T th, T pr, T pth, RhsT<T> &o) {
+  T s, c;
   fsincos(th, &s, &c);
-  double ir = frcp(r);
-  double ir2 = ir * ir;
-  double F = 1.0 - 2.0 * mc.M * ir;
-  double iF = frcp(F);
-  double is = frcp(s);
-  double is2 = is * is;
-  double Fr = 2.0 * mc.M * ir2;            // dF/dr
-  double gpp = ir2 * is2;                  // g^{phi phi}
-  double pt_iF = pt * iF;
+  const T M = (T)mc.M;
+  T ir = frcp(r);
+  T ir2 = ir * ir;
+  T F = T(1) - T(2) * M * ir;
+  T iF = frcp(F);
+  T is = frcp(s);
+  T is2 = is * is;
+  T Fr = T(2) * M * ir2;              // dF/dr
+  T gpp = ir2 * is2;                  // g^{phi phi}
+  T pt_iF = pt * iF;
   o.dt = -pt_iF;
   o.dr = F * pr;
   o.dth = pth * ir2;
   o.dph = pph * gpp;
-  double ang = pth * pth + pph * pph * is2; // p_th^2 + p_ph^2/s^2
-  o.dpr = -0.5 * Fr * (pt_iF * pt_iF + pr * pr) + ang * ir2 * ir;
+  T ang = pth * pth + pph * pph * is2; // p_th^2 + p_ph^2/s^2
+  o.dpr = T(-0.5) * Fr * (pt_iF * pt_iF + pr * pr) + ang * ir2 * ir;
   o.dpth = c * is * pph * pph * gpp;
   o.H2 = -pt * pt_iF + F * pr * pr + ang * ir2;
   o.s = s;
@@ -79,40 +83,40 @@ GP_HD void rhs_schwarzschild(const MetricConst &mc, double pt, double pph, doubl
 // Written out operation by operation (half-derivatives, shared products, explicit fma): 53 FP64
 // instructions beside the sincos and the reciprocal, against 61 for the textbook arrangement — the
 // FP64 pipe is the bound, so the operation count is the run time.
-GP_HD void rhs_kerr(const MetricConst &mc, double pt, double pph, double r, double th, double pr, double pth,
-                    Rhs &o) {
-  double s, c;
+template <class T>
+GP_HD void rhs_kerr(const MetricConst &mc, T pt, T pph, T r, T th, T pr, T pth, RhsT<T> &o) {
+  T s, c;
   fsincos(th, &s, &c);
-  const double a = mc.a, a2 = mc.a2;
-  double r2 = r * r;
-  double rr = r2 + a2;
-  double a2c = a2 * c;
-  double Sig = fma(a2c, c, r2);
-  double Del = fma(mc.m2M, r, rr);
+  const T a = (T)mc.a, a2 = (T)mc.a2;
+  T r2 = r * r;
+  T rr = r2 + a2;
+  T a2c = a2 * c;
+  T Sig = ffma(a2c, c, r2);
+  T Del = ffma((T)mc.m2M, r, rr);
   // one reciprocal for the three denominators Sigma, Delta, s
-  double SD = Sig * Del;
-  double inv = frcp(SD * s);
-  double is = inv * SD;
-  double t1 = inv * s;
-  double iSig = t1 * Del;
-  double iDel = t1 * Sig;
-  double as = a * s;
-  double W = fma(pph, is, as * pt);
-  double P = fma(rr, pt, a * pph);
-  double PiD = P * iDel;
-  double pr2 = pr * pr;
-  double N = fma(-P, PiD, fma(W, W, fma(pth, pth, Del * pr2)));
-  double H2 = N * iSig;
-  o.dt = fma(-rr, PiD, as * W) * iSig;
-  o.dph = fma(-a, PiD, W * is) * iSig;
+  T SD = Sig * Del;
+  T inv = frcp(SD * s);
+  T is = inv * SD;
+  T t1 = inv * s;
+  T iSig = t1 * Del;
+  T iDel = t1 * Sig;
+  T as = a * s;
+  T W = ffma(pph, is, as * pt);
+  T P = ffma(rr, pt, a * pph);
+  T PiD = P * iDel;
+  T pr2 = pr * pr;
+  T N = ffma(-P, PiD, ffma(W, W, ffma(pth, pth, Del * pr2)));
+  T H2 = N * iSig;
+  o.dt = ffma(-rr, PiD, as * W) * iSig;
+  o.dph = ffma(-a, PiD, W * is) * iSig;
   o.dr = (pr * iSig) * Del;
   o.dth = pth * iSig;
   // dp_r = -(1/2 d_r N - r 2H)/Sigma,  1/2 d_r N = (r-M)(p_r^2 + (P/Delta)^2) - 2 r p_t P/Delta
-  double halfNr = fma(-2.0, (r * pt) * PiD, (r - mc.M) * fma(PiD, PiD, pr2));
-  o.dpr = fma(r, H2, -halfNr) * iSig;
+  T halfNr = ffma(T(-2), (r * pt) * PiD, (r - (T)mc.M) * ffma(PiD, PiD, pr2));
+  o.dpr = ffma(r, H2, -halfNr) * iSig;
   // dp_th = -(1/2 d_th N + a^2 s c 2H)/Sigma,  1/2 d_th N = W c (a p_t - p_ph/s^2)
-  double halfNth = (W * c) * fma(-(pph * is), is, a * pt);
-  o.dpth = -fma(a2c * s, H2, halfNth) * iSig;
+  T halfNth = (W * c) * ffma(-(pph * is), is, a * pt);
+  o.dpth = -ffma(a2c * s, H2, halfNth) * iSig;
   o.H2 = H2;
   o.s = s;
   o.c = c;
@@ -169,42 +173,42 @@ GP_HD MNCore<T> mn_core(const MetricConst &mc, const T &x, const T &y) {
 
 // 2H = -p_t^2/f + f (p_ph + omega p_t)^2/(Delta s^2) + f (Delta p_r^2 + p_th^2)/E,
 // Delta = k^2 (x^2-1) (eq 22), from the line element eq 20 (R4).
-GP_HD void rhs_manko_novikov(const MetricConst &mc, double pt, double pph, double r, double th, double pr,
-                             double pth, Rhs &o) {
-  double s, c;
+template <class T>
+GP_HD void rhs_manko_novikov(const MetricConst &mc, T pt, T pph, T r, T th, T pr, T pth, RhsT<T> &o) {
+  typedef Dual2T<T> D;
+  T s, c;
   fsincos(th, &s, &c);
-  const double k = mc.mn_k;
-  Dual2 x((r - mc.M) * mc.mn_inv_k, 1.0, 0.0);
-  Dual2 y(c, 0.0, 1.0);
-  MNCore<Dual2> m = mn_core<Dual2>(mc, x, y);
-  Dual2 Del = (k * k) * (sqr(x) - 1.0);
-  Dual2 s2(s * s, 0.0, -2.0 * c);          // sin^2 = 1 - y^2
-  Dual2 iDs = recip(Del * s2);
-  Dual2 iE = recip(m.E);
-  Dual2 iF = recip(m.f);
-  Dual2 L = pph + m.omega * pt;             // p_ph + omega p_t
-  Dual2 fL = m.f * L * iDs;                 // = dphi/dlambda
-  Dual2 fE = m.f * iE;                      // g^{th th}
-  Dual2 K = Del * (pr * pr) + pth * pth;
-  Dual2 H2 = fL * L + fE * K - (pt * pt) * iF;
+  const T k = (T)mc.mn_k, ik = (T)mc.mn_inv_k;
+  D x((r - (T)mc.M) * ik, T(1), T(0));
+  D y(c, T(0), T(1));
+  MNCore<D> m = mn_core<D>(mc, x, y);
+  D Del = (k * k) * (sqr(x) - T(1));
+  D s2(s * s, T(0), T(-2) * c);          // sin^2 = 1 - y^2
+  D iDs = recip(Del * s2);
+  D iE = recip(m.E);
+  D iF = recip(m.f);
+  D L = pph + m.omega * pt;               // p_ph + omega p_t
+  D fL = m.f * L * iDs;                   // = dphi/dlambda
+  D fE = m.f * iE;                        // g^{th th}
+  D K = Del * (pr * pr) + pth * pth;
+  D H2 = fL * L + fE * K - (pt * pt) * iF;
   o.dt = -pt * iF.v + m.omega.v * fL.v;
   o.dph = fL.v;
   o.dr = fE.v * Del.v * pr;
   o.dth = fE.v * pth;
-  o.dpr = -0.5 * H2.dx * mc.mn_inv_k;       // d/dr = (1/k) d/dx
-  o.dpth = 0.5 * H2.dy * s;                 // d/dtheta = -sin(theta) d/dy
+  o.dpr = T(-0.5) * H2.dx * ik;           // d/dr = (1/k) d/dx
+  o.dpth = T(0.5) * H2.dy * s;            // d/dtheta = -sin(theta) d/dy
   o.H2 = H2.v;
   o.s = s;
   o.c = c;
-  o.is = 0.0;
+  o.is = T(0);
 }
 
-template <int METRIC>
-GP_HD void rhs_eval(const MetricConst &mc, double pt, double pph, double r, double th, double pr, double pth,
-                    Rhs &o) {
-  if (METRIC == METRIC_SCHW) rhs_schwarzschild(mc, pt, pph, r, th, pr, pth, o);
-  else if (METRIC == METRIC_KERR) rhs_kerr(mc, pt, pph, r, th, pr, pth, o);
-  else rhs_manko_novikov(mc, pt, pph, r, th, pr, pth, o);
+template <int METRIC, class T>
+GP_HD void rhs_eval(const MetricConst &mc, T pt, T pph, T r, T th, T pr, T pth, RhsT<T> &o) {
+  if (METRIC == METRIC_SCHW) rhs_schwarzschild<T>(mc, pt, pph, r, th, pr, pth, o);
+  else if (METRIC == METRIC_KERR) rhs_kerr<T>(mc, pt, pph, r, th, pr, pth, o);
+  else rhs_manko_novikov<T>(mc, pt, pph, r, th, pr, pth, o);
 }
 
 // ---- covariant metric at a point (host: observer tetrad, row a3) ------------------------------

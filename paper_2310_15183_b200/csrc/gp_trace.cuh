@@ -23,6 +23,7 @@ struct TraceParams {
   MetricConst mc;
   CameraConst cc;
   int scheme;                       // 0 RK4 fixed h, 1 RK4 h = h_rel r, 2 DP5(4)
+  int precision;                    // 0 FP64, 1 FP32 (RK4 schemes only)
   int max_crossings;                // 0 = disk off
   double h, h_rel, rtol, atol, h_cap_rel;
   long long max_steps;
@@ -104,28 +105,33 @@ __device__ __forceinline__ double kepler_g(const MetricConst &mc, double r, doub
 }
 
 // Monitors of row a10 carried per lane.
-struct Monitors {
-  double h_max, q_drift, Q0, iQ0, sin_min, err_margin;
+template <class T>
+struct MonitorsT {
+  T h_max, q_drift, Q0, iQ0, sin_min, err_margin;
 };
+typedef MonitorsT<double> Monitors;
+
+__device__ __forceinline__ float dmax(float run, float cand) { return cand > run ? cand : run; }
+__device__ __forceinline__ float dmin(float run, float cand) { return cand < run ? cand : run; }
+__device__ __forceinline__ bool finite_d(float x) { return fabsf(x) <= 3.402823466e38f; }
 
 // Carter constant, exact off shell (reading R23): Q = p_th^2 + c^2 (p_ph^2/s^2 - a^2 p_t^2) - 2 a^2 c^2 H.
-template <int METRIC>
-__device__ __forceinline__ double carter_q(const MetricConst &mc, double pt, double pph, double pth,
-                                           const Rhs &o) {
-  if (METRIC == METRIC_MN) return 0.0;
-  const double a2 = (METRIC == METRIC_KERR) ? mc.a2 : 0.0;
-  double c2 = o.c * o.c;
+template <int METRIC, class T>
+__device__ __forceinline__ T carter_q(const MetricConst &mc, T pt, T pph, T pth, const RhsT<T> &o) {
+  if (METRIC == METRIC_MN) return T(0);
+  const T a2 = (METRIC == METRIC_KERR) ? (T)mc.a2 : T(0);
+  T c2 = o.c * o.c;
   return pth * pth + c2 * (pph * pph * o.is * o.is - a2 * pt * pt) - a2 * c2 * o.H2;
 }
 
-template <int METRIC>
-__device__ __forceinline__ void monitor_apply(Monitors &mo, double absH, double Q, double abss, bool first) {
+template <int METRIC, class T>
+__device__ __forceinline__ void monitor_apply(MonitorsT<T> &mo, T absH, T Q, T abss, bool first) {
   mo.h_max = dmax(mo.h_max, absH);
   mo.sin_min = dmin(mo.sin_min, abss);
   if (METRIC != METRIC_MN) {
     if (first) mo.Q0 = Q;
-    if (first) mo.iQ0 = frcp(dmax(1.0, fabs(Q)));
-    double d = fabs(Q - mo.Q0) * mo.iQ0;
+    if (first) mo.iQ0 = frcp(dmax(T(1), (T)fabs(Q)));
+    T d = (T)fabs(Q - mo.Q0) * mo.iQ0;
     mo.q_drift = dmax(mo.q_drift, d);
   }
 }

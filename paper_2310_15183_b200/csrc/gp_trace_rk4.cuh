@@ -6,6 +6,10 @@
 // same formula on dy/ds = F/F_w (reading R14).  Reading R31: in an ordinary step each state the
 // equations are evaluated at is first tested against the capture radius; the first hit ends the
 // ray as CAPTURED (then one landing step from y_n).
+//
+// T is the arithmetic type of the state and of Hamilton's equations: double, or float for the
+// single-precision variant BASELINE.json configs[4] asks for (cfg.precision = 1).  The ray is
+// always born in double (rows a2, a3) and the record is always written in double.
 #ifndef GP_TRACE_RK4_CUH_
 #define GP_TRACE_RK4_CUH_
 
@@ -14,18 +18,20 @@ namespace gp {
 
 constexpr int kParkSlotsRk4 = 7;  // trial state (r, th, pr, pth, t, ph, lambda) across an equator landing
 
-template <int METRIC, bool DISK>
+template <int METRIC, bool DISK, class T>
 __global__ void __launch_bounds__(kBlock) trace_rk4(const __grid_constant__ TraceParams P) {
-  extern __shared__ double park[];  // [kParkSlotsRk4][kBlock] when DISK
+  extern __shared__ double park_raw[];  // [kParkSlotsRk4][kBlock] of T when DISK
+  T *park = reinterpret_cast<T *>(park_raw);
   const MetricConst &mc = P.mc;
   const int tid = threadIdx.x;
+  const T r_cap = (T)P.r_cap, r_esc = (T)P.r_esc, half_pi = (T)kHalfPi;
 
   int mode = MODE_IDLE;
   long long slot = -1;
-  double pt = 0.0, pph = 0.0;
-  double t = 0.0, r = 0.0, th = 0.0, ph = 0.0, pr = 0.0, pth = 0.0, lam = 0.0;
-  double target = 0.0;
-  Monitors mo = {0.0, 0.0, 0.0, 1.0, 0.0, 0.0};
+  T pt = T(0), pph = T(0);
+  T t = T(0), r = T(0), th = T(0), ph = T(0), pr = T(0), pth = T(0), lam = T(0);
+  T target = T(0);
+  MonitorsT<T> mo = {T(0), T(0), T(0), T(1), T(0), T(0)};
   unsigned n_acc = 0, n_cross = 0, n_rec = 0, n_land = 0, status = 0;
   bool exhausted = false;
   unsigned long long tot_rays = 0, tot_steps = 0, tot_rhs = 0;
@@ -41,15 +47,16 @@ __global__ void __launch_bounds__(kBlock) trace_rk4(const __grid_constant__ Trac
         if (slot < 0) {
           exhausted = true;
         } else {
-          double alpha, beta;
+          double alpha, beta, dpt, dpr, dpth, dpph;
           alpha_beta(P.cc, P.cc.ray_begin + slot * P.cc.ray_stride, alpha, beta);
-          initial_momentum(P.cc, alpha, beta, pt, pr, pth, pph);
-          t = 0.0; r = P.cc.r_obs; th = P.cc.theta_obs; ph = P.cc.phi_obs; lam = 0.0;
+          initial_momentum(P.cc, alpha, beta, dpt, dpr, dpth, dpph);
+          pt = (T)dpt; pr = (T)dpr; pth = (T)dpth; pph = (T)dpph;
+          t = T(0); r = (T)P.cc.r_obs; th = (T)P.cc.theta_obs; ph = (T)P.cc.phi_obs; lam = T(0);
           mode = MODE_NORMAL;
           n_acc = n_cross = n_rec = n_land = 0;
-          mo.h_max = 0.0; mo.q_drift = 0.0; mo.Q0 = 0.0;
-          mo.sin_min = __longlong_as_double(0x7ff0000000000000LL);
-          mo.err_margin = __longlong_as_double(0x7ff0000000000000LL);
+          mo.h_max = T(0); mo.q_drift = T(0); mo.Q0 = T(0);
+          mo.sin_min = (T)__longlong_as_double(0x7ff0000000000000LL);
+          mo.err_margin = (T)__longlong_as_double(0x7ff0000000000000LL);
         }
       }
     }
@@ -59,79 +66,79 @@ __global__ void __launch_bounds__(kBlock) trace_rk4(const __grid_constant__ Trac
       bool finished = false;
       // stop tests at the top of every ordinary step (R18)
       if (mode == MODE_NORMAL &&
-          ((long long)n_acc >= P.max_steps || (P.lambda_max > 0.0 && lam >= P.lambda_max))) {
+          ((long long)n_acc >= P.max_steps || (P.lambda_max > 0.0 && (double)lam >= P.lambda_max))) {
         status = GP_RAY_MAXSTEPS;
         finished = true;
       }
       if (!finished) {
         const bool normal = (mode == MODE_NORMAL);
         const bool land_r = (mode == MODE_LAND_R);
-        const double s = normal ? (P.scheme == 0 ? P.h : P.h_rel * r) : (land_r ? (target - r) : (target - th));
+        const T s = normal ? (P.scheme == 0 ? (T)P.h : (T)P.h_rel * r) : (land_r ? (target - r) : (target - th));
         // Landing steps are 1 in several hundred: their divisor work (Henon's 1/F_w) sits behind a
         // warp-uniform branch taken only when some lane of this convergence group is landing.
         const bool any_land = __any_sync(__activemask(), !normal);
-        double sl = 1.0;  // weighted sum of 1/F_w: d(lambda)/ds of a landing step (unused otherwise)
+        T sl = T(1);  // weighted sum of 1/F_w: d(lambda)/ds of a landing step (unused otherwise)
 #define GP_HENON(weight, first)                                                   \
   if (any_land) {                                                                 \
-    double iv = normal ? 1.0 : rcp_nr(land_r ? o.dr : o.dth);                     \
+    T iv = normal ? T(1) : frcp(land_r ? o.dr : o.dth);                           \
     o.dt *= iv; o.dr *= iv; o.dth *= iv; o.dph *= iv; o.dpr *= iv; o.dpth *= iv;  \
-    sl = (first) ? iv : sl + (weight) * iv;                                       \
+    sl = (first) ? iv : sl + T(weight) * iv;                                      \
   }
-        Rhs o;
+        RhsT<T> o;
         // k1 = F(y_n)
         rhs_eval<METRIC>(mc, pt, pph, r, th, pr, pth, o);
         if (normal)
-          monitor_apply<METRIC>(mo, fabs(0.5 * o.H2), carter_q<METRIC>(mc, pt, pph, pth, o), fabs(o.s),
+          monitor_apply<METRIC>(mo, (T)fabs(T(0.5) * o.H2), carter_q<METRIC>(mc, pt, pph, pth, o), (T)fabs(o.s),
                                 n_acc == 0);
         GP_HENON(1.0, true)
-        double st = o.dt, sr = o.dr, sth = o.dth, sph = o.dph, spr = o.dpr, spth = o.dpth;  // k1 + 2k2 + 2k3 + k4
-        const double hs = 0.5 * s;
+        T st = o.dt, sr = o.dr, sth = o.dth, sph = o.dph, spr = o.dpr, spth = o.dpth;  // k1 + 2k2 + 2k3 + k4
+        const T hs = T(0.5) * s;
         // k2 = F(y_n + h/2 k1)
-        double yr = r + hs * o.dr;
-        bool captured = normal && (yr < P.r_cap);
+        T yr = r + hs * o.dr;
+        bool captured = normal && (yr < r_cap);
         rhs_eval<METRIC>(mc, pt, pph, yr, th + hs * o.dth, pr + hs * o.dpr, pth + hs * o.dpth, o);
         GP_HENON(2.0, false)
-        st += 2.0 * o.dt; sr += 2.0 * o.dr; sth += 2.0 * o.dth; sph += 2.0 * o.dph; spr += 2.0 * o.dpr;
-        spth += 2.0 * o.dpth;
+        st += T(2) * o.dt; sr += T(2) * o.dr; sth += T(2) * o.dth; sph += T(2) * o.dph; spr += T(2) * o.dpr;
+        spth += T(2) * o.dpth;
         // k3 = F(y_n + h/2 k2)
         yr = r + hs * o.dr;
-        captured = captured || (normal && (yr < P.r_cap));
+        captured = captured || (normal && (yr < r_cap));
         rhs_eval<METRIC>(mc, pt, pph, yr, th + hs * o.dth, pr + hs * o.dpr, pth + hs * o.dpth, o);
         GP_HENON(2.0, false)
-        st += 2.0 * o.dt; sr += 2.0 * o.dr; sth += 2.0 * o.dth; sph += 2.0 * o.dph; spr += 2.0 * o.dpr;
-        spth += 2.0 * o.dpth;
+        st += T(2) * o.dt; sr += T(2) * o.dr; sth += T(2) * o.dth; sph += T(2) * o.dph; spr += T(2) * o.dpr;
+        spth += T(2) * o.dpth;
         // k4 = F(y_n + h k3)
         yr = r + s * o.dr;
-        captured = captured || (normal && (yr < P.r_cap));
+        captured = captured || (normal && (yr < r_cap));
         rhs_eval<METRIC>(mc, pt, pph, yr, th + s * o.dth, pr + s * o.dpr, pth + s * o.dpth, o);
         GP_HENON(1.0, false)
         st += o.dt; sr += o.dr; sth += o.dth; sph += o.dph; spr += o.dpr; spth += o.dpth;
 #undef GP_HENON
-        const double w = s * dp.sixth;
-        const double nt = t + w * st, nr = r + w * sr, nth = th + w * sth, nph = ph + w * sph,
-                     npr = pr + w * spr, npth = pth + w * spth;
+        const T w = s * (T)dp.sixth;
+        const T nt = t + w * st, nr = r + w * sr, nth = th + w * sth, nph = ph + w * sph,
+                npr = pr + w * spr, npth = pth + w * spth;
 
         if (normal) {
-          const double ysum = ((nt + nr) + (nth + nph)) + (npr + npth);
+          const T ysum = ((nt + nr) + (nth + nph)) + (npr + npth);
           const bool nonfinite = !captured && !finite_d(ysum);
           if (!nonfinite) ++n_acc;
           if (nonfinite) {
             status = GP_RAY_NONFINITE;   // record = last finite state y_n
             finished = true;
-          } else if (captured || nr > P.r_esc || nr < P.r_cap) {
-            const bool esc = !captured && nr > P.r_esc;
+          } else if (captured || nr > r_esc || nr < r_cap) {
+            const bool esc = !captured && nr > r_esc;
             status = esc ? GP_RAY_ESCAPED : GP_RAY_CAPTURED;
-            target = esc ? P.r_esc : P.r_cap;
+            target = esc ? r_esc : r_cap;
             mode = MODE_LAND_R;
           } else {
             bool commit = true;
-            if ((th - kHalfPi) * (nth - kHalfPi) < 0.0) {
+            if ((th - half_pi) * (nth - half_pi) < T(0)) {
               ++n_cross;
               if (DISK && n_rec < (unsigned)P.max_crossings) {
-                double *pk = park + tid;
+                T *pk = park + tid;
                 pk[0 * kBlock] = nr; pk[1 * kBlock] = nth; pk[2 * kBlock] = npr; pk[3 * kBlock] = npth;
                 pk[4 * kBlock] = nt; pk[5 * kBlock] = nph; pk[6 * kBlock] = lam + s;
-                target = kHalfPi;
+                target = half_pi;
                 mode = MODE_LAND_TH;
                 commit = false;
               }
@@ -147,13 +154,13 @@ __global__ void __launch_bounds__(kBlock) trace_rk4(const __grid_constant__ Trac
         } else {  // MODE_LAND_TH
           ++n_land;
           if (DISK) {
-            const double rc = nr;
+            const double rc = (double)nr;
             if (rc >= P.disk_r_in && rc <= P.disk_r_out) {
               P.disk[slot].r_cross[n_rec] = rc;
-              P.disk[slot].g[n_rec] = kepler_g(mc, rc, pt, pph);
+              P.disk[slot].g[n_rec] = kepler_g(mc, rc, (double)pt, (double)pph);
               ++n_rec;
             }
-            const double *pk = park + tid;
+            const T *pk = park + tid;
             r = pk[0 * kBlock]; th = pk[1 * kBlock]; pr = pk[2 * kBlock]; pth = pk[3 * kBlock];
             t = pk[4 * kBlock]; ph = pk[5 * kBlock]; lam = pk[6 * kBlock];
           }
@@ -163,8 +170,11 @@ __global__ void __launch_bounds__(kBlock) trace_rk4(const __grid_constant__ Trac
 
       if (finished) {
         const unsigned n_rhs = 4u * n_acc + 3u * n_land;
-        store_record(P.rays + slot, t, r, th, ph, pr, pth, lam, pt, pph, mo, status, n_acc, 0u, n_cross, n_rec,
-                     n_rhs);
+        Monitors mod = {(double)mo.h_max, (double)mo.q_drift, 0.0, 0.0, (double)mo.sin_min, (double)mo.err_margin};
+        // the exit surface is exact in the record whatever the arithmetic type
+        const double r_rec = (status == GP_RAY_ESCAPED) ? P.r_esc : (status == GP_RAY_CAPTURED ? P.r_cap : (double)r);
+        store_record(P.rays + slot, (double)t, r_rec, (double)th, (double)ph, (double)pr, (double)pth, (double)lam,
+                     (double)pt, (double)pph, mod, status, n_acc, 0u, n_cross, n_rec, n_rhs);
         if (DISK) {
           const double qnan = __longlong_as_double(0x7ff8000000000000LL);
           for (unsigned i = n_rec; i < 3u; ++i) {

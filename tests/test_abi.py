@@ -106,7 +106,8 @@ BAD = [
     ("scheme 9", lambda m, c, g: setattr(g, "scheme", 9), None, api.GP_E_BAD_PARAM),
     ("r_escape inside r_obs", lambda m, c, g: setattr(g, "r_escape", 10.0), None, api.GP_E_BAD_PARAM),
     ("4 crossings", lambda m, c, g: setattr(g, "max_crossings", 4), None, api.GP_E_BAD_PARAM),
-    ("FP32 variant not built", lambda m, c, g: setattr(g, "precision", 1), None, api.GP_E_UNSUPPORTED),
+    ("FP32 with the adaptive scheme", lambda m, c, g: setattr(g, "precision", 1), None, api.GP_E_UNSUPPORTED),
+    ("precision 2", lambda m, c, g: setattr(g, "precision", 2), None, api.GP_E_UNSUPPORTED),
     ("projection 1", lambda m, c, g: setattr(c, "projection", 1), None, api.GP_E_UNSUPPORTED),
 ]
 

@@ -359,3 +359,45 @@ def test_manko_novikov_equatorial_mirror_symmetry_on_the_gpu(gp):
     assert rel_err(up["phi"], dn["phi"])[ok].max() <= 1e-8
     assert rel_err(up["lambda"], dn["lambda"])[ok].max() <= 1e-9
     assert (img["status"] == 2).sum() > 100 and (img["status"] == 0).sum() > 15000
+
+
+# ---- the single-precision variant (BASELINE.json configs[4]: "an FP32 variant with its own stated
+# tolerance"; north_star: <= 1e-4) ------------------------------------------------------------------
+@pytest.mark.parametrize("name,cfgo,sel", [("C1", {}, (0, None, 1)),
+                                           ("C5a", dict(max_steps=20000), (1, None, 4099)),
+                                           ("C5b", dict(max_steps=20000), (1, None, 16411))])
+def test_fp32_variant_against_the_fp64_oracle(gp, O, name, cfgo, sel):
+    """cfg.precision = 1: state and Hamilton's equations in FP32 (RK4 schemes), compared with the
+    FP64 oracle.  Stated tolerance: |delta| <= 1e-4 max(1, |value|) on raw exit
+    theta, phi, lambda, t for at least 99.9 % of smooth escaped rays and <= 1e-3 for all of them.
+    Smooth here: sin(theta)_min >= 0.02 (the 1/sin^2 terms cost 1/s of the 6e-8 unit roundoff) and the
+    oracle's own rounding spread <= 1e-14 (x 2^29, the ratio of the unit roundoffs, that is 5e-6).
+    Captured rays: status only — t and phi diverge like ln(Delta) at the capture surface, where
+    Delta = r^2 - 2Mr + a^2 keeps 4 digits in FP32."""
+    w = W.workload(name)
+    w["cfg"].update(cfgo)
+    b, c, s = W.ray_selection(w, *sel)
+    orc, _ = O.trace(w, b, c, s)
+    probe, _ = O.trace(w, b, c, s, rounding_probe=True)
+    w["cfg"]["precision"] = 1
+    rays, _, counters = gp.api.trace_workload(w, b, c, s)
+    assert counters[1] == c
+    from parity_rules import rounding_spread
+    spread = rounding_spread(orc, probe)
+    sensitive = spread > 1e-14
+    mism = rays["status"].astype(np.int64) != orc["status"]
+    assert not (mism & ~sensitive).any(), f"status differs on {np.count_nonzero(mism & ~sensitive)} unflagged rays"
+    assert mism.mean() <= 0.005
+    esc = ~mism & (orc["status"] == 0)
+    smooth = esc & ~sensitive & (orc["sin_theta_min"] >= 0.02)
+    assert smooth.sum() >= 0.85 * esc.sum()
+    err = np.max([rel_err(rays[f], orc[f]) for f in FIELDS], axis=0)[smooth]
+    assert err.max() <= 1e-3, err.max()
+    assert (err <= 1e-4).mean() >= 0.999, (err > 1e-4).sum()
+    assert np.median(err) <= 5e-5
+    landed = ~mism & (orc["status"] <= 1)
+    assert np.array_equal(rays["r"][landed], orc["r"][landed])       # the exit surface is exact
+    dn = np.abs(rays["n_accepted"].astype(np.int64) - orc["n_accepted"])[smooth]
+    assert (dn <= 2).mean() >= 0.99
+    print(name, "fp32: smooth", int(smooth.sum()), "median", float(np.median(err)), "max", float(err.max()),
+          "status mismatches", int(mism.sum()))
