@@ -144,11 +144,14 @@ GP_HD void fsincos(double x, double *sn, double *cs) {
 #endif
 }
 
-// FP32 forms for the single-precision variant (cfg.precision = 1): the
-// correctly rounded reciprocal and the library's full-range sincosf / expf / sqrtf.
+// FP32 forms for the single-precision variant (cfg.precision = 1).
 GP_HD float frcp(float x) {
 #if defined(__CUDA_ARCH__)
-  return __frcp_rn(x);
+  // MUFU.RCP (about 1 ulp) + one Newton step, no denormal / slow-path branch (the integrator's finite
+  // tests catch x = 0)
+  float y;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return fmaf(y, fmaf(-x, y, 1.0f), y);
 #else
   return 1.0f / x;
 #endif
