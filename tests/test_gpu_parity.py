@@ -401,3 +401,36 @@ def test_fp32_variant_against_the_fp64_oracle(gp, O, name, cfgo, sel):
     assert (dn <= 2).mean() >= 0.99
     print(name, "fp32: smooth", int(smooth.sum()), "median", float(np.median(err)), "max", float(err.max()),
           "status mismatches", int(mism.sum()))
+
+
+def test_largest_sweep_8192_squared_sampled(gp, O):
+    """BASELINE.json configs[4] at its largest: 4096 x 4096 with 2 x 2 supersampling = 67 108 864 rays,
+    8.6 GB of records (byte offsets beyond 2^32), one launch.  The records stay on the device; the
+    counters, the status census and a scattered sample of records (compared with the oracle tracing
+    exactly those rays) come back."""
+    import torch
+    w = W.workload("C5a", supersample=2)
+    n = W.n_rays(w)
+    assert n == 67108864
+    cam = gp.api.camera_struct(w["camera"])
+    rays = torch.empty(n * 128, dtype=torch.uint8, device="cuda")
+    counters = torch.empty(64, dtype=torch.uint8, device="cuda")
+    gp.gp_trace(w["metric"]["id"], gp.api.metric_struct(w["metric"]), cam, gp.api.cfg_struct(w["cfg"]),
+                rays, None, counters)
+    torch.cuda.synchronize()
+    cnt = counters.cpu().numpy().view("<u8")
+    assert cnt[1] == n and cnt[0] >= n
+    rec = rays.view(n, 128)
+    status = rec[:, 104:108].contiguous().view(torch.int32).view(n)          # u32 status at byte 104
+    census = torch.bincount(status.to(torch.int64), minlength=5).cpu().numpy()
+    assert census[2:].sum() == 0 and census[0] > 0.9 * n and census[1] > 0.01 * n
+    # sampled parity: every 262 147th ray from ray 5, including slots far beyond the 2^32-byte mark
+    b, s = 5, 262147
+    c = (n - b + s - 1) // s
+    idx = torch.arange(b, n, s, device="cuda")
+    sample = rec[idx].cpu().numpy().view(gp.api.RAY_DTYPE).reshape(-1)
+    orc, _ = O.trace(w, b, c, s)
+    probe, _ = O.trace(w, b, c, s, rounding_probe=True)
+    check_parity(w, sample, orc, probe, "8192^2 sample", max_flagged_fraction=0.05)
+    del rays, rec
+    torch.cuda.empty_cache()
