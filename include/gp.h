@@ -195,6 +195,50 @@ int gp_eval_rhs(int metric_id, const gp_metric_params *metric, const void *state
 int gp_probe_fp64_fma(int64_t iters, void *scratch, size_t scratch_bytes, double *flops_out,
                       void *cuda_stream);
 
+/* ---- image formation (the drawing script's kernel that
+ * maps "output positions" to colours) -------
+ * One RGBA8 pixel per image pixel from the ray records of a finished trace of the same camera
+ * (ray = (j*S + sj)*W*S + (i*S + si), S = supersample; the S*S sub-ray colours are averaged).
+ * Per sub-ray, in FP64 with individually rounded operations (bit-exact against any IEEE-754
+ * implementation of the same formulas):
+ *   status != ESCAPED : shadow colour (0,0,0); in mode 2 (0,1,1) (cyan).
+ *   otherwise canonicalise the raw exit angles without transcendentals:
+ *     th = theta - 2pi*floor(theta/2pi); ph = phi; if (th > pi) { th = 2pi - th; ph = ph + pi; }
+ *     ph = ph - 2pi*floor(ph/2pi);
+ *   mode 0 (celestial grid, L404): base colour PALETTE8[4*(th >= pi/2) + min(3, floor(ph/(pi/2)))];
+ *     a point within grid_half_width_deg of a multiple of grid_step_deg in th or in ph takes the
+ *     line colour (0.05, 0.05, 0.05).
+ *   mode 1 (background texture with bilinear filtering, L422; procedural stand-in for the ESO
+ *     panorama): equirectangular tex_width x tex_height texels, texel (i, j) = the three low bytes
+ *     of SplitMix64(tex_seed * 0x9E3779B97F4A7C15 + j * tex_width + i) / 255; sample at
+ *     u = ph/(2pi)*tex_width - 0.5 (wrapping), v = th/pi*tex_height - 0.5 (clamped).
+ *   mode 2 (exit-time bands, L430): PALETTE6[floor(|t| / time_period) mod 6].
+ *   disk overlay (L735; needs `disk`; takes precedence over everything above, the disk is opaque):
+ *     if the first recorded crossing exists (r_cross[0] is not NaN), the colour is
+ *     g < 1: blue (0.1,0.2,1) -> white by (g - g_lo)/(1 - g_lo);  g >= 1: white -> red (1,0.1,0.1)
+ *     by (g - 1)/(g_hi - 1), both parameters clamped to [0, 1].
+ *   pixel byte = floor(255 * mean + 0.5), alpha = 255.
+ * PALETTE8 = (.85,.25,.25) (.25,.75,.25) (.25,.35,.9) (.9,.8,.2) (.55,.15,.15) (.15,.45,.15)
+ * (.15,.2,.6) (.6,.5,.1); PALETTE6 = (.9,.1,.1) (.9,.6,.1) (.8,.9,.1) (.1,.8,.2) (.1,.5,.9) (.6,.1,.9).
+ * rays: DEVICE, n = W*H*S*S gp_ray_record; disk: DEVICE n gp_disk_record or NULL (required when
+ * disk_overlay != 0); rgba8: DEVICE, W*H*4 bytes, row j = 0 first.  HBM-bound: reads 128 (+48) bytes
+ * per sub-ray, writes 4 bytes per pixel.  GP_E_BAD_PARAM on non-positive sizes, unknown mode,
+ * non-positive grid / period / texture sizes for the mode in use, g_lo >= 1 or g_hi <= 1.        */
+typedef struct gp_shade_cfg {
+  int32_t width, height, supersample;
+  int32_t mode;                 /* 0 celestial grid, 1 procedural texture, 2 exit-time bands */
+  double grid_step_deg, grid_half_width_deg;
+  int32_t tex_width, tex_height;
+  uint64_t tex_seed;
+  double time_period;
+  int32_t disk_overlay;         /* 0 off, 1 colour the first recorded disk crossing by g     */
+  int32_t reserved_;
+  double g_lo, g_hi;
+} gp_shade_cfg;
+
+int gp_shade(const gp_shade_cfg *cfg, const void *rays, size_t rays_bytes, const void *disk,
+             size_t disk_bytes, void *rgba8, size_t rgba_bytes, void *cuda_stream);
+
 /* Horizon radius r_H and prograde ISCO radius used by the library for these parameters
  * (r_isco = NaN for GP_MANKO_NOVIKOV).  Host-only helper.                               */
 int gp_metric_radii(int metric_id, const gp_metric_params *metric, double *r_horizon,

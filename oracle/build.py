@@ -16,23 +16,24 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "gp_oracle.cpp")
+SRC_SHADE = os.path.join(HERE, "gp_shade_oracle.cpp")
 LIB = os.path.join(HERE, "libgp_oracle.so")
 LIB_FMA = os.path.join(HERE, "libgp_oracle_fma.so")
 
 
 def build(force: bool = False) -> str:
-    deps = [SRC, os.path.join(HERE, "gp_oracle.h")]
+    deps = [SRC, SRC_SHADE, os.path.join(HERE, "gp_oracle.h")]
     if (not force and os.path.exists(LIB)
             and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in deps)):
         return LIB
     cmd = ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fcx-limited-range", "-fopenmp",
-           "-fPIC", "-shared", "-Wall", "-Wextra", "-o", LIB, SRC]
+           "-fPIC", "-shared", "-Wall", "-Wextra", "-o", LIB, SRC, SRC_SHADE]
     subprocess.check_call(cmd)
     return LIB
 
 
 def build_rounding_probe(force: bool = False) -> str:
-    deps = [SRC, os.path.join(HERE, "gp_oracle.h")]
+    deps = [SRC, SRC_SHADE, os.path.join(HERE, "gp_oracle.h")]
     if (not force and os.path.exists(LIB_FMA)
             and all(os.path.getmtime(LIB_FMA) >= os.path.getmtime(d) for d in deps)):
         return LIB_FMA
@@ -40,7 +41,7 @@ def build_rounding_probe(force: bool = False) -> str:
         if " fma" not in f.read():
             raise RuntimeError("the rounding probe needs a host CPU with FMA instructions")
     cmd = ["g++", "-std=c++17", "-O2", "-ffp-contract=fast", "-mfma", "-fcx-limited-range",
-           "-fopenmp", "-fPIC", "-shared", "-o", LIB_FMA, SRC]
+           "-fopenmp", "-fPIC", "-shared", "-o", LIB_FMA, SRC, SRC_SHADE]
     subprocess.check_call(cmd)
     return LIB_FMA
 

@@ -218,5 +218,62 @@ def trace_one(workload, alpha, beta, path_capacity=0):
     return out[0], (path[: n.value] if path is not None else None)
 
 
+# ---- image formation (gp_shade_oracle.cpp) --------------------------------------------------------
+class OrcShadeCfg(C.Structure):
+    _fields_ = [("width", _i64), ("height", _i64), ("supersample", _i64), ("mode", _i64),
+                ("grid_step_deg", _f64), ("grid_half_width_deg", _f64),
+                ("tex_width", _i64), ("tex_height", _i64), ("tex_seed", C.c_uint64),
+                ("time_period", _f64), ("disk_overlay", _i64), ("g_lo", _f64), ("g_hi", _f64)]
+
+
+def _shade_cfg(d):
+    return OrcShadeCfg(d["width"], d["height"], d.get("supersample", 1), d["mode"],
+                       d.get("grid_step_deg", 15.0), d.get("grid_half_width_deg", 0.5),
+                       d.get("tex_width", 1), d.get("tex_height", 1), d.get("tex_seed", 0),
+                       d.get("time_period", 1.0), d.get("disk_overlay", 0), d.get("g_lo", 0.3), d.get("g_hi", 1.5))
+
+
+def splitmix64(z):
+    f = lib().orc_splitmix64
+    f.argtypes, f.restype = [C.c_uint64], C.c_uint64
+    return f(z)
+
+
+def canonical_angles(theta, phi):
+    out = np.empty(2)
+    f = lib().orc_canonical_angles
+    f.argtypes, f.restype = [_f64, _f64, C.POINTER(_f64)], None
+    f(float(theta), float(phi), _dp(out))
+    return out
+
+
+def shade_ray(cfg, status, theta, phi, t, disk_r0=float("nan"), disk_g0=float("nan")):
+    out = np.empty(3)
+    f = lib().orc_shade_ray
+    f.argtypes, f.restype = [C.POINTER(OrcShadeCfg), _i64, _f64, _f64, _f64, _f64, _f64, C.POINTER(_f64)], None
+    f(C.byref(_shade_cfg(cfg)), int(status), float(theta), float(phi), float(t), float(disk_r0), float(disk_g0),
+      _dp(out))
+    return out
+
+
+def shade(cfg, status, theta, phi, t, disk_r0=None, disk_g0=None):
+    """RGBA8 image (H, W, 4) from per-sub-ray arrays of n = W*H*S*S entries."""
+    c = _shade_cfg(cfg)
+    n = c.width * c.height * c.supersample ** 2
+    st = np.ascontiguousarray(status, dtype=np.int64)
+    arr = [np.ascontiguousarray(a, dtype=np.float64) for a in (theta, phi, t)]
+    assert st.size == n and all(a.size == n for a in arr)
+    dr = np.ascontiguousarray(disk_r0, dtype=np.float64) if disk_r0 is not None else None
+    dg = np.ascontiguousarray(disk_g0, dtype=np.float64) if disk_g0 is not None else None
+    out = np.zeros((c.height, c.width, 4), dtype=np.uint8)
+    f = lib().orc_shade
+    P = C.POINTER
+    f.argtypes = [P(OrcShadeCfg), P(_i64), P(_f64), P(_f64), P(_f64), P(_f64), P(_f64), C.c_void_p]
+    f.restype = C.c_int
+    _check(f(C.byref(c), st.ctypes.data_as(P(_i64)), _dp(arr[0]), _dp(arr[1]), _dp(arr[2]),
+             _dp(dr) if dr is not None else None, _dp(dg) if dg is not None else None, out.ctypes.data), "shade")
+    return out
+
+
 def host_threads():
     return os.cpu_count() or 1
