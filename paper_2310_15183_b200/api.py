@@ -43,6 +43,14 @@ class gp_integrator_cfg(C.Structure):
                 ("max_crossings", _i32), ("reserved_", _i32)]
 
 
+class gp_shade_cfg(C.Structure):
+    _fields_ = [("width", _i32), ("height", _i32), ("supersample", _i32), ("mode", _i32),
+                ("grid_step_deg", _f64), ("grid_half_width_deg", _f64),
+                ("tex_width", _i32), ("tex_height", _i32), ("tex_seed", _u64),
+                ("time_period", _f64), ("disk_overlay", _i32), ("reserved_", _i32),
+                ("g_lo", _f64), ("g_hi", _f64)]
+
+
 class gp_out_buffers(C.Structure):
     _fields_ = [("rays", C.c_void_p), ("rays_bytes", C.c_size_t),
                 ("disk", C.c_void_p), ("disk_bytes", C.c_size_t),
@@ -59,7 +67,7 @@ RAY_DTYPE = np.dtype([
 DISK_DTYPE = np.dtype([("r_cross", "<f8", (3,)), ("g", "<f8", (3,))])
 assert RAY_DTYPE.itemsize == 128 and DISK_DTYPE.itemsize == 48
 
-EXPORTS = ("gp_trace", "gp_trace_host", "gp_init_conditions", "gp_eval_metric", "gp_eval_rhs",
+EXPORTS = ("gp_shade", "gp_trace", "gp_trace_host", "gp_init_conditions", "gp_eval_metric", "gp_eval_rhs",
            "gp_probe_fp64_fma", "gp_metric_radii", "gp_ray_record_size", "gp_disk_record_size",
            "gp_counters_size", "gp_version", "gp_strerror")
 
@@ -79,6 +87,8 @@ def _load():
     L.gp_eval_rhs.argtypes = [C.c_int, P(gp_metric_params), vp, _i64, vp, sz, vp]
     L.gp_probe_fp64_fma.argtypes = [_i64, vp, sz, P(_f64), vp]
     L.gp_metric_radii.argtypes = [C.c_int, P(gp_metric_params), P(_f64), P(_f64)]
+    L.gp_shade.argtypes = [P(gp_shade_cfg), vp, sz, vp, sz, vp, sz, vp]
+    L.gp_shade.restype = C.c_int
     for n in ("gp_trace", "gp_trace_host", "gp_init_conditions", "gp_eval_metric", "gp_eval_rhs",
               "gp_probe_fp64_fma", "gp_metric_radii", "gp_version"):
         getattr(L, n).restype = C.c_int
@@ -201,6 +211,22 @@ def gp_probe_fp64_fma(iters, scratch, stream=None):
     _check(lib.gp_probe_fp64_fma(int(iters), p, n, C.byref(flops), _stream_ptr(stream)),
            "gp_probe_fp64_fma")
     return flops.value
+
+
+def shade_struct(d):
+    return gp_shade_cfg(int(d["width"]), int(d["height"]), int(d.get("supersample", 1)), int(d["mode"]),
+                        d.get("grid_step_deg", 15.0), d.get("grid_half_width_deg", 0.5),
+                        int(d.get("tex_width", 1)), int(d.get("tex_height", 1)), int(d.get("tex_seed", 0)),
+                        d.get("time_period", 1.0), int(d.get("disk_overlay", 0)), 0,
+                        d.get("g_lo", 0.3), d.get("g_hi", 1.5))
+
+
+def gp_shade(cfg, rays, disk, rgba8, stream=None):
+    """Enqueue the image-formation kernel: rays / disk / rgba8 are CUDA uint8 tensors (disk may be None)."""
+    p, n = _dev(rays)
+    q, m = _dev(disk)
+    o, k = _dev(rgba8)
+    _check(lib.gp_shade(C.byref(cfg), p, n, q, m, o, k, _stream_ptr(stream)), "gp_shade")
 
 
 def gp_metric_radii(metric_id, metric):

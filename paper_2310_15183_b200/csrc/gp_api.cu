@@ -8,6 +8,7 @@
 
 #include "../../include/gp.h"
 #include "gp_trace.cuh"
+#include "gp_shade.cuh"
 
 static_assert(sizeof(gp_ray_record) == 128, "gp_ray_record must be 128 bytes");
 static_assert(sizeof(gp_disk_record) == 48, "gp_disk_record must be 48 bytes");
@@ -442,6 +443,47 @@ int gp_probe_fp64_fma(int64_t iters, void *scratch, size_t scratch_bytes, double
   k_probe_fma<<<blocks, threads, 0, (cudaStream_t)cuda_stream>>>(iters, 0.5, (double *)scratch);
   GP_CUDA(cudaGetLastError());
   *flops_out = 2.0 * 64.0 * (double)iters * (double)blocks * (double)threads;
+  return GP_OK;
+}
+
+int gp_shade(const gp_shade_cfg *cfg, const void *rays, size_t rays_bytes, const void *disk, size_t disk_bytes,
+             void *rgba8, size_t rgba_bytes, void *cuda_stream) {
+  if (!cfg || !rays || !rgba8) return GP_E_NULL;
+  if (cfg->width <= 0 || cfg->height <= 0 || cfg->supersample <= 0 || cfg->supersample > 16) return GP_E_BAD_PARAM;
+  if (cfg->mode < 0 || cfg->mode > 2) return GP_E_BAD_PARAM;
+  if (cfg->mode == 0 && !(cfg->grid_step_deg > 0.0 && cfg->grid_half_width_deg >= 0.0 &&
+                          isfinite(cfg->grid_step_deg) && isfinite(cfg->grid_half_width_deg)))
+    return GP_E_BAD_PARAM;
+  if (cfg->mode == 1 && (cfg->tex_width <= 0 || cfg->tex_height <= 0 || cfg->tex_width > (1 << 30) ||
+                         cfg->tex_height > (1 << 30)))
+    return GP_E_BAD_PARAM;
+  if (cfg->mode == 2 && !(cfg->time_period > 0.0 && isfinite(cfg->time_period))) return GP_E_BAD_PARAM;
+  if (cfg->disk_overlay != 0 && cfg->disk_overlay != 1) return GP_E_BAD_PARAM;
+  if (cfg->disk_overlay) {
+    if (!disk) return GP_E_NULL;
+    if (!(cfg->g_lo < 1.0) || !(cfg->g_hi > 1.0) || !isfinite(cfg->g_lo) || !isfinite(cfg->g_hi)) return GP_E_BAD_PARAM;
+  }
+  const long long S = cfg->supersample;
+  const size_t n = (size_t)cfg->width * (size_t)cfg->height * (size_t)(S * S);
+  const size_t npix = (size_t)cfg->width * (size_t)cfg->height;
+  if (rays_bytes < n * sizeof(gp_ray_record)) return GP_E_SIZE;
+  if (cfg->disk_overlay && disk_bytes < n * sizeof(gp_disk_record)) return GP_E_SIZE;
+  if (rgba_bytes < npix * 4) return GP_E_SIZE;
+  ShadeParams P;
+  memset(&P, 0, sizeof(P));
+  P.W = cfg->width; P.H = cfg->height; P.S = S;
+  P.mode = cfg->mode; P.disk_overlay = cfg->disk_overlay;
+  const double pi = 3.14159265358979323846;
+  P.step_rad = cfg->grid_step_deg * (pi / 180.0);
+  P.hw_rad = cfg->grid_half_width_deg * (pi / 180.0);
+  P.tw = cfg->tex_width; P.th = cfg->tex_height; P.tex_seed = cfg->tex_seed;
+  P.time_period = cfg->time_period; P.g_lo = cfg->g_lo; P.g_hi = cfg->g_hi;
+  P.rays = (const gp_ray_record *)rays;
+  P.disk = (const gp_disk_record *)disk;
+  P.rgba = (unsigned char *)rgba8;
+  const unsigned grid = (unsigned)((npix + 255) / 256);
+  k_shade<<<grid, 256, 0, (cudaStream_t)cuda_stream>>>(P);
+  GP_CUDA(cudaGetLastError());
   return GP_OK;
 }
 
