@@ -204,11 +204,30 @@ GP_HD void rhs_manko_novikov(const MetricConst &mc, T pt, T pph, T r, T th, T pr
   o.is = T(0);
 }
 
-template <int METRIC, class T>
+#if defined(__CUDACC__)
+// The Manko-Novikov evaluation is ~1000 instructions; inlined seven times it made trace_dp54<MN> 106 KB
+// of code and instruction fetch its largest stall (ncu: no_instruction 1.5 per issue).  One
+// out-of-line copy keeps that kernel inside the instruction cache: measured +9 % on the DP5(4) kernel
+// and -4 % on the four-stage RK4 kernel, which therefore keeps the inlined form (OUTLINE_MN = false).
+template <class T>
+__device__ __noinline__ void rhs_manko_novikov_call(const MetricConst &mc, T pt, T pph, T r, T th, T pr, T pth,
+                                                    RhsT<T> &o) {
+  rhs_manko_novikov<T>(mc, pt, pph, r, th, pr, pth, o);
+}
+#endif
+
+template <int METRIC, bool OUTLINE_MN = false, class T>
 GP_HD void rhs_eval(const MetricConst &mc, T pt, T pph, T r, T th, T pr, T pth, RhsT<T> &o) {
   if (METRIC == METRIC_SCHW) rhs_schwarzschild<T>(mc, pt, pph, r, th, pr, pth, o);
   else if (METRIC == METRIC_KERR) rhs_kerr<T>(mc, pt, pph, r, th, pr, pth, o);
-  else rhs_manko_novikov<T>(mc, pt, pph, r, th, pr, pth, o);
+  else {
+#if defined(__CUDA_ARCH__)
+    if (OUTLINE_MN) rhs_manko_novikov_call<T>(mc, pt, pph, r, th, pr, pth, o);
+    else rhs_manko_novikov<T>(mc, pt, pph, r, th, pr, pth, o);
+#else
+    rhs_manko_novikov<T>(mc, pt, pph, r, th, pr, pth, o);
+#endif
+  }
 }
 
 // ---- covariant metric at a point (host: observer tetrad, row a3) ------------------------------

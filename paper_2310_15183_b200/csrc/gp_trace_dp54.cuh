@@ -114,7 +114,7 @@ trace_dp54(const __grid_constant__ TraceParams P) {
     if (mode != MODE_IDLE) {
       // ---- A: F at the pending state (stage 7 of the attempt in flight / k1 of a fresh ray) ----
       Rhs o7;
-      rhs_eval<METRIC>(mc, pt, pph, nr, nth, npr, npth, o7);
+      rhs_eval<METRIC, true>(mc, pt, pph, nr, nth, npr, npth, o7);
 
       // ---- B: decisions ----
       bool finished = false;
@@ -314,13 +314,13 @@ trace_dp54(const __grid_constant__ TraceParams P) {
         double ar, ath, apr, apth;   // K_j of the stage just evaluated
         double br, bth, bpr, bpth;   // K's streamed back from shared memory
         // stage 2
-        rhs_eval<METRIC>(mc, pt, pph, r + s * (dp.A21 * k1r), th + s * (dp.A21 * k1th),
+        rhs_eval<METRIC, true>(mc, pt, pph, r + s * (dp.A21 * k1r), th + s * (dp.A21 * k1th),
                          pr + s * (dp.A21 * k1pr), pth + s * (dp.A21 * k1pth), o);
         GP_HENON(0.0)
         ar = o.dr; ath = o.dth; apr = o.dpr; apth = o.dpth;                         // K2
         sts2(KS(0), ar, ath); sts2(KS(1), apr, apth);
         // stage 3
-        rhs_eval<METRIC>(mc, pt, pph, r + s * (dp.A31 * k1r + dp.A32 * ar),
+        rhs_eval<METRIC, true>(mc, pt, pph, r + s * (dp.A31 * k1r + dp.A32 * ar),
                          th + s * (dp.A31 * k1th + dp.A32 * ath),
                          pr + s * (dp.A31 * k1pr + dp.A32 * apr),
                          pth + s * (dp.A31 * k1pth + dp.A32 * apth), o);
@@ -335,7 +335,7 @@ trace_dp54(const __grid_constant__ TraceParams P) {
           double xpr = dp.A41 * k1pr + dp.A43 * apr, xpth = dp.A41 * k1pth + dp.A43 * apth;
           lds2(KS(0), br, bth); lds2(KS(1), bpr, bpth);                             // K2
           xr += dp.A42 * br; xth += dp.A42 * bth; xpr += dp.A42 * bpr; xpth += dp.A42 * bpth;
-          rhs_eval<METRIC>(mc, pt, pph, r + s * xr, th + s * xth, pr + s * xpr, pth + s * xpth, o);
+          rhs_eval<METRIC, true>(mc, pt, pph, r + s * xr, th + s * xth, pr + s * xpr, pth + s * xpth, o);
         }
         GP_HENON(dp.B4)
         ar = o.dr; ath = o.dth; apr = o.dpr; apth = o.dpth;                         // K4
@@ -350,7 +350,7 @@ trace_dp54(const __grid_constant__ TraceParams P) {
           xr += dp.A52 * br; xth += dp.A52 * bth; xpr += dp.A52 * bpr; xpth += dp.A52 * bpth;
           lds2(KS(2), br, bth); lds2(KS(3), bpr, bpth);                             // K3
           xr += dp.A53 * br; xth += dp.A53 * bth; xpr += dp.A53 * bpr; xpth += dp.A53 * bpth;
-          rhs_eval<METRIC>(mc, pt, pph, r + s * xr, th + s * xth, pr + s * xpr, pth + s * xpth, o);
+          rhs_eval<METRIC, true>(mc, pt, pph, r + s * xr, th + s * xth, pr + s * xpr, pth + s * xpth, o);
         }
         GP_HENON(dp.B5)
         ar = o.dr; ath = o.dth; apr = o.dpr; apth = o.dpth;                         // K5
@@ -367,7 +367,7 @@ trace_dp54(const __grid_constant__ TraceParams P) {
           xr += dp.A63 * br; xth += dp.A63 * bth; xpr += dp.A63 * bpr; xpth += dp.A63 * bpth;
           lds2(KS(4), br, bth); lds2(KS(5), bpr, bpth);                             // K4
           xr += dp.A64 * br; xth += dp.A64 * bth; xpr += dp.A64 * bpr; xpth += dp.A64 * bpth;
-          rhs_eval<METRIC>(mc, pt, pph, r + s * xr, th + s * xth, pr + s * xpr, pth + s * xpth, o);
+          rhs_eval<METRIC, true>(mc, pt, pph, r + s * xr, th + s * xth, pr + s * xpr, pth + s * xpth, o);
         }
         GP_HENON(dp.B6)
         ar = o.dr; ath = o.dth; apr = o.dpr; apth = o.dpth;                         // K6
