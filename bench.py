@@ -405,10 +405,13 @@ def run_shade(args):
         "config": {"workload": f"{args.workload} at {side}x{side}", "stage": "shade", "mode": "texture 4096x2048",
                    "l2": "512 MiB of records read per step (> 126 MB L2)"},
         "roofline": {"bound": "hbm", "kernel": "k_shade", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                     "frac": achieved / peak, "traffic": None, "peak_kind": kind,
+                     "frac": achieved / peak,
+                     # dram__bytes_read.sum + dram__bytes_write.sum of one launch (profiles/kernels_r01d.md)
+                     "traffic": 5.546e8, "peak_kind": kind,
                      "alg_bytes_per_launch": alg_bytes,
-                     "note": "the 128-byte record layout serves the tracer's stores; this reader needs 28 of "
-                             "them but touches two 32-byte sectors per record (68 B of DRAM traffic per pixel)"},
+                     "note": "the reader needs 28 bytes of each 128-byte record, in its first and fourth sectors; "
+                             "DRAM delivers both 64-byte halves, so traffic is the whole record: 5.76 TB/s, 88 % "
+                             "of the copy bandwidth (profiles/kernels_r01d.md)"},
         "clocks": clocks, "gpu_launches": args.steps,
         "e2e": {"value": n / dt, "unit": "pixels/s", "h2d_bytes_per_step": n * 128, "d2h_bytes_per_step": n * 4}}))
 
