@@ -407,11 +407,11 @@ def run_shade(args):
         "roofline": {"bound": "hbm", "kernel": "k_shade", "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak,
                      # dram__bytes_read.sum + dram__bytes_write.sum of one launch (profiles/kernels_r01d.md)
-                     "traffic": 5.546e8, "peak_kind": kind,
+                     "traffic": 2.861e8, "peak_kind": kind,
                      "alg_bytes_per_launch": alg_bytes,
-                     "note": "the reader needs 28 bytes of each 128-byte record, in its first and fourth sectors; "
-                             "DRAM delivers both 64-byte halves, so traffic is the whole record: 5.76 TB/s, 88 % "
-                             "of the copy bandwidth (profiles/kernels_r01d.md)"},
+                     "note": "the reader needs 28 bytes per record, all in its first 64-byte half (ld with an "
+                             "L2::64B hint: 268 MB read per launch, was 537 MB); the kernel is then bound by its six "
+                             "IEEE FP64 divisions per sub-ray, not by HBM (profiles/kernels_r01d.md)"},
         "clocks": clocks, "gpu_launches": args.steps,
         "e2e": {"value": n / dt, "unit": "pixels/s", "h2d_bytes_per_step": n * 128, "d2h_bytes_per_step": n * 4}}))
 

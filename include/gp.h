@@ -102,15 +102,21 @@ enum {
  * covector is the time-reversed one: p_t > 0 is the photon energy measured at infinity per
  * unit locally (ZAMO) measured energy, and L_z = -p_phi (reading R12).        */
 typedef struct gp_ray_record {
-  double t, r, theta, phi, p_r, p_theta; /* state on the exit surface (or last state)    */
-  double lambda;                         /* affine parameter at exit                      */
-  double p_t, p_phi;                     /* constants of the ray                          */
-  double h_max;         /* max |H| over every state a step was attempted from            */
-  double q_drift;       /* Kerr/Schwarzschild: max |Q-Q0| / max(1,|Q0|), Carter constant  */
-  double sin_theta_min; /* min |sin theta| over the same states                           */
-  double err_margin;    /* scheme 2: min |err-1| over attempted steps; else +inf          */
-  uint32_t status;      /* GP_RAY_*                                                       */
-  uint32_t n_accepted, n_rejected;
+  /* bytes 0-31 */
+  double t, r, theta, phi; /* state on the exit surface (or last state)                   */
+  /* bytes 32-63: with the sector above, everything image formation reads (gp_shade)     */
+  double lambda;           /* affine parameter at exit                                     */
+  uint32_t status;         /* GP_RAY_*                                                     */
+  uint32_t n_accepted;
+  double p_r, p_theta;     /* rest of the exit state                                       */
+  /* bytes 64-95 */
+  double p_t, p_phi;       /* constants of the ray                                         */
+  double h_max;            /* max |H| over every state a step was attempted from          */
+  double q_drift;          /* Kerr/Schwarzschild: max |Q-Q0| / max(1,|Q0|), Carter constant */
+  /* bytes 96-127 */
+  double sin_theta_min;    /* min |sin theta| over the same states                         */
+  double err_margin;       /* scheme 2: min |err-1| over attempted steps; else +inf        */
+  uint32_t n_rejected;
   uint32_t n_equator_crossings; /* sign changes of theta - pi/2 over accepted steps       */
   uint32_t n_disk_recorded;     /* crossings with disk_r_in <= r <= disk_r_out, <= 3      */
   uint32_t n_rhs;               /* evaluations of Hamilton's equations spent on this ray  */

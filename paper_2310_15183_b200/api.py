@@ -59,10 +59,10 @@ class gp_out_buffers(C.Structure):
 
 # numpy views of the record layouts of include/gp.h
 RAY_DTYPE = np.dtype([
-    ("t", "<f8"), ("r", "<f8"), ("theta", "<f8"), ("phi", "<f8"), ("p_r", "<f8"), ("p_theta", "<f8"),
-    ("lambda", "<f8"), ("p_t", "<f8"), ("p_phi", "<f8"),
-    ("h_max", "<f8"), ("q_drift", "<f8"), ("sin_theta_min", "<f8"), ("err_margin", "<f8"),
-    ("status", "<u4"), ("n_accepted", "<u4"), ("n_rejected", "<u4"),
+    ("t", "<f8"), ("r", "<f8"), ("theta", "<f8"), ("phi", "<f8"),
+    ("lambda", "<f8"), ("status", "<u4"), ("n_accepted", "<u4"), ("p_r", "<f8"), ("p_theta", "<f8"),
+    ("p_t", "<f8"), ("p_phi", "<f8"), ("h_max", "<f8"), ("q_drift", "<f8"),
+    ("sin_theta_min", "<f8"), ("err_margin", "<f8"), ("n_rejected", "<u4"),
     ("n_equator_crossings", "<u4"), ("n_disk_recorded", "<u4"), ("n_rhs", "<u4")])
 DISK_DTYPE = np.dtype([("r_cross", "<f8", (3,)), ("g", "<f8", (3,))])
 assert RAY_DTYPE.itemsize == 128 and DISK_DTYPE.itemsize == 48

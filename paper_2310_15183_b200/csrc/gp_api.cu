@@ -3,6 +3,7 @@
 // There is no CPU path: every step of the method runs in the kernels of gp_trace*.cuh.
 #include <cuda_runtime.h>
 #include <math.h>
+#include <stddef.h>
 #include <stdio.h>
 #include <string.h>
 
@@ -11,6 +12,9 @@
 #include "gp_shade.cuh"
 
 static_assert(sizeof(gp_ray_record) == 128, "gp_ray_record must be 128 bytes");
+static_assert(offsetof(gp_ray_record, status) == 40 && offsetof(gp_ray_record, p_t) == 64 &&
+                  offsetof(gp_ray_record, n_rhs) == 124,
+              "gp_ray_record layout (gp_trace.cuh store_record and gp_shade.cuh read it by offset)");
 static_assert(sizeof(gp_disk_record) == 48, "gp_disk_record must be 48 bytes");
 
 namespace {

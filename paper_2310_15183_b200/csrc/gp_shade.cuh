@@ -2,8 +2,8 @@
 // kernel; formulas in include/gp.h "image formation").
 //
 // HBM-bound: one thread per output pixel reads the S*S records of its
-// sub-rays — only the 32-byte sectors it needs: (t, r, theta, phi) and the one holding status, plus
-// the first 8-byte pair of the disk record — and writes one 4-byte pixel.  Every FP64 operation
+// sub-rays — only the first 64-byte half of each: (t, r, theta, phi) and the sector holding status,
+// plus the first sector of the disk record — and writes one 4-byte pixel.  Every FP64 operation
 // is individually rounded (__dadd_rn / __dmul_rn / __ddiv_rn never contract into FMAs), so the
 // bytes are identical to any IEEE-754 evaluation of the same formulas in the same order.
 #ifndef GP_SHADE_CUH_
@@ -172,16 +172,24 @@ __global__ void k_shade(const __grid_constant__ ShadeParams P) {
   for (long long sj = 0; sj < P.S; ++sj)
     for (long long si = 0; si < P.S; ++si) {
       const long long ray = (j * P.S + sj) * P.W * P.S + (i * P.S + si);
-      const double t = __ldg(reinterpret_cast<const double *>(P.rays + ray));               // t
-      const double2 a = __ldg(reinterpret_cast<const double2 *>(P.rays + ray) + 1);        // theta, phi
-      const uint4 b = __ldg(reinterpret_cast<const uint4 *>(P.rays + ray) + 6);          // bytes 96..111: err_margin, status, n_accepted
+      // the first 64-byte half of the record: (t, r | theta, phi | lambda, status..) as three 128-bit loads
+      // with a 64-byte L2 prefetch-size hint, so that the second half is not pulled in with it
+      const char *rec = reinterpret_cast<const char *>(P.rays + ray);
+      double t, r_unused, th_raw, ph_raw;
+      unsigned b0, b1, status, b3;
+      asm volatile("ld.global.nc.L2::64B.v2.f64 {%0, %1}, [%2];" : "=d"(t), "=d"(r_unused) : "l"(rec));
+      asm volatile("ld.global.nc.L2::64B.v2.f64 {%0, %1}, [%2];" : "=d"(th_raw), "=d"(ph_raw) : "l"(rec + 16));
+      asm volatile("ld.global.nc.L2::64B.v4.u32 {%0, %1, %2, %3}, [%4];"
+                   : "=r"(b0), "=r"(b1), "=r"(status), "=r"(b3)
+                   : "l"(rec + 32));
+      (void)r_unused; (void)b0; (void)b1; (void)b3;
       double dr = qnan, dg = qnan;
       if (P.disk_overlay) {
         dr = __ldg(&P.disk[ray].r_cross[0]);
         dg = __ldg(&P.disk[ray].g[0]);
       }
       double rgb[3];
-      shade_ray(P, b255, b.z, a.x, a.y, t, dr, dg, rgb);
+      shade_ray(P, b255, status, th_raw, ph_raw, t, dr, dg, rgb);
       for (int k = 0; k < 3; ++k) sum[k] = sh::add(sum[k], rgb[k]);
     }
   const double inv = sh::div(1.0, (double)(P.S * P.S));

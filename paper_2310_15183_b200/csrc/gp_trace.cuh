@@ -143,13 +143,13 @@ __device__ __forceinline__ void store_record(gp_ray_record *rec, double t, doubl
                                              unsigned n_rej, unsigned n_cross, unsigned n_rec,
                                              unsigned n_rhs) {
   double *p = reinterpret_cast<double *>(rec);
-  store4(p, t, r, th, ph);
-  store4(p + 4, pr, pth, lam, pt);
-  store4(p + 8, pph, mo.h_max, mo.q_drift, mo.sin_min);
   double w0 = __hiloint2double((int)n_acc, (int)status);      // little endian: status, n_accepted
   double w1 = __hiloint2double((int)n_cross, (int)n_rej);     // n_rejected, n_equator_crossings
   double w2 = __hiloint2double((int)n_rhs, (int)n_rec);       // n_disk_recorded, n_rhs
-  store4(p + 12, mo.err_margin, w0, w1, w2);
+  store4(p, t, r, th, ph);
+  store4(p + 4, lam, w0, pr, pth);
+  store4(p + 8, pt, pph, mo.h_max, mo.q_drift);
+  store4(p + 12, mo.sin_min, mo.err_margin, w1, w2);
 }
 
 #endif  // __CUDACC__

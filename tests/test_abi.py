@@ -52,7 +52,8 @@ def test_record_layouts():
     assert gp.gp_counters_size() == 64
     assert gp.gp_version() == 100
     f = api.RAY_DTYPE.fields
-    assert f["lambda"][1] == 48 and f["err_margin"][1] == 96 and f["status"][1] == 104 and f["n_rhs"][1] == 124
+    assert f["lambda"][1] == 32 and f["status"][1] == 40 and f["p_r"][1] == 48 and f["p_t"][1] == 64
+    assert f["sin_theta_min"][1] == 96 and f["err_margin"][1] == 104 and f["n_rhs"][1] == 124
     assert C.sizeof(api.gp_camera) == 7 * 8 + 4 * 4 + 8 + 3 * 8 + 3 * 8
     assert C.sizeof(api.gp_integrator_cfg) == 8 + 5 * 8 + 8 + 8 + 2 * 8 + 2 * 8 + 8
 

@@ -444,7 +444,7 @@ def test_largest_sweep_8192_squared_sampled(gp, O):
     cnt = counters.cpu().numpy().view("<u8")
     assert cnt[1] == n and cnt[0] >= n
     rec = rays.view(n, 128)
-    status = rec[:, 104:108].contiguous().view(torch.int32).view(n)          # u32 status at byte 104
+    status = rec[:, 40:44].contiguous().view(torch.int32).view(n)            # u32 status at byte 40
     census = torch.bincount(status.to(torch.int64), minlength=5).cpu().numpy()
     assert census[2:].sum() == 0 and census[0] > 0.9 * n and census[1] > 0.01 * n
     # sampled parity: every 262 147th ray from ray 5, including slots far beyond the 2^32-byte mark
