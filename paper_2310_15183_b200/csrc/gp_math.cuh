@@ -104,8 +104,9 @@ __device__ __forceinline__ void sincos_fast(double x, double *sn, double *cs) {
   // quadrant: q mod 4 = 0: (s, c); 1: (c, -s); 2: (-s, -c); 3: (-c, s)
   double a = (q & 1) ? cr : sr;
   double b = (q & 1) ? sr : cr;
-  *sn = (q & 2) ? -a : a;
-  *cs = ((q + 1) & 2) ? -b : b;
+  // sign flips on the high word (one LOP3 each) instead of FP64 negate + select
+  *sn = __hiloint2double(__double2hiint(a) ^ ((q & 2) << 30), __double2loint(a));
+  *cs = __hiloint2double(__double2hiint(b) ^ (((q + 1) & 2) << 30), __double2loint(b));
 }
 
 // x^(-1/5) for x in [1e-5, 1e4] (the controller clamps outside, R10 item 3): FP32 seed from the
