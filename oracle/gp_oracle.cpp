@@ -337,7 +337,64 @@ void alpha_beta(const orc_camera *cam, int64_t ray, double *alpha, double *beta)
 // Replaces P:L338-348 (eq 54-55): same content (null vector, fixed normalisation, lowered
 // index), built from an orthonormal frame instead of a Euclidean screen.
 // ------------------------------------------------------------------------------------------
+// The paper's own camera, P:L314-348 (section 3.3.1, Fig 2-3, eq 51-55): a flat screen in Euclidean
+// xyz (z = the Boyer-Lindquist axis), offset from the origin, start point and direction per pixel,
+// converted to Boyer-Lindquist by inverting eq 51-53 and differentiating the inverse, made null by
+// solving eq 54 for dt/dlambda, scaled so that dt/dlambda = -1, lowered with eq 55.
+// Readings: the screen is centred at r_obs c_hat with c_hat the unit vector at (theta_obs, phi_obs)
+// (the paper: viewing along -y, then rotating about the x axis); its axes are e_phi (alpha) and
+// e_up = -e_theta (beta), the same orientation as the pinhole camera; the direction is
+// -c_hat + (2f/d) (alpha e_phi + beta e_up) ("add the x and z position to the velocities,
+// multiplying by a factor 2f/d").  eq 51-53 use the spin a of the metric (0 for Schwarzschild).
+int initial_state_screen(const orc_metric *m, const orc_camera *cam, double alpha, double beta, double st[8]) {
+  const double a = (m->id == 0) ? 0.0 : m->a;
+  const double so = std::sin(cam->theta_obs), co = std::cos(cam->theta_obs);
+  const double sp = std::sin(cam->phi_obs), cp = std::cos(cam->phi_obs);
+  const double chat[3] = {so * cp, so * sp, co};
+  const double eph[3] = {-sp, cp, 0.0};
+  const double eup[3] = {-co * cp, -co * sp, so};
+  const double k2 = cam->focal_2f_over_d;
+  double X[3], V[3];
+  for (int i = 0; i < 3; ++i) {
+    X[i] = cam->r_obs * chat[i] + alpha * eph[i] + beta * eup[i];
+    V[i] = -chat[i] + k2 * (alpha * eph[i] + beta * eup[i]);
+  }
+  // inverse of eq 51-53: r^2 is the positive root of r^4 - w r^2 - a^2 z^2 = 0, w = |X|^2 - a^2
+  const double w = X[0] * X[0] + X[1] * X[1] + X[2] * X[2] - a * a;
+  const double r = std::sqrt(0.5 * (w + std::sqrt(w * w + 4.0 * a * a * X[2] * X[2])));
+  const double th = std::acos(X[2] / r);
+  const double ph = std::atan2(X[1], X[0]);
+  const double sth = std::sin(th), cth = std::cos(th), sph = std::sin(ph), cph = std::cos(ph);
+  const double R = std::sqrt(r * r + a * a), Sig = r * r + a * a * cth * cth;
+  // derivative of the inverse map applied to V
+  const double u = V[0] * cph + V[1] * sph;
+  double dph = (-V[0] * sph + V[1] * cph) / (R * sth);
+  double dr = R * (r * sth * u + R * cth * V[2]) / Sig;
+  double dth = (R * cth * u - r * sth * V[2]) / Sig;
+  double g[5];
+  if (metric_cov<double>(m, r, th, g)) return -1;
+  const double gtt = g[0], gtp = g[1], gpp = g[2], grr = g[3], gthth = g[4];
+  // eq 54 as a quadratic in dt: g_tt dt^2 + 2 g_tphi dphi dt + S = 0; the root with dt < 0
+  const double S = grr * dr * dr + gthth * dth * dth + gpp * dph * dph;
+  const double B = gtp * dph;
+  const double dt = (-B + std::sqrt(B * B - gtt * S)) / gtt;
+  const double sc = -1.0 / dt;  // scale so that dt/dlambda = -1
+  dr *= sc;
+  dth *= sc;
+  dph *= sc;
+  st[0] = 0.0;
+  st[1] = r;
+  st[2] = th;
+  st[3] = ph;
+  st[4] = -gtt + gtp * dph;   // eq 55 with dt = -1
+  st[5] = grr * dr;
+  st[6] = gthth * dth;
+  st[7] = -gtp + gpp * dph;
+  return 0;
+}
+
 int initial_state(const orc_metric *m, const orc_camera *cam, double alpha, double beta, double st[8]) {
+  if (cam->projection == 1) return initial_state_screen(m, cam, alpha, beta, st);
   double g[5];
   if (metric_cov<double>(m, cam->r_obs, cam->theta_obs, g)) return -1;
   double gtt = g[0], gtp = g[1], gpp = g[2], grr = g[3], gthth = g[4];
@@ -559,7 +616,7 @@ void trace_ray(const orc_metric *m, const orc_camera *cam, const orc_cfg *cfg, d
   int64_t status = -1;
   auto f = [&](const double *yy, double *dy) { rhs(S, yy, dy); };
 
-  double h = (scheme == 2) ? cfg->h_cap_rel * cam->r_obs : 0.0;  // R10 item 4
+  double h = (scheme == 2) ? cfg->h_cap_rel * st[1] : 0.0;  // R10 item 4 (st[1] = r_obs for the pinhole)
   double k[7][7];
   if (scheme == 2) f(y, k[0]);
   if (path) path->push(lam, y, h);

@@ -36,6 +36,11 @@ typedef struct orc_camera {
   int64_t width, height, supersample;
   uint64_t jitter_seed;
   double jitter_amp_px, shift_x_px, shift_y_px;
+  /* 0: pinhole in the ZAMO tetrad (BASELINE.json); 1: the paper's Euclidean screen:
+   * start points alpha e_phi + beta e_up on a flat screen centred at r_obs c_hat, directions
+   * -c_hat + focal_2f_over_d (alpha e_phi + beta e_up) (0 = parallel rays, "focal distance infinity") */
+  int64_t projection;
+  double focal_2f_over_d;
 } orc_camera;
 
 typedef struct orc_cfg {

@@ -22,7 +22,8 @@ class OrcCamera(C.Structure):
                 ("alpha_min", _f64), ("alpha_max", _f64), ("beta_min", _f64), ("beta_max", _f64),
                 ("width", _i64), ("height", _i64), ("supersample", _i64),
                 ("jitter_seed", C.c_uint64),
-                ("jitter_amp_px", _f64), ("shift_x_px", _f64), ("shift_y_px", _f64)]
+                ("jitter_amp_px", _f64), ("shift_x_px", _f64), ("shift_y_px", _f64),
+                ("projection", _i64), ("focal_2f_over_d", _f64)]
 
 
 class OrcCfg(C.Structure):
@@ -99,7 +100,8 @@ def _camera(d):
     return OrcCamera(d["r_obs"], d["theta_obs"], d.get("phi_obs", 0.0),
                      d["alpha_min"], d["alpha_max"], d["beta_min"], d["beta_max"],
                      d["width"], d["height"], d.get("supersample", 1), d.get("jitter_seed", 0),
-                     d.get("jitter_amp_px", 0.0), d.get("shift_x_px", 0.0), d.get("shift_y_px", 0.0))
+                     d.get("jitter_amp_px", 0.0), d.get("shift_x_px", 0.0), d.get("shift_y_px", 0.0),
+                     d.get("projection", 0), d.get("focal_2f_over_d", 0.0))
 
 
 def _cfg(d):
