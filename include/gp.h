@@ -25,7 +25,7 @@
 extern "C" {
 #endif
 
-#define GP_VERSION 100 /* major*10000 + minor*100 + patch */
+#define GP_VERSION 101 /* major*10000 + minor*100 + patch */
 
 /* ---- spacetimes (section 2.2) ------------------------------------------- */
 enum {
@@ -57,11 +57,21 @@ typedef struct gp_camera {
   double alpha_min, alpha_max, beta_min, beta_max; /* image-plane window, units of length */
   int32_t width, height;                           /* pixels, > 0                         */
   int32_t supersample;                             /* S >= 1: S x S sub-rays per pixel    */
-  int32_t projection;                              /* 0 = pinhole in the ZAMO tetrad      */
+  int32_t projection;                              /* 0 = pinhole in the ZAMO tetrad; 1 = the paper's
+                                                      Euclidean screen (below)             */
   uint64_t jitter_seed;
   double jitter_amp_px;          /* 0 = sub-pixel centres; 0.5 = uniform in +-0.5 px      */
   double shift_x_px, shift_y_px; /* rigid shift of the whole grid (chaos companion run)   */
   int64_t ray_begin, ray_count, ray_stride; /* ray_stride >= 1; all rays < Wt*Ht          */
+  /* projection = 1, PAPER.md L314-348 (section 3.3.1, Fig 2-3, eq 51-55): a flat screen in the
+   * Euclidean xyz of eq 51-53, centred at r_obs c_hat (c_hat = unit vector at theta_obs, phi_obs),
+   * spanned by e_phi (alpha) and e_up = -e_theta (beta).  Pixel (alpha, beta) starts AT
+   * r_obs c_hat + alpha e_phi + beta e_up with direction -c_hat + focal_2f_over_d (alpha e_phi +
+   * beta e_up) (0 = parallel rays, "focal distance infinity"); position and direction go to
+   * Boyer-Lindquist by inverting eq 51-53 (a = the metric's spin), dt/dlambda solves eq 54 and the
+   * ray is scaled to dt/dlambda = -1 before eq 55 lowers the index.  Needs r_escape beyond every
+   * start point.  Ignored when projection = 0.                                                  */
+  double focal_2f_over_d;
 } gp_camera;
 
 /* ---- integrator ---------------------------------------------------------------------

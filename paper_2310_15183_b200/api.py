@@ -31,7 +31,8 @@ class gp_camera(C.Structure):
                 ("width", _i32), ("height", _i32), ("supersample", _i32), ("projection", _i32),
                 ("jitter_seed", _u64), ("jitter_amp_px", _f64),
                 ("shift_x_px", _f64), ("shift_y_px", _f64),
-                ("ray_begin", _i64), ("ray_count", _i64), ("ray_stride", _i64)]
+                ("ray_begin", _i64), ("ray_count", _i64), ("ray_stride", _i64),
+                ("focal_2f_over_d", _f64)]
 
 
 class gp_integrator_cfg(C.Structure):
@@ -129,7 +130,7 @@ def camera_struct(c, ray_begin=0, ray_count=None, ray_stride=1):
                      int(c["width"]), int(c["height"]), S, int(c.get("projection", 0)),
                      int(c.get("jitter_seed", 0)), c.get("jitter_amp_px", 0.0),
                      c.get("shift_x_px", 0.0), c.get("shift_y_px", 0.0),
-                     int(ray_begin), int(ray_count), int(ray_stride))
+                     int(ray_begin), int(ray_count), int(ray_stride), c.get("focal_2f_over_d", 0.0))
 
 
 def cfg_struct(g):

@@ -80,7 +80,8 @@ double isco_prograde(int metric_id, const MetricConst &mc) {
 int make_camera(int metric_id, const MetricConst &mc, const gp_camera *c, double eps_capture, CameraConst *cc) {
   if (!c) return GP_E_NULL;
   if (c->width <= 0 || c->height <= 0 || c->supersample <= 0) return GP_E_BAD_PARAM;
-  if (c->projection != 0) return GP_E_UNSUPPORTED;
+  if (c->projection != 0 && c->projection != 1) return GP_E_UNSUPPORTED;
+  if (c->projection == 1 && !(c->focal_2f_over_d >= 0.0 && isfinite(c->focal_2f_over_d))) return GP_E_BAD_PARAM;
   if (!(c->alpha_max > c->alpha_min) || !(c->beta_max > c->beta_min)) return GP_E_BAD_PARAM;
   if (!isfinite(c->alpha_min) || !isfinite(c->alpha_max) || !isfinite(c->beta_min) || !isfinite(c->beta_max))
     return GP_E_BAD_PARAM;
@@ -115,6 +116,16 @@ int make_camera(int metric_id, const MetricConst &mc, const gp_camera *c, double
   cc->r_obs = c->r_obs;
   cc->theta_obs = c->theta_obs;
   cc->phi_obs = c->phi_obs;
+  cc->projection = c->projection;
+  cc->metric_id = metric_id;
+  cc->k2 = c->focal_2f_over_d;
+  cc->a_cam = (metric_id == GP_SCHWARZSCHILD) ? 0.0 : mc.a;
+  {
+    const double so = sin(c->theta_obs), co = cos(c->theta_obs), sp = sin(c->phi_obs), cp = cos(c->phi_obs);
+    cc->chat[0] = so * cp; cc->chat[1] = so * sp; cc->chat[2] = co;
+    cc->eph[0] = -sp; cc->eph[1] = cp; cc->eph[2] = 0.0;
+    cc->eup[0] = -co * cp; cc->eup[1] = -co * sp; cc->eup[2] = so;
+  }
   // observer's ZAMO tetrad from the covariant metric of the selected spacetime (reading R12)
   double g[5];
   metric_cov(metric_id, mc, c->r_obs, c->theta_obs, g);
@@ -145,6 +156,15 @@ int make_params(int metric_id, const gp_metric_params *m, const gp_camera *cam, 
   if (rc) return rc;
   if (cfg->max_steps < 0 || cfg->max_steps > 500000000LL) return GP_E_BAD_PARAM;
   if (!(cfg->r_escape > cam->r_obs) || !isfinite(cfg->r_escape)) return GP_E_BAD_PARAM;
+  if (cam->projection == 1) {
+    // every start point of the flat screen must lie inside the escape sphere: r <= |X| and the
+    // farthest point is a window corner
+    double am = fmax(fabs(cam->alpha_min), fabs(cam->alpha_max)), bm = fmax(fabs(cam->beta_min), fabs(cam->beta_max));
+    double pad = (cam->jitter_amp_px + fabs(cam->shift_x_px) + fabs(cam->shift_y_px) + 1.0);
+    am += pad * (cam->alpha_max - cam->alpha_min) / cam->width;
+    bm += pad * (cam->beta_max - cam->beta_min) / cam->height;
+    if (!(cfg->r_escape > sqrt(cam->r_obs * cam->r_obs + am * am + bm * bm))) return GP_E_BAD_PARAM;
+  }
   if (cfg->scheme == 0 && !(cfg->h > 0.0 && isfinite(cfg->h))) return GP_E_BAD_PARAM;
   if (cfg->scheme == 1 && !(cfg->h_rel > 0.0 && isfinite(cfg->h_rel))) return GP_E_BAD_PARAM;
   if (cfg->scheme == 2) {
@@ -231,14 +251,15 @@ int launch_trace(int metric_id, const TraceParams &P, cudaStream_t stream) {
 }
 
 // ---- step-level kernels (parity of rows a2-a5 in isolation) -------------------------------------
-__global__ void k_init_conditions(const __grid_constant__ CameraConst cc, double *states8, double *ab2) {
+__global__ void k_init_conditions(const __grid_constant__ CameraConst cc, const __grid_constant__ MetricConst mc,
+                                  double *states8, double *ab2) {
   long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= cc.ray_count) return;
-  double alpha, beta, pt, pr, pth, pph;
+  double alpha, beta, r, th, ph, pt, pr, pth, pph;
   alpha_beta(cc, cc.ray_begin + k * cc.ray_stride, alpha, beta);
-  initial_momentum(cc, alpha, beta, pt, pr, pth, pph);
+  ray_birth(cc, mc, cc.ray_begin + k * cc.ray_stride, r, th, ph, pt, pr, pth, pph);
   double *s = states8 + 8 * k;
-  s[0] = 0.0; s[1] = cc.r_obs; s[2] = cc.theta_obs; s[3] = cc.phi_obs;
+  s[0] = 0.0; s[1] = r; s[2] = th; s[3] = ph;
   s[4] = pt; s[5] = pr; s[6] = pth; s[7] = pph;
   if (ab2) {
     ab2[2 * k] = alpha;
@@ -392,7 +413,7 @@ int gp_init_conditions(int metric_id, const gp_metric_params *metric, const gp_c
   if (states_bytes < n * 64) return GP_E_SIZE;
   if (alpha_beta2 && ab_bytes < n * 16) return GP_E_SIZE;
   const unsigned grid = (unsigned)((n + 255) / 256);
-  k_init_conditions<<<grid, 256, 0, (cudaStream_t)cuda_stream>>>(cc, (double *)states8, (double *)alpha_beta2);
+  k_init_conditions<<<grid, 256, 0, (cudaStream_t)cuda_stream>>>(cc, mc, (double *)states8, (double *)alpha_beta2);
   GP_CUDA(cudaGetLastError());
   return GP_OK;
 }

@@ -27,6 +27,12 @@ struct CameraConst {
   double sq_grr, sq_gthth, sq_gpp; // sqrt(g_rr), sqrt(g_thth), sqrt(g_phiphi)
   double inv_zeta;                 // sqrt(-(g_tt + Omega g_tphi))
   double Omega;                    // -g_tphi/g_phiphi
+  // projection = 1 (the paper's Euclidean screen): frame and focal factor
+  int projection;
+  int metric_id;
+  double k2;                       // 2f/d
+  double a_cam;                    // spin used by eq 51-53 (0 for Schwarzschild)
+  double chat[3], eph[3], eup[3];  // screen normal (towards the observer) and its two axes
 };
 
 #if defined(__CUDACC__)

@@ -37,6 +37,65 @@ struct TraceParams {
 
 enum { MODE_IDLE = 0, MODE_FRESH = 1, MODE_NORMAL = 2, MODE_LAND_R = 3, MODE_LAND_TH = 4 };
 
+#if defined(__CUDACC__)
+// Rows a2 + a3 for one ray: image-plane point, then the initial state of the selected camera.
+// projection 0: the pinhole of gp_camera.cuh (every ray starts at the observer).
+// projection 1: the paper's Euclidean screen: start point and direction on a
+// flat screen in the xyz of eq 51-53, to Boyer-Lindquist by inverting eq 51-53 and differentiating
+// the inverse, dt/dlambda from eq 54 (the root < 0), scaled to dt/dlambda = -1, lowered by eq 55.
+// Kept out of line: it runs once per ray and must not weigh on the register allocation of the step loop.
+__device__ __noinline__ void ray_birth_screen(const CameraConst &cc, const MetricConst &mc, double alpha,
+                                              double beta, double *out7) {
+  const double a = cc.a_cam;
+  double X[3], V[3];
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    double off = alpha * cc.eph[i] + beta * cc.eup[i];
+    X[i] = cc.r_obs * cc.chat[i] + off;
+    V[i] = cc.k2 * off - cc.chat[i];
+  }
+  const double w = X[0] * X[0] + X[1] * X[1] + X[2] * X[2] - a * a;
+  const double r = sqrt(0.5 * (w + sqrt(w * w + 4.0 * a * a * X[2] * X[2])));
+  const double th = acos(X[2] / r);
+  const double ph = atan2(X[1], X[0]);
+  double sth, cth, sph, cph;
+  sincos(th, &sth, &cth);
+  sincos(ph, &sph, &cph);
+  const double R = sqrt(r * r + a * a), Sig = r * r + a * a * cth * cth;
+  const double u = V[0] * cph + V[1] * sph;
+  double dph = (V[1] * cph - V[0] * sph) / (R * sth);
+  double dr = R * (r * sth * u + R * cth * V[2]) / Sig;
+  double dth = (R * cth * u - r * sth * V[2]) / Sig;
+  double g[5];
+  metric_cov(cc.metric_id, mc, r, th, g);
+  const double S = g[3] * dr * dr + g[4] * dth * dth + g[2] * dph * dph;
+  const double B = g[1] * dph;
+  const double dt = (sqrt(B * B - g[0] * S) - B) / g[0];
+  const double sc = -1.0 / dt;
+  dr *= sc; dth *= sc; dph *= sc;
+  out7[0] = r; out7[1] = th; out7[2] = ph;
+  out7[3] = g[1] * dph - g[0];
+  out7[4] = g[3] * dr;
+  out7[5] = g[4] * dth;
+  out7[6] = g[2] * dph - g[1];
+}
+
+__device__ __forceinline__ void ray_birth(const CameraConst &cc, const MetricConst &mc, long long ray, double &r,
+                                          double &th, double &ph, double &pt, double &pr, double &pth,
+                                          double &pph) {
+  double alpha, beta;
+  alpha_beta(cc, ray, alpha, beta);
+  if (cc.projection == 0) {
+    initial_momentum(cc, alpha, beta, pt, pr, pth, pph);
+    r = cc.r_obs; th = cc.theta_obs; ph = cc.phi_obs;
+  } else {
+    double o[7];
+    ray_birth_screen(cc, mc, alpha, beta, o);
+    r = o[0]; th = o[1]; ph = o[2]; pt = o[3]; pr = o[4]; pth = o[5]; pph = o[6];
+  }
+}
+#endif
+
 constexpr int kBlock = 128;
 constexpr unsigned kFull = 0xffffffffu;
 constexpr double kHalfPi = 1.57079632679489661923;

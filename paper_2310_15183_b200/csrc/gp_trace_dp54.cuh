@@ -97,10 +97,8 @@ trace_dp54(const __grid_constant__ TraceParams P) {
           exhausted = true;
         } else {
           // a2 + a3
-          double alpha, beta;
-          alpha_beta(P.cc, P.cc.ray_begin + slot * P.cc.ray_stride, alpha, beta);
-          initial_momentum(P.cc, alpha, beta, pt, npr, npth, pph);
-          nt = 0.0; nr = P.cc.r_obs; nth = P.cc.theta_obs; nph = P.cc.phi_obs; nlam = 0.0;
+          ray_birth(P.cc, mc, P.cc.ray_begin + slot * P.cc.ray_stride, nr, nth, nph, pt, npr, npth, pph);
+          nt = 0.0; nlam = 0.0;
           mode = MODE_FRESH;
           n_acc = n_rej = n_cross = n_rec = n_land = 0;
           const double inf = __longlong_as_double(0x7ff0000000000000LL);
@@ -126,7 +124,7 @@ trace_dp54(const __grid_constant__ TraceParams P) {
         sts1(CS(C_T), nt); sts1(CS(C_PH), nph); sts1(CS(C_LAM), nlam);
         k1r = o7.dr; k1th = o7.dth; k1pr = o7.dpr; k1pth = o7.dpth;
         sts1(CS(C_K1T), o7.dt); sts1(CS(C_K1PH), o7.dph);
-        h = P.h_cap_rel * P.cc.r_obs;       // R10 item 4
+        h = P.h_cap_rel * nr;               // R10 item 4: h0 = cap x the start radius (r_obs for the pinhole)
         monH = fabs(0.5 * o7.H2); monQ = carter_q<METRIC>(mc, pt, pph, npth, o7); monS = fabs(o7.s);
         mode = MODE_NORMAL;
         moved = true;

@@ -47,11 +47,10 @@ __global__ void __launch_bounds__(kBlock) trace_rk4(const __grid_constant__ Trac
         if (slot < 0) {
           exhausted = true;
         } else {
-          double alpha, beta, dpt, dpr, dpth, dpph;
-          alpha_beta(P.cc, P.cc.ray_begin + slot * P.cc.ray_stride, alpha, beta);
-          initial_momentum(P.cc, alpha, beta, dpt, dpr, dpth, dpph);
+          double dr0, dth0, dph0, dpt, dpr, dpth, dpph;
+          ray_birth(P.cc, mc, P.cc.ray_begin + slot * P.cc.ray_stride, dr0, dth0, dph0, dpt, dpr, dpth, dpph);
           pt = (T)dpt; pr = (T)dpr; pth = (T)dpth; pph = (T)dpph;
-          t = T(0); r = (T)P.cc.r_obs; th = (T)P.cc.theta_obs; ph = (T)P.cc.phi_obs; lam = T(0);
+          t = T(0); r = (T)dr0; th = (T)dth0; ph = (T)dph0; lam = T(0);
           mode = MODE_NORMAL;
           n_acc = n_cross = n_rec = n_land = 0;
           mo.h_max = T(0); mo.q_drift = T(0); mo.Q0 = T(0);

@@ -457,3 +457,45 @@ def test_largest_sweep_8192_squared_sampled(gp, O):
     check_parity(w, sample, orc, probe, "8192^2 sample", max_flagged_fraction=0.05)
     del rays, rec
     torch.cuda.empty_cache()
+
+
+# ---- the paper's own camera (projection = 1; eq 51-55) ------------------------
+def _screen(w, k2=0.0):
+    w = copy.deepcopy(w)
+    w["camera"].update(projection=1, focal_2f_over_d=k2)
+    return w
+
+
+@pytest.mark.parametrize("name,k2", [("C1", 0.0), ("C2", 0.0), ("C2", 0.01), ("C4", 0.0)])
+def test_screen_camera_initial_conditions(gp, O, name, k2):
+    import torch
+    w = _screen(W.workload(name), k2)
+    b, c, s = W.ray_selection(w, 3, 3000, 977)
+    cam = gp.api.camera_struct(w["camera"], b, c, s)
+    st = torch.empty((c, 8), dtype=torch.float64, device="cuda")
+    ab = torch.empty((c, 2), dtype=torch.float64, device="cuda")
+    gp.gp_init_conditions(w["metric"]["id"], gp.api.metric_struct(w["metric"]), cam, st, ab)
+    torch.cuda.synchronize()
+    ab, st = ab.cpu().numpy(), st.cpu().numpy()
+    ab_o = O.alpha_beta(w["camera"], b + s * np.arange(c))
+    assert np.array_equal(ab.view(np.uint64), ab_o.view(np.uint64))
+    for i in range(0, c, 29):
+        so = O.initial_state(w["metric"], w["camera"], ab_o[i, 0], ab_o[i, 1])
+        # positions to 1e-13; the momenta pass through acos/atan2, the Jacobian and the quadratic of eq 54:
+        # 1e-11 of the largest component (p_theta, p_phi ~ r times the O(1) direction cosines)
+        assert np.allclose(st[i, :4], so[:4], rtol=1e-13, atol=1e-13), (i, st[i], so)
+        assert np.abs(st[i, 4:] - so[4:]).max() <= 1e-11 * np.abs(so[4:]).max(), (i, st[i], so)
+
+
+@pytest.mark.parametrize("name,k2,sel", [("C2", 0.0, (5, None, 61)), ("C2", 0.008, (9, None, 127)),
+                                         ("C5a", 0.0, (1, None, 16411))])
+def test_screen_camera_trace_parity(gp, O, name, k2, sel):
+    w = _screen(W.workload(name), k2)
+    if name == "C5a":
+        w["cfg"]["max_steps"] = 20000
+    rays, _, _, orc, probe = run_both(gp, O, w, *sel)
+    res, smooth = check_parity(w, rays, orc, probe, f"screen {name} k2={k2}", max_flagged_fraction=0.03)
+    # (with 2f/d = 0.008 the rays fan out by +-0.1 rad and only a handful still meet the hole)
+    assert (orc["status"] == 1).sum() > (20 if k2 == 0.0 else 3) and (orc["status"] == 0).sum() > 500
+    # every ray starts on the flat screen, not at the observer: the start radius varies over the image
+    assert res["status_mismatch"] == 0
