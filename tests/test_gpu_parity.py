@@ -499,3 +499,45 @@ def test_screen_camera_trace_parity(gp, O, name, k2, sel):
     assert (orc["status"] == 1).sum() > (20 if k2 == 0.0 else 3) and (orc["status"] == 0).sum() > 500
     # every ray starts on the flat screen, not at the observer: the start radius varies over the image
     assert res["status_mismatch"] == 0
+
+
+def test_no_write_outside_the_callers_buffers(gp):
+    """compute-sanitizer is not available on this pool, so the bounds are checked with canaries: every
+    output buffer sits between two guard pages filled with 0xA5 that must come back untouched, for
+    ragged ray counts, both kernels, the disk variant and the image-formation kernel."""
+    import torch
+    G = 4096
+    for name, count in (("C2", 1), ("C2", 1000), ("C3", 777), ("C1", 4096), ("C5a", 333)):
+        w = W.workload(name)
+        w["cfg"]["max_steps"] = min(w["cfg"]["max_steps"], 20000)
+        b, c, s = W.ray_selection(w, 17, count, 5)
+        cam = gp.api.camera_struct(w["camera"], b, c, s)
+        cfg = gp.api.cfg_struct(w["cfg"])
+        bufs = {}
+        for key, nbytes in (("rays", c * 128), ("disk", c * 48 if cfg.max_crossings else 0), ("counters", 64)):
+            if nbytes == 0:
+                bufs[key] = (None, None)
+                continue
+            raw = torch.full((nbytes + 2 * G,), 0xA5, dtype=torch.uint8, device="cuda")
+            bufs[key] = (raw, raw[G:G + nbytes])
+        gp.gp_trace(w["metric"]["id"], gp.api.metric_struct(w["metric"]), cam, cfg, bufs["rays"][1],
+                    bufs["disk"][1], bufs["counters"][1])
+        torch.cuda.synchronize()
+        for key, (raw, view) in bufs.items():
+            if raw is None:
+                continue
+            assert bool((raw[:G] == 0xA5).all()) and bool((raw[-G:] == 0xA5).all()), (name, count, key)
+        cnt = bufs["counters"][1].cpu().numpy().view("<u8")
+        assert cnt[1] == c
+        rec = bufs["rays"][1].cpu().numpy().view(gp.api.RAY_DTYPE)
+        assert (rec["status"] <= 4).all() and np.isfinite(rec["lambda"]).all()
+    # image formation
+    w = W.workload("C2", width=50, height=30, supersample=2)
+    rays, _, _ = gp.api.trace_workload(w)
+    r = torch.from_numpy(rays.view(np.uint8).copy()).cuda()
+    raw = torch.full((50 * 30 * 4 + 2 * G,), 0xA5, dtype=torch.uint8, device="cuda")
+    gp.gp_shade(gp.api.shade_struct(dict(width=50, height=30, supersample=2, mode=1, tex_width=64, tex_height=32)),
+                r, None, raw[G:G + 6000])
+    torch.cuda.synchronize()
+    assert bool((raw[:G] == 0xA5).all()) and bool((raw[-G:] == 0xA5).all())
+    assert bool((raw[G:G + 6000].view(-1, 4)[:, 3] == 255).all())
