@@ -907,4 +907,65 @@ int orc_trace_one(const orc_metric *m, const orc_camera *cam, const orc_cfg *cfg
   return 0;
 }
 
+// Orbits from explicit initial states (the time-like test orbits of section 3.2.1 are
+// the same equations with H = -1/2; neighbouring null orbits).  See gp_oracle.h.
+int orc_integrate_orbits(const orc_metric *m, const orc_orbit_cfg *cfg, const double *states8, int64_t n,
+                         double *samples, int64_t *status, int64_t *n_steps) {
+  if (!m || !cfg || !states8 || !samples || n < 0 || cfg->n_samples < 1) return -1;
+  if (!(cfg->rtol > 0.0) || !(cfg->atol >= 0.0) || !(cfg->h0 > 0.0) || !(cfg->h_max > 0.0) ||
+      !(cfg->lambda_end > 0.0))
+    return -1;
+  const double r_cap = horizon_radius(m) * (1.0 + cfg->eps_capture);
+  const double NaN = std::numeric_limits<double>::quiet_NaN();
+  const int64_t K = cfg->n_samples;
+#pragma omp parallel for schedule(dynamic, 1)
+  for (int64_t i = 0; i < n; ++i) {
+    const double *st = states8 + 8 * i;
+    double *out = samples + 8 * K * i;
+    for (int64_t j = 0; j < 8 * K; ++j) out[j] = NaN;
+    Sys S;
+    S.m = m;
+    S.pt = st[4];
+    S.pphi = st[7];
+    auto f = [&](const double *yy, double *dy) { rhs(S, yy, dy); };
+    double y[6] = {st[0], st[1], st[2], st[3], st[5], st[6]};
+    double lam = 0.0, h = cfg->h0;
+    double k[7][7];
+    f(y, k[0]);
+    int64_t next = 0, steps = 0, stat = 0;
+    while (next < K) {
+      if (steps >= cfg->max_steps) { stat = 2; break; }
+      if (h < 1e-14 * std::fmax(1.0, std::fabs(lam))) { stat = 4; break; }
+      const double lam_next = (double)(next + 1) * cfg->lambda_end / (double)K;
+      const double room = lam_next - lam;
+      double hs = std::fmin(h, cfg->h_max);
+      const bool cut = !(hs < room);       // the step is cut short (or exactly fits) at the sample time
+      if (cut) hs = room;
+      double ynew[6], errvec[7];
+      dp54_step(f, 6, y, hs, k, ynew, errvec);
+      ++steps;
+      double err = error_norm(y, ynew, errvec, cfg->rtol, cfg->atol);
+      if (!std::isfinite(err) || !all_finite(ynew, 6)) { h = hs * 0.2; continue; }
+      double fac = (err == 0.0) ? 5.0 : 0.9 * std::pow(err, -0.2);
+      if (err > 1.0) { h = hs * std::fmax(0.2, fac); continue; }
+      double hnew = hs * std::fmin(5.0, std::fmax(0.2, fac));
+      h = cut ? std::fmax(h, hnew) : hnew;
+      for (int c = 0; c < 6; ++c) y[c] = ynew[c];
+      for (int c = 0; c < 6; ++c) k[0][c] = k[6][c];   // FSAL
+      lam = cut ? lam_next : lam + hs;
+      if (y[1] < r_cap) { stat = 1; break; }
+      if (cut) {
+        double *o = out + 8 * next;
+        // 2H = p_mu dq^mu/dlambda: p_t dt + p_r dr + p_th dth + p_ph dph with the FSAL slopes
+        double H2 = S.pt * k[0][0] + y[4] * k[0][1] + y[5] * k[0][2] + S.pphi * k[0][3];
+        o[0] = y[0]; o[1] = y[1]; o[2] = y[2]; o[3] = y[3]; o[4] = y[4]; o[5] = y[5]; o[6] = H2; o[7] = lam;
+        ++next;
+      }
+    }
+    status[i] = stat;
+    n_steps[i] = steps;
+  }
+  return 0;
+}
+
 }  // extern "C"

@@ -96,6 +96,20 @@ int orc_trace(const orc_metric *m, const orc_camera *cam, const orc_cfg *cfg, in
 int orc_trace_one(const orc_metric *m, const orc_camera *cam, const orc_cfg *cfg, double alpha,
                   double beta, orc_record *out, double *path, int64_t n_path_max, int64_t *n_path);
 
+/* ---- orbits from explicit initial states (section 3.2.1: time-like test orbits with
+ * H = -1/2; Fig 11: neighbouring null orbits).  The same Hamilton's equations and the same
+ * Dormand-Prince pair, integrated to lambda_end with the state sampled at lambda_k = (k+1) lambda_end /
+ * n_samples: every attempted step is min(h, h_max, lambda_next - lambda); a step cut short by a sample
+ * time keeps the controller's previous proposal when that is larger.  samples: n * n_samples * 8
+ * doubles (t, r, theta, phi, p_r, p_theta, 2H, lambda), NaN after an orbit ended early; status per
+ * orbit: 0 reached lambda_end, 1 captured (r < r_H (1 + eps_capture)), 2 step budget, 4 step underflow. */
+typedef struct orc_orbit_cfg {
+  double rtol, atol, h0, h_max, lambda_end, eps_capture;
+  int64_t n_samples, max_steps;
+} orc_orbit_cfg;
+int orc_integrate_orbits(const orc_metric *m, const orc_orbit_cfg *cfg, const double *states8, int64_t n,
+                         double *samples, int64_t *status, int64_t *n_steps);
+
 #ifdef __cplusplus
 }
 #endif

@@ -277,5 +277,30 @@ def shade(cfg, status, theta, phi, t, disk_r0=None, disk_g0=None):
     return out
 
 
+# ---- orbits from explicit initial states -----------------------------------------------------------
+class OrcOrbitCfg(C.Structure):
+    _fields_ = [("rtol", _f64), ("atol", _f64), ("h0", _f64), ("h_max", _f64), ("lambda_end", _f64),
+                ("eps_capture", _f64), ("n_samples", _i64), ("max_steps", _i64)]
+
+
+def integrate_orbits(metric, states8, cfg):
+    """states8: (n, 8) array (t, r, theta, phi, p_t, p_r, p_theta, p_phi); cfg: dict.  Returns
+    (samples (n, n_samples, 8), status (n,), n_steps (n,))."""
+    st = np.ascontiguousarray(states8, dtype=np.float64).reshape(-1, 8)
+    n = st.shape[0]
+    c = OrcOrbitCfg(cfg["rtol"], cfg["atol"], cfg["h0"], cfg["h_max"], cfg["lambda_end"],
+                    cfg.get("eps_capture", 1e-3), cfg["n_samples"], cfg.get("max_steps", 10 ** 7))
+    samples = np.empty((n, c.n_samples, 8))
+    status = np.zeros(n, dtype=np.int64)
+    steps = np.zeros(n, dtype=np.int64)
+    f = lib().orc_integrate_orbits
+    P = C.POINTER
+    f.argtypes = [P(OrcMetric), P(OrcOrbitCfg), P(_f64), _i64, P(_f64), P(_i64), P(_i64)]
+    f.restype = C.c_int
+    _check(f(C.byref(_metric(metric)), C.byref(c), _dp(st), n, _dp(samples), status.ctypes.data_as(P(_i64)),
+             steps.ctypes.data_as(P(_i64))), "integrate_orbits")
+    return samples, status, steps
+
+
 def host_threads():
     return os.cpu_count() or 1
