@@ -255,6 +255,28 @@ typedef struct gp_shade_cfg {
 int gp_shade(const gp_shade_cfg *cfg, const void *rays, size_t rays_bytes, const void *disk,
              size_t disk_bytes, void *rgba8, size_t rgba_bytes, void *cuda_stream);
 
+/* ---- orbits from explicit initial states (section 3.2.1 and Fig 1: time-like
+ * test orbits, the same equations with H = -1/2; L719, Fig 11: neighbouring null orbits; SURVEY.md
+ * section 8(f) NEXT-3) --------------------------------------------------------------------------
+ * Integrates n states (t, r, theta, phi, p_t, p_r, p_theta, p_phi; any value of H) with the
+ * Dormand-Prince pair and the controller of scheme 2 from lambda = 0 to lambda_end, every attempted
+ * step being min(h, h_max, lambda_next - lambda) so that the state is sampled exactly at
+ * lambda_k = (k+1) lambda_end / n_samples, k < n_samples; a step cut short by a sample time keeps
+ * the controller's previous proposal when that is larger; the first proposal is h0.
+ * states8: DEVICE n*8 doubles.  samples: DEVICE n*n_samples*8 doubles, per sample
+ * (t, r, theta, phi, p_r, p_theta, 2H, lambda), NaN after an orbit ended early.  status: DEVICE n
+ * uint32 (GP_RAY_ESCAPED = reached lambda_end, GP_RAY_CAPTURED = r < r_H (1 + eps_capture),
+ * GP_RAY_MAXSTEPS, GP_RAY_STEP_UNDERFLOW).  n_steps: DEVICE n uint64 attempted steps.
+ * GP_E_BAD_PARAM on non-positive rtol, h0, h_max, lambda_end, n_samples, negative atol / max_steps. */
+typedef struct gp_orbit_cfg {
+  double rtol, atol, h0, h_max, lambda_end, eps_capture;
+  int64_t n_samples, max_steps;
+} gp_orbit_cfg;
+
+int gp_integrate_orbits(int metric_id, const gp_metric_params *metric, const gp_orbit_cfg *cfg,
+                        const void *states8, int64_t n, void *samples, size_t samples_bytes, void *status,
+                        size_t status_bytes, void *n_steps, size_t n_steps_bytes, void *cuda_stream);
+
 /* Horizon radius r_H and prograde ISCO radius used by the library for these parameters
  * (r_isco = NaN for GP_MANKO_NOVIKOV).  Host-only helper.                               */
 int gp_metric_radii(int metric_id, const gp_metric_params *metric, double *r_horizon,

@@ -283,9 +283,10 @@ class OrcOrbitCfg(C.Structure):
                 ("eps_capture", _f64), ("n_samples", _i64), ("max_steps", _i64)]
 
 
-def integrate_orbits(metric, states8, cfg):
+def integrate_orbits(metric, states8, cfg, rounding_probe=False):
     """states8: (n, 8) array (t, r, theta, phi, p_t, p_r, p_theta, p_phi); cfg: dict.  Returns
-    (samples (n, n_samples, 8), status (n,), n_steps (n,))."""
+    (samples (n, n_samples, 8), status (n,), n_steps (n,)).  rounding_probe=True runs the
+    FMA-contracted build of the same source (flagging aid only, see lib_rounding_probe)."""
     st = np.ascontiguousarray(states8, dtype=np.float64).reshape(-1, 8)
     n = st.shape[0]
     c = OrcOrbitCfg(cfg["rtol"], cfg["atol"], cfg["h0"], cfg["h_max"], cfg["lambda_end"],
@@ -293,7 +294,7 @@ def integrate_orbits(metric, states8, cfg):
     samples = np.empty((n, c.n_samples, 8))
     status = np.zeros(n, dtype=np.int64)
     steps = np.zeros(n, dtype=np.int64)
-    f = lib().orc_integrate_orbits
+    f = (lib_rounding_probe() if rounding_probe else lib()).orc_integrate_orbits
     P = C.POINTER
     f.argtypes = [P(OrcMetric), P(OrcOrbitCfg), P(_f64), _i64, P(_f64), P(_i64), P(_i64)]
     f.restype = C.c_int

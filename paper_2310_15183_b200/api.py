@@ -52,6 +52,11 @@ class gp_shade_cfg(C.Structure):
                 ("g_lo", _f64), ("g_hi", _f64)]
 
 
+class gp_orbit_cfg(C.Structure):
+    _fields_ = [("rtol", _f64), ("atol", _f64), ("h0", _f64), ("h_max", _f64), ("lambda_end", _f64),
+                ("eps_capture", _f64), ("n_samples", _i64), ("max_steps", _i64)]
+
+
 class gp_out_buffers(C.Structure):
     _fields_ = [("rays", C.c_void_p), ("rays_bytes", C.c_size_t),
                 ("disk", C.c_void_p), ("disk_bytes", C.c_size_t),
@@ -68,7 +73,7 @@ RAY_DTYPE = np.dtype([
 DISK_DTYPE = np.dtype([("r_cross", "<f8", (3,)), ("g", "<f8", (3,))])
 assert RAY_DTYPE.itemsize == 128 and DISK_DTYPE.itemsize == 48
 
-EXPORTS = ("gp_shade", "gp_trace", "gp_trace_host", "gp_init_conditions", "gp_eval_metric", "gp_eval_rhs",
+EXPORTS = ("gp_integrate_orbits", "gp_shade", "gp_trace", "gp_trace_host", "gp_init_conditions", "gp_eval_metric", "gp_eval_rhs",
            "gp_probe_fp64_fma", "gp_metric_radii", "gp_ray_record_size", "gp_disk_record_size",
            "gp_counters_size", "gp_version", "gp_strerror")
 
@@ -88,6 +93,9 @@ def _load():
     L.gp_eval_rhs.argtypes = [C.c_int, P(gp_metric_params), vp, _i64, vp, sz, vp]
     L.gp_probe_fp64_fma.argtypes = [_i64, vp, sz, P(_f64), vp]
     L.gp_metric_radii.argtypes = [C.c_int, P(gp_metric_params), P(_f64), P(_f64)]
+    L.gp_integrate_orbits.argtypes = [C.c_int, P(gp_metric_params), P(gp_orbit_cfg), vp, _i64, vp, sz, vp, sz,
+                                      vp, sz, vp]
+    L.gp_integrate_orbits.restype = C.c_int
     L.gp_shade.argtypes = [P(gp_shade_cfg), vp, sz, vp, sz, vp, sz, vp]
     L.gp_shade.restype = C.c_int
     for n in ("gp_trace", "gp_trace_host", "gp_init_conditions", "gp_eval_metric", "gp_eval_rhs",
@@ -212,6 +220,21 @@ def gp_probe_fp64_fma(iters, scratch, stream=None):
     _check(lib.gp_probe_fp64_fma(int(iters), p, n, C.byref(flops), _stream_ptr(stream)),
            "gp_probe_fp64_fma")
     return flops.value
+
+
+def orbit_struct(d):
+    return gp_orbit_cfg(d["rtol"], d["atol"], d["h0"], d["h_max"], d["lambda_end"], d.get("eps_capture", 1e-3),
+                        int(d["n_samples"]), int(d.get("max_steps", 10 ** 7)))
+
+
+def gp_integrate_orbits(metric_id, metric, cfg, states8, samples, status, n_steps, stream=None):
+    """states8 (n, 8) f64, samples (n, n_samples, 8) f64, status (n,) int32, n_steps (n,) int64: CUDA tensors."""
+    p, _ = _dev(states8)
+    q, m = _dev(samples)
+    r, k = _dev(status)
+    u, v = _dev(n_steps)
+    _check(lib.gp_integrate_orbits(int(metric_id), C.byref(metric), C.byref(cfg), p, states8.shape[0], q, m, r, k,
+                                   u, v, _stream_ptr(stream)), "gp_integrate_orbits")
 
 
 def shade_struct(d):

@@ -10,6 +10,7 @@
 #include "../../include/gp.h"
 #include "gp_trace.cuh"
 #include "gp_shade.cuh"
+#include "gp_orbits.cuh"
 
 static_assert(sizeof(gp_ray_record) == 128, "gp_ray_record must be 128 bytes");
 static_assert(offsetof(gp_ray_record, status) == 40 && offsetof(gp_ray_record, p_t) == 64 &&
@@ -468,6 +469,41 @@ int gp_probe_fp64_fma(int64_t iters, void *scratch, size_t scratch_bytes, double
   k_probe_fma<<<blocks, threads, 0, (cudaStream_t)cuda_stream>>>(iters, 0.5, (double *)scratch);
   GP_CUDA(cudaGetLastError());
   *flops_out = 2.0 * 64.0 * (double)iters * (double)blocks * (double)threads;
+  return GP_OK;
+}
+
+int gp_integrate_orbits(int metric_id, const gp_metric_params *metric, const gp_orbit_cfg *cfg,
+                        const void *states8, int64_t n, void *samples, size_t samples_bytes, void *status,
+                        size_t status_bytes, void *n_steps, size_t n_steps_bytes, void *cuda_stream) {
+  if (!metric || !cfg) return GP_E_NULL;
+  OrbitParams P;
+  memset(&P, 0, sizeof(P));
+  int rc = make_metric(metric_id, metric, &P.mc);
+  if (rc) return rc;
+  if (!(cfg->rtol > 0.0) || !(cfg->atol >= 0.0) || !(cfg->h0 > 0.0) || !(cfg->h_max > 0.0) ||
+      !(cfg->lambda_end > 0.0) || !(cfg->eps_capture >= 0.0) || cfg->n_samples < 1 || cfg->max_steps < 0 || n < 0)
+    return GP_E_BAD_PARAM;
+  if (!isfinite(cfg->rtol) || !isfinite(cfg->atol) || !isfinite(cfg->h0) || !isfinite(cfg->h_max) ||
+      !isfinite(cfg->lambda_end) || !isfinite(cfg->eps_capture))
+    return GP_E_BAD_PARAM;
+  if (n == 0) return GP_OK;
+  if (!states8 || !samples || !status || !n_steps) return GP_E_NULL;
+  if (samples_bytes < (size_t)n * (size_t)cfg->n_samples * 64 || status_bytes < (size_t)n * 4 ||
+      n_steps_bytes < (size_t)n * 8)
+    return GP_E_SIZE;
+  P.rtol = cfg->rtol; P.atol = cfg->atol; P.h0 = cfg->h0; P.h_max = cfg->h_max; P.lambda_end = cfg->lambda_end;
+  P.r_cap = P.mc.r_horizon * (1.0 + cfg->eps_capture);
+  P.n = n; P.n_samples = cfg->n_samples; P.max_steps = cfg->max_steps;
+  P.states8 = (const double *)states8;
+  P.samples = (double *)samples;
+  P.status = (unsigned *)status;
+  P.n_steps = (unsigned long long *)n_steps;
+  const unsigned grid = (unsigned)((n + 127) / 128);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (metric_id == GP_SCHWARZSCHILD) k_integrate_orbits<METRIC_SCHW><<<grid, 128, 0, st>>>(P);
+  else if (metric_id == GP_KERR) k_integrate_orbits<METRIC_KERR><<<grid, 128, 0, st>>>(P);
+  else k_integrate_orbits<METRIC_MN><<<grid, 128, 0, st>>>(P);
+  GP_CUDA(cudaGetLastError());
   return GP_OK;
 }
 
