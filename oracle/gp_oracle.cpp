@@ -300,6 +300,43 @@ void kepler(const orc_metric *m, double r, double pt, double pphi, double out[3]
   out[2] = 1.0 / (ut * (pt + Om * pphi));
 }
 
+// The same emitter for any of the metrics, as the paper states it (eq 56, reading R20):
+// a circular equatorial orbit has dp_r/dlambda = 0 and p_r = p_theta = 0; with p_t = -1 that is the
+// quadratic  d_r g^{phi phi} p_phi^2 + 2 d_r g^{t phi} p_t p_phi + d_r g^{tt} p_t^2 = 0  in p_phi
+// (the paper differentiates numerically; here the derivatives are the oracle's own d_r g^{mu nu}).
+// The root with Omega > 0 is taken (the +phi direction of Omega_K = sqrt(M)/(r^{3/2} + a sqrt(M)), R19:
+// co-rotating when a > 0).  Then p is
+// normalised to p^2 = -1 and g = 1/[u^t (p_t + Omega p_phi)] (R19).  Returns -1 when no circular
+// orbit exists at r (negative discriminant or a space-like root).
+int kepler_general(const orc_metric *m, double r, double pt, double pphi, double out[3]) {
+  double g[15];
+  if (metric_inv(m, r, kHalfPi, g)) return -1;
+  const double gtt = g[0], gtp = g[1], gpp = g[2];
+  const double A = g[7], B = g[6], C = g[5];      // d_r g^{phi phi}, d_r g^{t phi}, d_r g^{tt}
+  const double disc = B * B - A * C;
+  if (!(disc >= 0.0)) return -1;
+  double best_Om = 0.0, best_ut = 0.0;
+  bool found = false;
+  for (int k = 0; k < 2; ++k) {
+    double pph_e = (B + (k == 0 ? 1.0 : -1.0) * std::sqrt(disc)) / A;   // p_t = -1
+    double ut_raw = -gtt + gtp * pph_e;                                   // g^{t mu} p_mu
+    double uph_raw = -gtp + gpp * pph_e;
+    double N = -(gtt - 2.0 * gtp * pph_e + gpp * pph_e * pph_e);          // -p^2
+    if (!(N > 0.0) || !(ut_raw > 0.0)) continue;
+    double Om = uph_raw / ut_raw;
+    if (Om > 0.0) {
+      best_Om = Om;
+      best_ut = ut_raw / std::sqrt(N);
+      found = true;
+    }
+  }
+  if (!found) return -1;
+  out[0] = best_Om;
+  out[1] = best_ut;
+  out[2] = 1.0 / (best_ut * (pt + best_Om * pphi));
+  return 0;
+}
+
 // ------------------------------------------------------------------------------------------
 // O1: ray index -> (alpha, beta)   (R11; evaluated with individually rounded operations)
 // ------------------------------------------------------------------------------------------
@@ -710,8 +747,9 @@ void trace_ray(const orc_metric *m, const orc_camera *cam, const orc_cfg *cfg, d
         ++n_land;
         double rc = yl[1];
         if (rc >= r_in && rc <= r_out) {
-          double kp[3];
-          kepler(m, rc, S.pt, S.pphi, kp);
+          double kp[3] = {NaN, NaN, NaN};
+          if (m->id == 2) kepler_general(m, rc, S.pt, S.pphi, kp);   // no circular orbit there: g = NaN
+          else kepler(m, rc, S.pt, S.pphi, kp);
           rec->disk_r[n_rec] = rc;
           rec->disk_g[n_rec] = kp[2];
           ++n_rec;
@@ -829,6 +867,11 @@ int orc_kepler(const orc_metric *m, double r, double p_t, double p_phi, double *
   return 0;
 }
 
+int orc_kepler_general(const orc_metric *m, double r, double p_t, double p_phi, double *out3) {
+  if (!valid_metric(m)) return -1;
+  return kepler_general(m, r, p_t, p_phi, out3);
+}
+
 void orc_dp54_tableau(double *c7, double *a49, double *b7, double *e7) {
   for (int i = 0; i < 7; ++i) {
     c7[i] = DP_C[i];
@@ -872,7 +915,7 @@ static int valid_run(const orc_metric *m, const orc_camera *cam, const orc_cfg *
   if (!valid_metric(m) || !cam || !cfg) return 0;
   if (cfg->scheme < 0 || cfg->scheme > 2) return 0;
   if (cfg->max_crossings < 0 || cfg->max_crossings > 3) return 0;
-  if (cfg->max_crossings > 0 && m->id == 2) return 0;
+  if (cfg->max_crossings > 0 && m->id == 2 && !(cfg->disk_r_in > 0.0)) return 0;  // no ISCO formula for Manko-Novikov
   if (cam->width <= 0 || cam->height <= 0 || cam->supersample <= 0) return 0;
   return 1;
 }

@@ -81,6 +81,8 @@ int orc_rhs(const orc_metric *m, const double *state8, double *rhs6);
 int orc_radii(const orc_metric *m, double *r_horizon, double *r_isco);
 /* prograde Keplerian emitter: Omega_K, u^t, and g for a ray with constants (p_t, p_phi) */
 int orc_kepler(const orc_metric *m, double r, double p_t, double p_phi, double *out3);
+/* the same from eq 56 solved with the metric's own d_r g^{mu nu} (any metric) */
+int orc_kepler_general(const orc_metric *m, double r, double p_t, double p_phi, double *out3);
 /* Dormand-Prince tableau: c[7], a[7*7] (row-major, lower triangle), b5[7], e[7] */
 void orc_dp54_tableau(double *c7, double *a49, double *b7, double *e7);
 /* one explicit step of scheme (0/1: RK4, 2: DP5(4)) from state8 with step h, for tests:

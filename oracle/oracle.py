@@ -174,6 +174,15 @@ def kepler(metric, r, p_t, p_phi):
     return out  # Omega_K, u^t, g
 
 
+def kepler_general(metric, r, p_t, p_phi):
+    out = np.empty(3)
+    f = lib().orc_kepler_general
+    f.argtypes = [C.POINTER(OrcMetric), _f64, _f64, _f64, C.POINTER(_f64)]
+    f.restype = C.c_int
+    _check(f(C.byref(_metric(metric)), float(r), float(p_t), float(p_phi), _dp(out)), "kepler_general")
+    return out  # Omega, u^t, g
+
+
 def dp54_tableau():
     c, a, b, e = np.empty(7), np.empty(49), np.empty(7), np.empty(7)
     lib().orc_dp54_tableau(_dp(c), _dp(a), _dp(b), _dp(e))
