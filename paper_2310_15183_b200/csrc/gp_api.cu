@@ -173,7 +173,8 @@ int make_params(int metric_id, const gp_metric_params *m, const gp_camera *cam, 
     if (!isfinite(cfg->rtol) || !isfinite(cfg->atol) || !isfinite(cfg->h_cap_rel)) return GP_E_BAD_PARAM;
   }
   if (cfg->max_crossings < 0 || cfg->max_crossings > 3) return GP_E_BAD_PARAM;
-  if (cfg->max_crossings > 0 && metric_id == GP_MANKO_NOVIKOV) return GP_E_UNSUPPORTED;
+  // a Manko-Novikov disk needs an explicit inner radius: there is no ISCO formula for that metric
+  if (cfg->max_crossings > 0 && metric_id == GP_MANKO_NOVIKOV && !(cfg->disk_r_in > 0.0)) return GP_E_BAD_PARAM;
   if (isnan(cfg->lambda_max)) return GP_E_BAD_PARAM;
   P->scheme = cfg->scheme;
   P->precision = cfg->precision;
@@ -247,7 +248,7 @@ int launch_trace(int metric_id, const TraceParams &P, cudaStream_t stream) {
     case GP_KERR:
       return disk ? launch_one<METRIC_KERR, true>(P, stream) : launch_one<METRIC_KERR, false>(P, stream);
     default:
-      return launch_one<METRIC_MN, false>(P, stream);
+      return disk ? launch_one<METRIC_MN, true>(P, stream) : launch_one<METRIC_MN, false>(P, stream);
   }
 }
 

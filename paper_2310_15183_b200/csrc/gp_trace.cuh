@@ -153,7 +153,7 @@ __device__ __forceinline__ long long fetch_slot(unsigned need_mask, bool need, u
 
 // Prograde Keplerian emitter on the equator (eq 56 in closed form; L372,
 // eq 57; readings R19/R20): g = (p.u_obs)/(p.u_emit) = 1/[u^t (p_t + Omega_K p_phi)].
-__device__ __forceinline__ double kepler_g(const MetricConst &mc, double r, double pt, double pph) {
+__device__ __forceinline__ double kepler_g_closed(const MetricConst &mc, double r, double pt, double pph) {
   double sM = sqrt(mc.M);
   double sr = sqrt(r);
   double r32 = r * sr;
@@ -161,6 +161,45 @@ __device__ __forceinline__ double kepler_g(const MetricConst &mc, double r, doub
   double Om = sM / den;
   double ut = den / (sqrt(r32) * sqrt(r32 - 3.0 * mc.M * sr + 2.0 * mc.a * sM));
   return 1.0 / (ut * (pt + Om * pph));
+}
+
+// The same emitter from eq 56 itself, for metrics without a closed form (Manko-Novikov): with
+// p_t = -1 the circular-orbit condition dp_r/dlambda = 0 is the quadratic
+// d_r g^{phi phi} p_phi^2 - 2 d_r g^{t phi} p_phi + d_r g^{tt} = 0; the derivatives come from the dual
+// numbers of metric_inv15; the root with Omega > 0 is taken and p normalised to p^2 = -1.  NaN when
+// there is no circular orbit at r.  Runs once per recorded crossing: kept out of line.
+__device__ __noinline__ double kepler_g_general(int metric, const MetricConst &mc, double r, double pt, double pph) {
+  double g[15];
+  metric_inv15(metric, mc, r, kHalfPi, g);
+  const double gtt = g[0], gtp = g[1], gpp = g[2];
+  const double A = g[7], B = g[6], C = g[5];
+  const double disc = B * B - A * C;
+  double Om_best = 0.0, ut_best = 0.0;
+  bool found = false;
+  if (disc >= 0.0) {
+    const double sq = sqrt(disc);
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+      double pe = (B + (k == 0 ? sq : -sq)) / A;
+      double ut_raw = gtp * pe - gtt;
+      double uph_raw = gpp * pe - gtp;
+      double N = -(gtt - 2.0 * gtp * pe + gpp * pe * pe);
+      double Om = uph_raw / ut_raw;
+      if (N > 0.0 && ut_raw > 0.0 && Om > 0.0) {
+        Om_best = Om;
+        ut_best = ut_raw / sqrt(N);
+        found = true;
+      }
+    }
+  }
+  if (!found) return __longlong_as_double(0x7ff8000000000000LL);
+  return 1.0 / (ut_best * (pt + Om_best * pph));
+}
+
+template <int METRIC>
+__device__ __forceinline__ double kepler_g(const MetricConst &mc, double r, double pt, double pph) {
+  if (METRIC == METRIC_MN) return kepler_g_general(METRIC_MN, mc, r, pt, pph);
+  return kepler_g_closed(mc, r, pt, pph);
 }
 
 // Monitors of row a10 carried per lane.

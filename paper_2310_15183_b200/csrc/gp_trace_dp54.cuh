@@ -222,7 +222,7 @@ trace_dp54(const __grid_constant__ TraceParams P) {
           double rc = nr;
           if (rc >= P.disk_r_in && rc <= P.disk_r_out) {
             P.disk[slot].r_cross[n_rec] = rc;
-            P.disk[slot].g[n_rec] = kepler_g(mc, rc, pt, pph);
+            P.disk[slot].g[n_rec] = kepler_g<METRIC>(mc, rc, pt, pph);
             ++n_rec;
           }
           r = lds1(PS(0)); th = lds1(PS(1)); pr = lds1(PS(2)); pth = lds1(PS(3));

@@ -156,7 +156,7 @@ __global__ void __launch_bounds__(kBlock) trace_rk4(const __grid_constant__ Trac
             const double rc = (double)nr;
             if (rc >= P.disk_r_in && rc <= P.disk_r_out) {
               P.disk[slot].r_cross[n_rec] = rc;
-              P.disk[slot].g[n_rec] = kepler_g(mc, rc, (double)pt, (double)pph);
+              P.disk[slot].g[n_rec] = kepler_g<METRIC>(mc, rc, (double)pt, (double)pph);
               ++n_rec;
             }
             const T *pk = park + tid;

@@ -123,10 +123,11 @@ def test_validation_is_synchronous(entry, what, mutate, metric_id, code):
     assert _call(W.workload("C2"), mutate, metric_id, entry=entry) == code
 
 
-def test_manko_novikov_needs_spin_and_has_no_disk():
+def test_manko_novikov_needs_spin_and_an_explicit_inner_disk_radius():
     w = W.workload("C4")
     assert _call(w, lambda m, c, g: setattr(m, "a", 0.0)) == api.GP_E_BAD_PARAM  # eq 23 divides by S/M
-    assert _call(w, lambda m, c, g: setattr(g, "max_crossings", 2)) == api.GP_E_UNSUPPORTED
+    # no ISCO formula for this metric: disk_r_in = 0 ("use the ISCO") is refused, an explicit one accepted
+    assert _call(w, lambda m, c, g: setattr(g, "max_crossings", 2)) == api.GP_E_BAD_PARAM
 
 
 def test_buffer_checks():

@@ -541,3 +541,31 @@ def test_no_write_outside_the_callers_buffers(gp):
     torch.cuda.synchronize()
     assert bool((raw[:G] == 0xA5).all()) and bool((raw[-G:] == 0xA5).all())
     assert bool((raw[G:G + 6000].view(-1, 4)[:, 3] == 255).all())
+
+
+# ---- Manko-Novikov disk with the general-metric emitter (eq 56 solved; PAPER.md Figs 16-17) -------
+@pytest.mark.parametrize("scheme", ["dp54", "rk4"])
+def test_manko_novikov_disk_with_the_eq56_emitter(gp, O, scheme):
+    w = W.workload("C4", width=256, height=256, theta_obs=math.radians(80.0))
+    w["cfg"].update(max_steps=3000, max_crossings=3, disk_r_in=4.0, disk_r_out=20.0)
+    if scheme == "rk4":
+        w["cfg"].update(scheme=1, h_rel=0.02, max_steps=6000)
+    rays, disk, _, orc, probe = run_both(gp, O, w, 3, None, 7)
+    res, ok = check_parity(w, rays, orc, probe, f"MN disk {scheme}", max_flagged_fraction=0.03)
+    n_rec = orc["n_disk_recorded"]
+    assert (n_rec > 0).sum() > 300 and n_rec.max() >= 2
+    # crossings are compared on the smooth escaped rays (the mask check_parity returns)
+    good = ok
+    for k in range(3):
+        have = good & (n_rec > k)
+        assert np.array_equal(np.isnan(disk["r_cross"][good, k]), np.isnan(orc["disk_r"][good, k]))
+        if have.any():
+            assert rel_err(disk["r_cross"][have, k], orc["disk_r"][have, k]).max() <= TOL
+            assert rel_err(disk["g"][have, k], orc["disk_g"][have, k]).max() <= 1e-8   # d_r g^{mu nu}: duals vs complex step
+    g = disk["g"][good & (n_rec > 0), 0]
+    assert np.isfinite(g).all() and (g > 1).any() and (g < 1).any()
+    # disk_r_in = 0 asks for the ISCO, which this metric has no formula for
+    w["cfg"]["disk_r_in"] = 0.0
+    with pytest.raises(gp.api.GpError) as e:
+        gp.api.trace_workload(w, 0, 10, 1)
+    assert e.value.code == gp.api.GP_E_BAD_PARAM
