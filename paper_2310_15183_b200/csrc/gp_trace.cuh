@@ -96,7 +96,10 @@ __device__ __forceinline__ void ray_birth(const CameraConst &cc, const MetricCon
 }
 #endif
 
-constexpr int kBlock = 128;
+#ifndef GP_BLOCK
+#define GP_BLOCK 128
+#endif
+constexpr int kBlock = GP_BLOCK;
 constexpr unsigned kFull = 0xffffffffu;
 constexpr double kHalfPi = 1.57079632679489661923;
 
