@@ -139,14 +139,16 @@ def oracle_sample(w, seconds):
     probe = min(total, 4096)
     stride = max(1, total // probe) | 1
     b, c, s = W.ray_selection(w, 1, probe, stride)
+    # all host cores, also under torchrun (which exports OMP_NUM_THREADS=1)
+    cores = os.cpu_count() or 1
     t0 = time.perf_counter()
-    _, used = O.trace(w, b, c, s)
+    _, used = O.trace(w, b, c, s, n_threads=cores)
     rate = c / max(time.perf_counter() - t0, 1e-6)
     count = int(min(total, max(probe, rate * seconds)))
     stride = 1 if count >= total else (-(-total // count)) | 1   # odd stride: the sample scatters over the image
     b, c, s = W.ray_selection(w, 0, None, stride)
     t0 = time.perf_counter()
-    rec, used = O.trace(w, b, c, s)
+    rec, used = O.trace(w, b, c, s, n_threads=cores)
     dt = time.perf_counter() - t0
     return {"value": c / dt, "unit": "geodesics/s", "cores": int(used), "kind": "oracle",
             "sample": f"{c} rays of {w['name']} (every {s}th ray from ray {b}), {dt:.2f} s wall, "
