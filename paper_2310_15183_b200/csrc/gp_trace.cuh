@@ -106,13 +106,14 @@ constexpr double kHalfPi = 1.57079632679489661923;
 // Dormand & Prince (1980) 5(4) pair, reading R10.  The coefficients sit in __constant__ memory so
 // that DFMA/DMUL take them as c[bank][offset] operands: as literals each use cost two UMOVs
 // (profiles/r01: 17 % of all warp instructions).
-struct DpTableau {
-  double A21;
+// Rows start on 16-byte boundaries so that the compiler can fetch two coefficients per LDCU.128.
+struct alignas(16) DpTableau {
+  double A21, pad0_;
   double A31, A32;
-  double A41, A42, A43;
+  double A41, A42, A43, pad1_;
   double A51, A52, A53, A54;
-  double A61, A62, A63, A64, A65;
-  double B1, B3, B4, B5, B6;
+  double A61, A62, A63, A64, A65, pad2_;
+  double B1, B3, B4, B5, B6, pad3_;
   double E1, E3, E4, E5, E6, E7;
   double safety, fac_min, fac_max, err_lo, err_hi, h_floor;  // controller constants, R10 items 3 and 5
   double sixth;                                              // RK4 weight 1/6 (eq 44)
@@ -120,12 +121,12 @@ struct DpTableau {
 
 #if defined(__CUDACC__)
 __constant__ DpTableau dp = {
-    1.0 / 5.0,
+    1.0 / 5.0, 0.0,
     3.0 / 40.0, 9.0 / 40.0,
-    44.0 / 45.0, -56.0 / 15.0, 32.0 / 9.0,
+    44.0 / 45.0, -56.0 / 15.0, 32.0 / 9.0, 0.0,
     19372.0 / 6561.0, -25360.0 / 2187.0, 64448.0 / 6561.0, -212.0 / 729.0,
-    9017.0 / 3168.0, -355.0 / 33.0, 46732.0 / 5247.0, 49.0 / 176.0, -5103.0 / 18656.0,
-    35.0 / 384.0, 500.0 / 1113.0, 125.0 / 192.0, -2187.0 / 6784.0, 11.0 / 84.0,
+    9017.0 / 3168.0, -355.0 / 33.0, 46732.0 / 5247.0, 49.0 / 176.0, -5103.0 / 18656.0, 0.0,
+    35.0 / 384.0, 500.0 / 1113.0, 125.0 / 192.0, -2187.0 / 6784.0, 11.0 / 84.0, 0.0,
     71.0 / 57600.0, -71.0 / 16695.0, 71.0 / 1920.0, -17253.0 / 339200.0, 22.0 / 525.0, -1.0 / 40.0,
     0.9, 0.2, 5.0, 1.0e-5, 1.0e4, 1.0e-14,
     1.0 / 6.0};
