@@ -178,9 +178,12 @@ int gp_trace(int metric_id, const gp_metric_params *metric, const gp_camera *cam
              const gp_integrator_cfg *cfg, const gp_out_buffers *out, void *cuda_stream);
 
 /* Same computation with HOST output buffers (out->* are host pointers, pinned or
- * pageable; counters may be NULL).  Allocates device scratch with cudaMallocAsync on the
- * stream, runs gp_trace, copies the records back and SYNCHRONISES the stream before
- * returning.  This is the end-to-end call bench.py times.                               */
+ * pageable; counters may be NULL).  Pinned (page-locked, mapped) rays / disk buffers are written
+ * by the kernel itself, record by record as the rays end, so the transfer overlaps the tracing;
+ * pageable buffers are staged through device scratch from a library-owned stream-ordered pool and
+ * copied back.  Either way the stream is SYNCHRONISED before returning.  This is the end-to-end
+ * call bench.py times.  (One device per process: the scratch pool and the 64-byte device counters
+ * belong to the device current at the first call.)                                           */
 int gp_trace_host(int metric_id, const gp_metric_params *metric, const gp_camera *camera,
                   const gp_integrator_cfg *cfg, const gp_out_buffers *out, void *cuda_stream);
 

@@ -356,6 +356,38 @@ int gp_trace_host(int metric_id, const gp_metric_params *metric, const gp_camera
   }
   if (out->counters && out->counters_bytes < 64) return GP_E_SIZE;
   cudaStream_t stream = (cudaStream_t)cuda_stream;
+  // Pinned (page-locked, mapped) host buffers are written by the kernel itself: a lane stores its
+  // 128-byte record once, when its ray ends, so the records cross PCIe while the other rays are still
+  // being integrated and no device-to-host copy remains after the kernel.  Pageable buffers take the
+  // staged path below (device scratch + cudaMemcpyAsync).
+  {
+    cudaPointerAttributes ar, ad;
+    bool direct = n > 0 && cudaPointerGetAttributes(&ar, out->rays) == cudaSuccess &&
+                  ar.type == cudaMemoryTypeHost && ar.devicePointer != nullptr;
+    if (direct && disk)
+      direct = cudaPointerGetAttributes(&ad, out->disk) == cudaSuccess && ad.type == cudaMemoryTypeHost &&
+               ad.devicePointer != nullptr;
+    cudaGetLastError();  // a pageable pointer leaves cudaErrorInvalidValue behind on old drivers
+    if (direct) {
+      static unsigned long long *dcount = nullptr;   // 64-byte device counters (the work counter stays on the device)
+      if (!dcount) GP_CUDA(cudaMalloc((void **)&dcount, 64));
+      gp_out_buffers dev;
+      dev.counters = dcount;
+      dev.counters_bytes = 64;
+      dev.rays = ar.devicePointer;
+      dev.rays_bytes = rays_b;
+      dev.disk = disk ? ad.devicePointer : nullptr;
+      dev.disk_bytes = disk_b;
+      rc = gp_trace(metric_id, metric, camera, cfg, &dev, cuda_stream);
+      if (rc != GP_OK) return rc;
+      cudaError_t e = cudaSuccess;
+      if (out->counters) e = cudaMemcpyAsync(out->counters, dcount, 64, cudaMemcpyDeviceToHost, stream);
+      cudaError_t e3 = cudaStreamSynchronize(stream);
+      if (e != cudaSuccess) return cuda_fail(e);
+      if (e3 != cudaSuccess) return cuda_fail(e3);
+      return GP_OK;
+    }
+  }
   // one scratch allocation: counters | ray records | disk records
   const size_t off_rays = 64, off_disk = off_rays + ((rays_b + 63) & ~(size_t)63);
   // The scratch comes from a library-owned stream-ordered pool that keeps its memory between

@@ -313,6 +313,17 @@ def test_step_budget_and_host_entry(gp, O):
     assert host_r.tobytes() == dev_r.tobytes()
     assert host_d.tobytes() == dev_d.tobytes()
     assert np.array_equal(host_c[1:4], dev_c[1:4])
+    # pinned host buffers: the kernel stores the records straight into them (no staging copy)
+    import torch
+    pin_r = torch.zeros(c * 128, dtype=torch.uint8, pin_memory=True).numpy().view(gp.api.RAY_DTYPE)
+    pin_d = torch.zeros(c * 48, dtype=torch.uint8, pin_memory=True).numpy().view(gp.api.DISK_DTYPE)
+    pin_c = np.zeros(8, dtype=np.uint64)
+    gp.gp_trace_host(w["metric"]["id"], gp.api.metric_struct(w["metric"]),
+                     gp.api.camera_struct(w["camera"], b, c, s), gp.api.cfg_struct(w["cfg"]),
+                     pin_r, pin_d, pin_c)
+    assert pin_r.tobytes() == dev_r.tobytes()
+    assert pin_d.tobytes() == dev_d.tobytes()
+    assert np.array_equal(pin_c[1:4], dev_c[1:4])
 
 
 # ---- full size, in the launch configuration bench.py times ------------------------------------
