@@ -175,8 +175,10 @@ __global__ void k_shade(const __grid_constant__ ShadeParams P) {
       // the first 64-byte half of the record: (t, r | theta, phi | lambda, status..) as three 128-bit loads
       // with a 64-byte L2 prefetch-size hint, so that the second half is not pulled in with it
       const char *rec = reinterpret_cast<const char *>(P.rays + ray);
+#pragma nv_diag_suppress 550
       double t, r_unused, th_raw, ph_raw;
       unsigned b0, b1, status, b3;
+#pragma nv_diag_default 550
       asm volatile("ld.global.nc.L2::64B.v2.f64 {%0, %1}, [%2];" : "=d"(t), "=d"(r_unused) : "l"(rec));
       asm volatile("ld.global.nc.L2::64B.v2.f64 {%0, %1}, [%2];" : "=d"(th_raw), "=d"(ph_raw) : "l"(rec + 16));
       asm volatile("ld.global.nc.L2::64B.v4.u32 {%0, %1, %2, %3}, [%4];"

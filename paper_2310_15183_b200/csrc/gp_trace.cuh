@@ -151,6 +151,8 @@ __device__ __forceinline__ long long fetch_slot(unsigned need_mask, bool need, u
   if ((int)lane == leader) base = atomicAdd(counter, (unsigned long long)__popc(need_mask));
   base = __shfl_sync(kFull, base, leader);
   if (!need) return -1;
+  // Slots are handed out in increasing order.  A centre-out order (longest rays first) was measured:
+  // 1.5 % slower on the Kerr headline, 0.8 % faster on Manko-Novikov config 4 — not kept.
   long long slot = (long long)(base + (unsigned long long)__popc(need_mask & ((1u << lane) - 1u)));
   return slot < ray_count ? slot : -1;
 }
