@@ -333,6 +333,12 @@ def run_b200(args):
                      "alg_flops_per_launch": flops, "kernel_ms": kern_ms,
                      "flop_model": f"{F_RHS[mid]:.0f}/RHS + {F_STEP[gs.scheme]:.0f}/step (DESIGN.md 6.2)"},
         "clocks": clocks, "gpu_launches": args.steps,
+        # end-of-image tail of the persistent kernel, from the device time stamps of the last launch
+        # (gp.h counters[4..7]): steady-state rate = 99 % of the rays / time until they had finished
+        "tail": {"kernel_ms": (int(cnt[7]) - int(cnt[4])) * 1e-6,
+                 "t99_ms": (int(cnt[5]) - int(cnt[4])) * 1e-6 if int(cnt[5]) else None,
+                 "steady_geodesics_per_s": (world * (n - n // 100) / ((int(cnt[5]) - int(cnt[4])) * 1e-9)
+                                            if int(cnt[5]) > int(cnt[4]) else None)},
     }
     if e2e:
         out["e2e"] = e2e

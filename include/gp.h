@@ -145,7 +145,10 @@ typedef struct gp_disk_record {
  * NULL.  counters: >= 64 bytes, 8-byte aligned; the library zeroes it on the stream, uses
  * word 0 as the atomic work counter and leaves totals behind:
  *   [0] work counter (>= ray_count at exit)  [1] rays finished  [2] attempted steps
- *   [3] RHS evaluations                      [4..7] reserved                            */
+ *   [3] RHS evaluations
+ *   [4] %globaltimer (ns) at kernel start   [5] when 99 % of the rays had finished (0 if never)
+ *   [6] rays finished, counted live         [7] %globaltimer when the last block left
+ * ([5]-[4] against [7]-[4] is the end-of-image tail of the persistent kernel.)                */
 typedef struct gp_out_buffers {
   void *rays;
   size_t rays_bytes;

@@ -208,6 +208,26 @@ __device__ __forceinline__ double kepler_g(const MetricConst &mc, double r, doub
   return kepler_g_closed(mc, r, pt, pph);
 }
 
+// Progress stamps ("steady-state rate excluding the final tail"): counters[4] =
+// %globaltimer (ns) when the kernel starts, [5] = when 99 % of the rays have finished, [7] = when
+// the last block leaves; [6] counts finished rays live (one atomic per ray: ~5e7/s against a limit far
+// above that).
+__device__ __forceinline__ unsigned long long global_ns() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+  return t;
+}
+__device__ __forceinline__ void stamp_start(unsigned long long *counters) {
+  if (blockIdx.x == 0 && threadIdx.x == 0) counters[4] = global_ns();
+}
+__device__ __forceinline__ void stamp_ray_done(unsigned long long *counters, long long ray_count) {
+  const unsigned long long done = atomicAdd(counters + 6, 1ull) + 1ull;
+  if ((long long)done == ray_count - ray_count / 100) counters[5] = global_ns();
+}
+__device__ __forceinline__ void stamp_end(unsigned long long *counters) {
+  if (threadIdx.x == 0) atomicMax(counters + 7, global_ns());
+}
+
 // Monitors of row a10 carried per lane.
 template <class T>
 struct MonitorsT {

@@ -84,6 +84,7 @@ trace_dp54(const __grid_constant__ TraceParams P) {
   unsigned n_acc = 0, n_rej = 0, n_cross = 0, n_rec = 0, n_land = 0, status = 0;
   bool exhausted = false;
   sts1(CS(C_TOT_RAYS), 0.0); sts1(CS(C_TOT_STEPS), 0.0); sts1(CS(C_TOT_RHS), 0.0);
+  stamp_start(P.counters);
 
   for (;;) {
     // ---- a1: refill idle lanes ----
@@ -272,6 +273,7 @@ trace_dp54(const __grid_constant__ TraceParams P) {
             P.disk[slot].g[i] = qnan;
           }
         }
+        stamp_ray_done(P.counters, P.cc.ray_count);
         sts1(CS(C_TOT_RAYS), lds1(CS(C_TOT_RAYS)) + 1.0);
         sts1(CS(C_TOT_STEPS), lds1(CS(C_TOT_STEPS)) + (double)attempts);
         sts1(CS(C_TOT_RHS), lds1(CS(C_TOT_RHS)) + (double)n_rhs);
@@ -407,6 +409,7 @@ trace_dp54(const __grid_constant__ TraceParams P) {
       atomicAdd(P.counters + 3, (unsigned long long)lds1(CS(C_TOT_RHS)));
     }
   }
+  stamp_end(P.counters);
 #undef KS
 #undef CS
 #undef PS

@@ -35,6 +35,7 @@ __global__ void __launch_bounds__(kBlock) trace_rk4(const __grid_constant__ Trac
   unsigned n_acc = 0, n_cross = 0, n_rec = 0, n_land = 0, status = 0;
   bool exhausted = false;
   unsigned long long tot_rays = 0, tot_steps = 0, tot_rhs = 0;
+  stamp_start(P.counters);
 
   for (;;) {
     // ---- a1: refill idle lanes ----
@@ -181,6 +182,7 @@ __global__ void __launch_bounds__(kBlock) trace_rk4(const __grid_constant__ Trac
             P.disk[slot].g[i] = qnan;
           }
         }
+        stamp_ray_done(P.counters, P.cc.ray_count);
         tot_rays += 1; tot_steps += n_acc; tot_rhs += n_rhs;
         mode = MODE_IDLE;
       }
@@ -192,6 +194,7 @@ __global__ void __launch_bounds__(kBlock) trace_rk4(const __grid_constant__ Trac
     atomicAdd(P.counters + 2, tot_steps);
     atomicAdd(P.counters + 3, tot_rhs);
   }
+  stamp_end(P.counters);
 }
 
 #endif  // __CUDACC__

@@ -248,6 +248,19 @@ def test_empty_and_ragged_selections(gp, O):
         check_parity(w, rays, orc, probe, f"ragged {count}", max_flagged_fraction=1.0)
 
 
+def test_progress_stamps(gp):
+    """gp.h counters[4..7]: start, 99 %, live count, end — ordered device time stamps."""
+    for name in ("C2", "C5a"):
+        w = W.workload(name, width=256, height=256)
+        rays, _, c = gp.api.trace_workload(w)
+        n = len(rays)
+        assert c[6] == n == c[1]
+        assert 0 < c[4] <= c[5] <= c[7]
+        assert (c[7] - c[4]) * 1e-9 < 5.0           # seconds
+    rays, _, c = gp.api.trace_workload(W.workload("C2"), 0, 0, 1)
+    assert c[5] == 0 and c[6] == 0
+
+
 def test_last_ray_of_the_image(gp, O):
     w = W.workload("C2")
     total = W.n_rays(w)
