@@ -162,3 +162,37 @@ def test_no_cpu_fallback_without_a_gpu():
     assert _call(w, out=out, entry="gp_trace_host") == api.GP_E_CUDA
     assert "CUDA error" in gp.gp_strerror(api.GP_E_CUDA)
     assert not rays.view(np.uint8).any()
+
+
+def test_shade_and_orbit_validation_is_synchronous():
+    """The two entry points of the widened scope validate before anything is enqueued (no GPU needed)."""
+    vp = C.c_void_p
+    ok = api.shade_struct(dict(width=4, height=4, mode=0))
+    call = lambda cfg, rays=0x1000, nb=16 * 128, disk=None, db=0, out=0x2000, ob=64: api.lib.gp_shade(
+        C.byref(cfg), vp(rays), nb, vp(disk) if disk else None, db, vp(out), ob, None)
+    assert call(api.shade_struct(dict(width=4, height=4, mode=5))) == api.GP_E_BAD_PARAM
+    assert call(api.shade_struct(dict(width=0, height=4, mode=0))) == api.GP_E_BAD_PARAM
+    assert call(api.shade_struct(dict(width=4, height=4, mode=0, grid_step_deg=-1.0))) == api.GP_E_BAD_PARAM
+    assert call(api.shade_struct(dict(width=4, height=4, mode=1, tex_width=0, tex_height=8))) == api.GP_E_BAD_PARAM
+    assert call(api.shade_struct(dict(width=4, height=4, mode=2, time_period=0.0))) == api.GP_E_BAD_PARAM
+    assert call(api.shade_struct(dict(width=4, height=4, mode=0, disk_overlay=1))) == api.GP_E_NULL
+    assert call(api.shade_struct(dict(width=4, height=4, mode=0, disk_overlay=1, g_lo=1.2)), disk=0x3000,
+                db=16 * 48) == api.GP_E_BAD_PARAM
+    assert call(ok, nb=15 * 128) == api.GP_E_SIZE
+    assert call(ok, ob=63) == api.GP_E_SIZE
+    assert api.lib.gp_shade(C.byref(ok), None, 0, None, 0, vp(0x2000), 64, None) == api.GP_E_NULL
+
+    m = api.gp_metric_params(1.0, 0.9, 0.0)
+    good = dict(rtol=1e-9, atol=1e-9, h0=0.1, h_max=1.0, lambda_end=10.0, n_samples=4)
+    orb = lambda cfg, n=2, sb=2 * 4 * 64, stb=8, nsb=16, metric=m, mid=api.GP_KERR: api.lib.gp_integrate_orbits(
+        mid, C.byref(metric), C.byref(api.orbit_struct(cfg)), vp(0x1000), n, vp(0x2000), sb, vp(0x3000), stb,
+        vp(0x4000), nsb, None)
+    for bad in (dict(good, rtol=0.0), dict(good, atol=-1.0), dict(good, h0=0.0), dict(good, h_max=-1.0),
+                dict(good, lambda_end=0.0), dict(good, n_samples=0), dict(good, max_steps=-1)):
+        assert orb(bad) == api.GP_E_BAD_PARAM, bad
+    assert orb(good, sb=2 * 4 * 64 - 1) == api.GP_E_SIZE
+    assert orb(good, stb=7) == api.GP_E_SIZE and orb(good, nsb=15) == api.GP_E_SIZE
+    assert orb(good, mid=9) == api.GP_E_BAD_METRIC
+    assert orb(good, metric=api.gp_metric_params(1.0, 1.5, 0.0)) == api.GP_E_BAD_PARAM
+    assert orb(good, n=0) == api.GP_OK            # nothing to do, nothing enqueued
+    assert orb(good, n=-1) == api.GP_E_BAD_PARAM
