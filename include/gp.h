@@ -185,8 +185,9 @@ int gp_trace(int metric_id, const gp_metric_params *metric, const gp_camera *cam
  * by the kernel itself, record by record as the rays end, so the transfer overlaps the tracing;
  * pageable buffers are staged through device scratch from a library-owned stream-ordered pool and
  * copied back.  Either way the stream is SYNCHRONISED before returning.  This is the end-to-end
- * call bench.py times.  (One device per process: the scratch pool and the 64-byte device counters
- * belong to the device current at the first call.)                                           */
+ * call bench.py times.  (One device per process and one call at a time: the scratch pool and the
+ * 64-byte device counters are library-owned and belong to the device current at the first call;
+ * gp_trace itself owns nothing and may run concurrently on different streams and buffers.)      */
 int gp_trace_host(int metric_id, const gp_metric_params *metric, const gp_camera *camera,
                   const gp_integrator_cfg *cfg, const gp_out_buffers *out, void *cuda_stream);
 
