@@ -593,3 +593,29 @@ def test_manko_novikov_disk_with_the_eq56_emitter(gp, O, scheme):
     with pytest.raises(gp.api.GpError) as e:
         gp.api.trace_workload(w, 0, 10, 1)
     assert e.value.code == gp.api.GP_E_BAD_PARAM
+
+
+def test_concurrent_traces_on_two_streams(gp):
+    """gp_trace owns nothing: two calls on different streams with different buffers may overlap and must
+    give the records of the same calls run one after the other."""
+    import torch
+    specs = [("C2", 0, 20000, 13), ("C5a", 5, 20000, 829)]
+    ref = [gp.api.trace_workload(W.workload(n), b, c, s)[0] for n, b, c, s in specs]
+    streams = [torch.cuda.Stream() for _ in specs]
+    bufs = []
+    for (n, b, c, s), st in zip(specs, streams):
+        w = W.workload(n)
+        rays = torch.empty(c * 128, dtype=torch.uint8, device="cuda")
+        cnt = torch.empty(64, dtype=torch.uint8, device="cuda")
+        bufs.append((rays, cnt))
+    torch.cuda.synchronize()
+    for _ in range(3):                       # enqueue alternately so that the launches interleave
+        for (n, b, c, s), st, (rays, cnt) in zip(specs, streams, bufs):
+            w = W.workload(n)
+            gp.gp_trace(w["metric"]["id"], gp.api.metric_struct(w["metric"]), gp.api.camera_struct(w["camera"], b, c, s),
+                        gp.api.cfg_struct(w["cfg"]), rays, None, cnt, st)
+    torch.cuda.synchronize()
+    for (rays, cnt), r in zip(bufs, ref):
+        got = rays.cpu().numpy().view(gp.api.RAY_DTYPE)
+        assert got.tobytes() == r.tobytes()
+        assert cnt.cpu().numpy().view("<u8")[1] == len(r)
