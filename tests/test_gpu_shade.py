@@ -1,8 +1,9 @@
 """Image formation through the C-ABI (gp_shade) against oracle/gp_shade_oracle.cpp: byte for byte.
 
-The records shaded are the CUDA path's own (they are inputs here: the step under test is records ->
-pixels), handed to the oracle as plain arrays; synthetic records cover the branches a traced image
-rarely reaches (raw angles far outside the principal range, every status, NaN disk slots)."""
+The records shaded come from the ORACLE's trace of the frame (no oracle input ever comes from the CUDA
+path): they are packed into the library's 128-byte layout for gp_shade and handed to the shading oracle
+as plain arrays.  Synthetic records cover the branches a traced image rarely reaches (raw angles far
+outside the principal range, every status, NaN disk slots)."""
 import math
 
 import numpy as np
@@ -23,6 +24,19 @@ def gp():
 def O():
     from oracle import oracle as O
     return O
+
+
+def records_from_oracle(gp, orc):
+    """Oracle trace records -> (gp_ray_record array, gp_disk_record array) in the library's layout."""
+    rays = np.zeros(len(orc), dtype=gp.api.RAY_DTYPE)
+    for f in ("t", "r", "theta", "phi", "lambda", "p_r", "p_theta", "p_t", "p_phi", "h_max", "q_drift",
+              "sin_theta_min", "err_margin"):
+        rays[f] = orc[f]
+    for f in ("status", "n_accepted", "n_rejected", "n_equator_crossings", "n_disk_recorded", "n_rhs"):
+        rays[f] = orc[f].astype(np.uint32)
+    disk = np.zeros(len(orc), dtype=gp.api.DISK_DTYPE)
+    disk["r_cross"], disk["g"] = orc["disk_r"], orc["disk_g"]
+    return rays, disk
 
 
 def gpu_shade(gp, cfg, rays_np, disk_np=None):
@@ -50,7 +64,7 @@ MODES = [dict(mode=0, grid_step_deg=15.0, grid_half_width_deg=0.4),
 @pytest.mark.parametrize("S", [1, 2])
 def test_shade_traced_kerr_image_is_bit_exact(gp, O, mode, S):
     w = W.workload("C2", width=192, height=160, supersample=S)
-    rays, _, _ = gp.api.trace_workload(w)
+    rays, _ = records_from_oracle(gp, O.trace(w)[0])
     cfg = dict(width=192, height=160, supersample=S, **mode)
     img = gpu_shade(gp, cfg, rays)
     ref = oracle_shade(O, cfg, rays)
@@ -64,7 +78,7 @@ def test_shade_traced_kerr_image_is_bit_exact(gp, O, mode, S):
 
 def test_shade_disk_overlay_is_bit_exact(gp, O):
     w = W.workload("C3", width=256, height=256)
-    rays, disk, _ = gp.api.trace_workload(w)
+    rays, disk = records_from_oracle(gp, O.trace(w)[0])
     cfg = dict(width=256, height=256, mode=0, grid_step_deg=10.0, grid_half_width_deg=0.3, disk_overlay=1,
                g_lo=0.2, g_hi=1.6)
     img = gpu_shade(gp, cfg, rays, disk)
