@@ -151,7 +151,7 @@ def oracle_sample(w, seconds):
     rec, used = O.trace(w, b, c, s, n_threads=cores)
     dt = time.perf_counter() - t0
     return {"value": c / dt, "unit": "geodesics/s", "cores": int(used), "kind": "oracle",
-            "sample": f"{c} rays of {w['name']} (every {s}th ray from ray {b}), {dt:.2f} s wall, "
+            "sample": f"{c} rays of {w['name']} (ray stride {s} from ray {b}), {dt:.2f} s wall, "
                       f"OpenMP dynamic over rays, g++ -O2 -ffp-contract=off",
             "rhs_evals_per_s": float(rec["n_rhs"].sum()) / dt, "seconds": dt, "rays": c}
 
