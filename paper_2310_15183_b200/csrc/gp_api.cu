@@ -185,7 +185,7 @@ int make_params(int metric_id, const gp_metric_params *m, const gp_camera *cam, 
   P->atol = cfg->atol;
   P->h_cap_rel = cfg->h_cap_rel;
   P->max_steps = cfg->max_steps;
-  P->lambda_max = cfg->lambda_max;
+  P->lambda_max = cfg->lambda_max > 0.0 ? cfg->lambda_max : (double)INFINITY;  // <= 0 = no affine budget
   P->r_cap = P->mc.r_horizon * (1.0 + cfg->eps_capture);
   P->r_esc = cfg->r_escape;
   if (cfg->max_crossings > 0) {

@@ -27,7 +27,7 @@ struct TraceParams {
   int max_crossings;                // 0 = disk off
   double h, h_rel, rtol, atol, h_cap_rel;
   long long max_steps;
-  double lambda_max;
+  double lambda_max;   // +inf when the configuration has no affine budget (cfg.lambda_max <= 0)
   double r_cap, r_esc;              // r_H (1 + eps_capture), r_escape
   double disk_r_in, disk_r_out;
   gp_ray_record *rays;

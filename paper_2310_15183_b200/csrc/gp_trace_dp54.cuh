@@ -239,11 +239,11 @@ trace_dp54(const __grid_constant__ TraceParams P) {
 
       // stop tests in the oracle's order (R18, R10 item 5), then the monitors of the new state (R22)
       if (mode == MODE_NORMAL) {
-        if ((long long)n_acc + (long long)n_rej >= P.max_steps ||
-            (P.lambda_max > 0.0 && lam >= P.lambda_max)) {
+        // max_steps <= 5e8 (validated by the host) fits the 32-bit counters; lambda_max is +inf when off
+        if (n_acc + n_rej >= (unsigned)P.max_steps || lam >= P.lambda_max) {
           status = GP_RAY_MAXSTEPS;
           finished = true;
-        } else if (h < dp.h_floor * dmax(1.0, fabs(lam))) {
+        } else if (h < dp.h_floor || h < dp.h_floor * fabs(lam)) {   // h < h_floor max(1, |lambda|)
           status = GP_RAY_STEP_UNDERFLOW;
           finished = true;
         } else if (moved) {

@@ -66,7 +66,7 @@ __global__ void __launch_bounds__(kBlock) trace_rk4(const __grid_constant__ Trac
       bool finished = false;
       // stop tests at the top of every ordinary step (R18)
       if (mode == MODE_NORMAL &&
-          ((long long)n_acc >= P.max_steps || (P.lambda_max > 0.0 && (double)lam >= P.lambda_max))) {
+          (n_acc >= (unsigned)P.max_steps || (double)lam >= P.lambda_max)) {
         status = GP_RAY_MAXSTEPS;
         finished = true;
       }

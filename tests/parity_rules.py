@@ -129,7 +129,9 @@ def check_h_drift(rays, orc, smooth, adaptive, label=""):
     if not esc.any():
         return
     gh, oh = rays["h_max"][esc], orc["h_max"][esc]
-    assert (np.abs(gh - oh) <= 1e-11 + 0.25 * np.maximum(gh, oh)).all(), f"{label}: |H| drift differs"
+    bad = np.abs(gh - oh) > 1e-11 + 0.25 * np.maximum(gh, oh)
+    assert not bad.any(), (f"{label}: |H| drift differs on {bad.sum()} of {bad.size} rays, e.g. CUDA "
+                           f"{gh[bad][:3]} against oracle {oh[bad][:3]}")
     assert (gh <= 1.5 * oh + 1e-11).all(), f"{label}: the CUDA path drifts more than the oracle"
     if adaptive:
         assert (gh <= 1e-8).mean() >= 0.998, f"{label}: GPU |H| drift above 1e-8 on {(gh > 1e-8).sum()} rays"
