@@ -323,8 +323,8 @@ def run_b200(args):
                      "achieved": achieved, "peak": peak_nominal, "unit": "TFLOP/s",
                      "frac": achieved / peak_nominal,
                      # dram__bytes_read.sum + dram__bytes_write.sum of one headline launch, from the
-                     # ncu --set full capture summarised in profiles/trace_dp54_r01c.md
-                     "traffic": 8.29e7 if args.workload == "headline" else None,
+                     # ncu --set full capture summarised in profiles/trace_dp54_r01f.md
+                     "traffic": 8.32e7 if args.workload == "headline" else None,
                      "peak_kind": f"nominal {'FP32' if fp32 else 'FP64'} FMA: {props.multi_processor_count} SMs x "
                                   f"{lanes} lanes x 2 x {sm_max:.0f} MHz",
                      "peak_probe": None if fp32 else peak_probe,
