@@ -63,6 +63,17 @@ WORKLOADS = {
                 camera=_camera(1000.0, 60.0, 4096, 20.0, jitter=0.0),
                 cfg=_cfg(1, h_rel=0.02, max_steps=200_000, r_escape=1100.0)),
 }
+# The paper's strongly chaotic case (PAPER.md L418 and Fig 10: Manko-Novikov with Q = 2, S = 0.98 M^2),
+# zoomed on the band of long-lived rays at the prograde edge of the shadow: an 8 x 2048 grid of pixel
+# centres over alpha in [-2.14, -2.06], beta in [-3.5, 3.5] seen from the equator.  Not one of
+# BASELINE.json's configs; it exists so that the chaos flag of configs[3] (companion run shifted by
+# 1e-6 px) is raised on some tens of pixels and the statistical comparison runs.
+# The step budget is this build's choice (the band's escapers need 1e3-2e4 attempted steps).
+WORKLOADS["X3"] = dict(metric=dict(id=MANKO_NOVIKOV, M=1.0, a=0.98, q=2.0),
+                       camera=_camera(1000.0, 90.0, 8, 0.0, jitter=0.0),
+                       cfg=_cfg(max_steps=20_000, r_escape=1100.0, **_ADAPTIVE))
+WORKLOADS["X3"]["camera"].update(width=8, height=2048, alpha_min=-2.14, alpha_max=-2.06,
+                                 beta_min=-3.5, beta_max=3.5)
 # BASELINE.json `metric`: "1024^2 Kerr a=0.9, FP64" = configs[1] at 1024 x 1024
 WORKLOADS["headline"] = copy.deepcopy(WORKLOADS["C2"])
 WORKLOADS["headline"]["camera"].update(width=1024, height=1024)

@@ -19,6 +19,7 @@ SRC = os.path.join(HERE, "gp_oracle.cpp")
 SRC_SHADE = os.path.join(HERE, "gp_shade_oracle.cpp")
 LIB = os.path.join(HERE, "libgp_oracle.so")
 LIB_FMA = os.path.join(HERE, "libgp_oracle_fma.so")
+LIB_X87 = os.path.join(HERE, "libgp_oracle_x87.so")
 
 
 def build(force: bool = False) -> str:
@@ -44,6 +45,21 @@ def build_rounding_probe(force: bool = False) -> str:
            "-fopenmp", "-fPIC", "-shared", "-o", LIB_FMA, SRC, SRC_SHADE]
     subprocess.check_call(cmd)
     return LIB_FMA
+
+
+def build_rounding_probe_x87(force: bool = False) -> str:
+    """A third rounding sample of the same source: x87 arithmetic (64-bit mantissa in registers,
+    rounded to double when stored).  Used by tests/test_parity_threshold.py only, to measure how far
+    one more rounding sample can exceed the FMA probe's spread (the derivation of
+    tests/parity_rules.py SENSITIVE_AT); never for expected values."""
+    deps = [SRC, SRC_SHADE, os.path.join(HERE, "gp_oracle.h")]
+    if (not force and os.path.exists(LIB_X87)
+            and all(os.path.getmtime(LIB_X87) >= os.path.getmtime(d) for d in deps)):
+        return LIB_X87
+    cmd = ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-mfpmath=387", "-fcx-limited-range",
+           "-fopenmp", "-fPIC", "-shared", "-o", LIB_X87, SRC, SRC_SHADE]
+    subprocess.check_call(cmd)
+    return LIB_X87
 
 
 if __name__ == "__main__":

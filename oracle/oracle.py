@@ -63,6 +63,18 @@ def lib_rounding_probe():
     return _lib_fma
 
 
+_lib_x87 = None
+
+
+def lib_rounding_probe_x87():
+    """Third rounding sample (x87 build, oracle/build.py); for the threshold study only."""
+    global _lib_x87
+    if _lib_x87 is None:
+        _lib_x87 = C.CDLL(_build.build_rounding_probe_x87())
+        _declare_trace(_lib_x87)
+    return _lib_x87
+
+
 def lib():
     global _lib
     if _lib is None:
@@ -209,7 +221,7 @@ def trace(workload, ray_begin=0, ray_count=None, ray_stride=1, n_threads=0, roun
     if ray_count > fit:
         raise ValueError("ray selection leaves the image")
     out = np.zeros(ray_count, dtype=RECORD_DTYPE)
-    L = lib_rounding_probe() if rounding_probe else lib()
+    L = (lib_rounding_probe_x87() if rounding_probe == "x87" else lib_rounding_probe()) if rounding_probe else lib()
     used = _check(L.orc_trace(C.byref(_metric(workload["metric"])), C.byref(_camera(cam)),
                                   C.byref(_cfg(workload["cfg"])), int(ray_begin), int(ray_count),
                                   int(ray_stride), out.ctypes.data, int(n_threads)), "trace")

@@ -2,32 +2,48 @@
 
 BASELINE.json north_star: status bit-exact outside flagged regions; raw exit (theta, phi, lambda, t)
 within 1e-9 max(1, |value|) on smooth pixels.  A ray is *smooth* unless one of the flags below is
-set.  Every flag is computed from the oracle (and, for the controller margin, from both sides'
-own records), never from the GPU-oracle difference it then excuses:
+set.  Every flag is computed from the ORACLE's records alone (the oracle build and its two
+rounding variants), never from the CUDA path's records and never from the difference it excuses:
 
-  marginal   min over both sides of err_margin = min_steps |err - 1| < 1e-5: an accept/reject
-             decision of the step controller sat within rounding of its threshold (R30);
+  marginal   the oracle's err_margin = min_steps |err - 1| < 1e-5: an accept/reject decision of the
+             step controller sat within rounding of its threshold (R30).  Rays where only the CUDA
+             path's own margin is that small are counted (`gpu_only_marginal`) and excuse nothing;
   near_axis  sin(theta)_min < 1e-3 along the oracle's ray: the 1/sin^2(theta) terms amplify
              rounding (PAPER.md L723: "the simulation breaks at the axis");
-  sensitive  the oracle disagrees WITH ITSELF by more than 3e-11 (a thirtieth of the tolerance: the
-             probe is one sample of the rounding noise, and over 1e4-1e5 rays a second sample — the GPU —
-             exceeds ten times the first now and then; measured 1.47e-9 on 1 of 9362 rays at 1e-10) when
-             nothing changes but the rounding of its arithmetic: the same source built with FMA
-             contraction (oracle/build.py build_rounding_probe).  Two correct FP64 evaluations of
-             the same algorithm cannot be asked to agree more closely than that.  This catches the
+  sensitive  the oracle disagrees WITH ITSELF by more than SENSITIVE_AT when nothing changes but the
+             rounding of its arithmetic: the same source built with FMA contraction
+             (oracle/build.py build_rounding_probe).  Two correct FP64 evaluations of the same
+             algorithm cannot be asked to agree more closely than that.  This catches the
              near-critical rays (rounding amplified by e^{orbits}), Manko-Novikov rays that graze the
              ill-conditioned neighbourhood of the singular ring, and every fixed-step ray whose
              stages straddle the horizon.
 
+SENSITIVE_AT = TOL / 30 is FROZEN.  Derivation (DESIGN.md section 5, "the sensitivity threshold";
+reproduced by tests/test_parity_threshold.py from the oracle alone, no GPU): the FMA probe is ONE
+sample of a ray's rounding noise and the CUDA path is another, so what matters is how far a second
+sample can exceed the first.  Over the 262 144 rays of config C2 a third build of the oracle
+(x87 extended intermediates) was compared with the first two: among the 4231 rays with a
+measurable spread the ratio (third sample) / (FMA spread) exceeds 3 on 3.4 %, 10 on 0.14 %, 30 on
+0.02 % of them and never 100.  Summing P(ratio > TOL / spread) over the unflagged rays gives the
+expected number of rays that a further rounding sample moves past TOL per full C2 image: 0.018 at
+TOL / 3, 0.007 at TOL / 10, 0.003 at TOL / 30 (213 rays lie within a factor 30 below that last
+threshold, 14 above it).  The oracle's variants share one formulation, though, while the CUDA path
+evaluates a different arrangement of the same formulas, and the one smooth ray it ever moved past
+TOL (1.47e-9, Manko-Novikov, first GPU run of round 1) had a spread between TOL / 30 and TOL / 10.
+TOL / 30 is the largest of the round fractions 1/3, 1/10, 1/30 that covers both; it is not to be
+changed when a test goes red.
+
 Flagged rays are still compared: status must agree unless marginal or sensitive, and the exit
 state must agree to max(1e-6, 100 x the oracle's own rounding spread).  Callers bound the
-flagged fraction.
+flagged fraction, and every call prints how many rays each flag covered and how many comparisons
+each one actually excused (`excused_*` in the summary).
 """
 import numpy as np
 
 TOL = 1e-9
 FLAGGED_TOL = 1e-6
-SENSITIVE_AT = 3e-11
+SENSITIVE_AT = TOL / 30.0     # frozen; derivation in the module docstring and DESIGN.md section 5
+MARGINAL_AT = 1e-5
 FIELDS = ("theta", "phi", "lambda", "t")
 
 
@@ -49,66 +65,113 @@ def rounding_spread(orc, orc_probe):
     return d
 
 
-def flags(rays, orc, orc_probe):
+def flags(orc, orc_probe):
+    """Flags of the module docstring, from the oracle's records and its rounding probe ONLY."""
     spread = rounding_spread(orc, orc_probe)
-    return dict(marginal=np.minimum(orc["err_margin"], rays["err_margin"]) < 1e-5,
+    return dict(marginal=orc["err_margin"] < MARGINAL_AT,
                 near_axis=orc["sin_theta_min"] < 1e-3,
                 sensitive=spread > SENSITIVE_AT,
                 spread=spread)
 
 
 def check_parity(rays, orc, orc_probe, tol=TOL, label="", max_flagged_fraction=0.02,
-                 manko_novikov=False):
+                 manko_novikov=False, max_shadow_code_fraction=0.005, smooth_outlier_fraction=0.0):
     """Element-by-element comparison under the rules above; returns summary numbers.
-    manko_novikov=True: a CAPTURED ray's exit state is compared by status only (R24): the
-    capture surface x = 1 + eps hugs the singular horizon of PAPER.md L234, where fixed-step
-    rays wind phi by 1e6 rad with |H| ~ 1e6 on both sides alike — there is no exit state to pin."""
-    fl = flags(rays, orc, orc_probe)
+    manko_novikov=True changes two things.  (R38) a status mismatch between two "not escaped" codes
+    (CAPTURED at x = 1 + eps against MAXSTEPS after stalling just above it) is counted in
+    `shadow_code_differs` and bounded by max_shadow_code_fraction instead of failing.  (R24) the exit
+    state of a Manko-Novikov CAPTURED ray is compared like any other when it is smooth (1e-9); a
+    CAPTURED ray that the oracle's own rounding probe flags is compared by status only — the
+    capture surface x = 1 + eps hugs the singular horizon of PAPER.md L234, where fixed-step rays wind
+    phi by 1e6 rad with |H| ~ 1e6 on both sides alike and the probe's spread is itself one draw from
+    a distribution as wide as the values (measured: 1.6e4 rad against a probe spread of 1e2).
+    smooth_outlier_fraction > 0 (workload X3 only, the chaotic band): that fraction of the smooth rays
+    may miss `tol` if they stay within FLAGGED_TOL, and flagged rays are compared by status only;
+    tests/test_parity_threshold.py shows on the oracle alone that a third rounding sample moves the
+    same fraction of that band's probe-smooth rays (there one rounding sample does not predict the next)."""
+    fl = flags(orc, orc_probe)
     gs, os_ = rays["status"].astype(np.int64), orc["status"]
     mism = gs != os_
     shadow_code_differs = 0
     if manko_novikov:
-        # R24: what is compared bit for bit is the classification escaped / not escaped.  Which of the
-        # "not escaped" codes a shadow ray ends with (CAPTURED at x = 1 + eps, or MAXSTEPS after stalling
-        # just above it) depends on how e^{2 gamma} rho^2 is evaluated as x -> 1: the oracle's literal
-        # form (eq 28 with the 1/2 ln term of eq 33) cancels there and its error estimate turns to noise
-        # (measured at 80 degrees: ~830 rejected steps, stall at r = 1.4406 against r_cap = 1.43733),
-        # the kernel's log-free form reaches the surface.  The paper counts both as shadow (P:L404).
+        # R38: what is compared bit for bit is the classification escaped / not escaped.  Which of the
+        # "not escaped" codes a shadow ray ends with depends on how e^{2 gamma} rho^2 is evaluated as
+        # x -> 1: the oracle's literal form (eq 28 with the 1/2 ln term of eq 33) cancels there and its
+        # error estimate turns to noise (tests/test_oracle_mn_mpmath.py measures where), the kernel's
+        # log-free form reaches the surface.  The paper counts both as shadow (P:L404).
         both_shadow = (gs != 0) & (os_ != 0)
         shadow_code_differs = int((mism & both_shadow).sum())
         mism = mism & ~both_shadow
+        assert shadow_code_differs <= max_shadow_code_fraction * len(orc) + 1, (
+            f"{label}: {shadow_code_differs} of {len(orc)} shadow rays end CAPTURED on one side and "
+            f"MAXSTEPS on the other")
     excused = fl["marginal"] | fl["sensitive"]
     assert not (mism & ~excused).any(), (
         f"{label}: status differs on {np.count_nonzero(mism & ~excused)} unflagged rays "
         f"(first at {np.flatnonzero(mism & ~excused)[:5]})")
     # the exit state is defined (and unique) for escaped and captured rays; MAXSTEPS rays: status only (R21)
-    ended = ~mism & ((os_ == 0) if manko_novikov else (os_ <= 1))
+    ended = (gs == os_) & (os_ <= 1)
     flagged = fl["marginal"] | fl["near_axis"] | fl["sensitive"]
     smooth = ended & ~flagged
     loose = np.maximum(FLAGGED_TOL, 100.0 * fl["spread"])
     out = {}
+    past_tol = np.zeros(len(orc), dtype=bool)
+    smooth_outliers = np.zeros(len(orc), dtype=bool)
+    loosely = ended & flagged & np.isfinite(loose)
+    if manko_novikov:
+        loosely &= os_ == 0            # R24: flagged CAPTURED rays by status only
+    if smooth_outlier_fraction > 0.0:
+        loosely &= False               # chaotic band: flagged rays by status only (R21)
     for f in FIELDS:
         e = rel_err(rays[f], orc[f])
         out[f] = float(e[smooth].max()) if smooth.any() else 0.0
         bad = smooth & ~(e <= tol)
+        if smooth_outlier_fraction > 0.0:
+            smooth_outliers |= bad
+            bad = smooth & ~(e <= FLAGGED_TOL)
         assert not bad.any(), (f"{label}: {f} off by {e[bad].max():.3e} on {bad.sum()} smooth rays, "
                                f"first {np.flatnonzero(bad)[:5]}")
-        badf = ended & flagged & np.isfinite(loose) & ~(e <= loose)
+        badf = loosely & ~(e <= loose)
         assert not badf.any(), (f"{label}: {f} off by {e[badf].max():.3e} on {badf.sum()} flagged rays, "
                                 f"first {np.flatnonzero(badf)[:5]}")
+        past_tol |= ended & flagged & ~(e <= tol)
     # exact on the exit surface; the constants of the ray to rounding
     on_surface = (gs == os_) & (os_ <= 1)
     assert np.array_equal(rays["r"][on_surface], orc["r"][on_surface]), f"{label}: exit radius is not the surface"
     for f in ("p_t", "p_phi"):
         assert rel_err(rays[f], orc[f]).max() <= 1e-13, f
-    # step counters agree on smooth rays (a differing count is a differing controller decision)
+    assert smooth_outliers.sum() <= smooth_outlier_fraction * max(1, smooth.sum()), (
+        f"{label}: {smooth_outliers.sum()} of {smooth.sum()} smooth rays beyond {tol:g}")
+    # Step counters on smooth rays.  A differing count is a differing accept / reject decision whose
+    # effect on the exit state stayed below the tolerance (the solution is converged to ~1e-10, so two
+    # step sequences agree to that).  Closed-form metrics: err carries ~1e-6 of rounding (it is a
+    # cancellation to 1e-10 of terms known to 1e-16) and MARGINAL_AT = 1e-5 covers every flip: at most
+    # 1e-4 of the smooth rays, or one ray of a small sample.  Manko-Novikov: the dual-number RHS through
+    # exp and sqrt is good to ~1e-13, err to ~1e-4, so decisions with |err - 1| up to 1e-4 flip without
+    # the oracle's margin saying so: up to 2 % of the smooth rays; the count is reported.
+    counts_differ = 0
+    allow = 0.02 if manko_novikov else 1e-4
     for f in ("n_accepted", "n_rejected", "n_equator_crossings", "n_disk_recorded", "n_rhs"):
         d = rays[f][smooth].astype(np.int64) != orc[f][smooth]
-        assert (d.mean() <= 1e-4) if d.size else True, f"{label}: {f} differs on {d.sum()} smooth rays"
+        counts_differ = max(counts_differ, int(d.sum()))
+        if smooth_outlier_fraction == 0.0:
+            assert d.sum() <= max(1.0, allow * d.size), f"{label}: {f} differs on {d.sum()} of {d.size} smooth rays"
     n = max(1, len(orc))
-    out.update(n=len(orc), smooth=int(smooth.sum()), marginal=int(fl["marginal"].sum()),
-               near_axis=int(fl["near_axis"].sum()), sensitive=int(fl["sensitive"].sum()),
+    only_gpu_marginal = (rays["err_margin"] < MARGINAL_AT) & ~fl["marginal"]
+    out.update(n=len(orc), ended=int(ended.sum()), smooth=int(smooth.sum()),
+               smooth_captured=int((smooth & (os_ == 1)).sum()),
+               marginal=int(fl["marginal"].sum()), near_axis=int(fl["near_axis"].sum()),
+               sensitive=int(fl["sensitive"].sum()), gpu_only_marginal=int(only_gpu_marginal.sum()),
                status_mismatch=int(mism.sum()), shadow_code_differs=shadow_code_differs,
+               step_counts_differ_on_smooth=counts_differ, smooth_outliers=int(smooth_outliers.sum()),
+               flagged_captured_by_status_only=int((ended & flagged & (os_ == 1)).sum()) if manko_novikov else 0,
+               # what the flags actually excused: status mismatches let through, and ended rays whose exit
+               # state is past TOL (but inside the loose bound), by the flag that covers them
+               excused_status=int((mism & excused).sum()),
+               excused_exit_marginal=int((past_tol & fl["marginal"]).sum()),
+               excused_exit_near_axis=int((past_tol & fl["near_axis"]).sum()),
+               excused_exit_sensitive=int((past_tol & fl["sensitive"]).sum()),
+               uncompared_probe_status_differs=int((ended & ~np.isfinite(fl["spread"])).sum()),
                flagged_fraction=float(flagged.sum()) / n)
     assert out["flagged_fraction"] <= max_flagged_fraction, (
         f"{label}: {flagged.sum()} of {len(orc)} rays flagged — the flags must stay the exception")
@@ -116,7 +179,27 @@ def check_parity(rays, orc, orc_probe, tol=TOL, label="", max_flagged_fraction=0
     return out
 
 
-def check_h_drift(rays, orc, smooth, adaptive, label=""):
+def same_step_sequence(rays, orc):
+    """Rays on which both sides took the same number of accepted and rejected steps: the monitors
+    (running maxima / minima over the discrete step end points) sample the same points there."""
+    return ((rays["n_accepted"].astype(np.int64) == orc["n_accepted"])
+            & (rays["n_rejected"].astype(np.int64) == orc["n_rejected"]))
+
+
+def chaos_flags(orc, companion):
+    """BASELINE.json configs[3] / reading R21: a pixel is chaotic when the ORACLE's companion run,
+    shifted by (1e-6, 1e-6) px, ends in the other class (escaped / not escaped: for Manko-Novikov every
+    "not escaped" code is shadow, R38) or, both escaped, leaves in a direction more than 1 rad away."""
+    def unit(rec):
+        return np.stack([np.sin(rec["theta"]) * np.cos(rec["phi"]), np.sin(rec["theta"]) * np.sin(rec["phi"]),
+                         np.cos(rec["theta"])], 1)
+    ea, eb = orc["status"] == 0, companion["status"] == 0
+    with np.errstate(invalid="ignore"):
+        ang = np.arccos(np.clip((unit(orc) * unit(companion)).sum(1), -1.0, 1.0))
+    return (ea != eb) | (ea & eb & (ang > 1.0))
+
+
+def check_h_drift(rays, orc, smooth, adaptive, label="", manko_novikov=False):
     """|H| drift (R22) on smooth escaped rays.  The two sides must report the same drift
     (1e-11 + 25 %: the running maximum is itself a rounding-level cancellation, and the oracle's
     own FMA build moves it by up to 14 %), the CUDA path may not drift more than 1.5 x the oracle,
@@ -128,11 +211,18 @@ def check_h_drift(rays, orc, smooth, adaptive, label=""):
     esc = smooth & (orc["status"] == 0) & (rays["status"] == 0)
     if not esc.any():
         return
-    gh, oh = rays["h_max"][esc], orc["h_max"][esc]
+    # the running maximum is taken over the step end points: it is compared where both sides stepped
+    # through the same sequence (same_step_sequence); elsewhere only the bound below applies
+    same = esc & same_step_sequence(rays, orc)
+    gh, oh = rays["h_max"][same], orc["h_max"][same]
     bad = np.abs(gh - oh) > 1e-11 + 0.25 * np.maximum(gh, oh)
-    assert not bad.any(), (f"{label}: |H| drift differs on {bad.sum()} of {bad.size} rays, e.g. CUDA "
-                           f"{gh[bad][:3]} against oracle {oh[bad][:3]}")
-    assert (gh <= 1.5 * oh + 1e-11).all(), f"{label}: the CUDA path drifts more than the oracle"
+    # Manko-Novikov: equal counts do not prove equal sequences (a rejection at another step, see the
+    # counter rule in check_parity), so 1 % of those rays may sample other points
+    allow = 0.01 * bad.size if manko_novikov else 0.0
+    assert bad.sum() <= allow, (f"{label}: |H| drift differs on {bad.sum()} of {bad.size} rays, e.g. CUDA "
+                                f"{gh[bad][:3]} against oracle {oh[bad][:3]}")
+    assert ((gh > 1.5 * oh + 1e-11).sum() <= allow), f"{label}: the CUDA path drifts more than the oracle"
+    gh, oh = rays["h_max"][esc], orc["h_max"][esc]
     if adaptive:
         assert (gh <= 1e-8).mean() >= 0.998, f"{label}: GPU |H| drift above 1e-8 on {(gh > 1e-8).sum()} rays"
         assert (oh <= 1e-8).mean() >= 0.998, f"{label}: oracle |H| drift above 1e-8 on {(oh > 1e-8).sum()} rays"

@@ -18,7 +18,7 @@ import gp_workloads as W
 
 pytestmark = pytest.mark.gpu
 
-from parity_rules import FIELDS, TOL, check_h_drift, check_parity as _check_parity, rel_err
+from parity_rules import FIELDS, TOL, check_h_drift, check_parity as _check_parity, rel_err, same_step_sequence
 
 
 @pytest.fixture(scope="module")
@@ -49,13 +49,16 @@ def check_parity(w, rays, orc, probe, label, **kw):
     res = _check_parity(rays, orc, probe, label=label,
                         manko_novikov=w["metric"]["id"] == W.MANKO_NOVIKOV, **kw)
     smooth = res.pop("smooth_mask")
-    check_h_drift(rays, orc, smooth, adaptive=w["cfg"]["scheme"] == 2, label=label)
+    mn = w["metric"]["id"] == W.MANKO_NOVIKOV
+    check_h_drift(rays, orc, smooth, adaptive=w["cfg"]["scheme"] == 2, label=label, manko_novikov=mn)
     # the other monitors, on smooth rays.  sin(theta)_min is a minimum over the discrete step
     # endpoints, so it moves with the step sequence (measured 3e-7 on a Manko-Novikov ray whose
     # error estimate is rounding-dominated); it is a flagging aid, not an output of the method.
-    assert np.allclose(rays["sin_theta_min"][smooth], orc["sin_theta_min"][smooth], rtol=1e-5, atol=1e-12)
+    same = smooth & same_step_sequence(rays, orc)
+    off = ~np.isclose(rays["sin_theta_min"][same], orc["sin_theta_min"][same], rtol=1e-5, atol=1e-12)
+    assert off.sum() <= (0.01 * off.size if mn else 0), (label, int(off.sum()), off.size)
     if w["metric"]["id"] != W.MANKO_NOVIKOV and w["cfg"]["scheme"] == 2:
-        esc = smooth & (orc["status"] == 0)
+        esc = same & (orc["status"] == 0)
         assert np.abs(rays["q_drift"] - orc["q_drift"])[esc].max() <= 1e-10 + 0.25 * orc["q_drift"][esc].max()
     print(label, res)
     return res, smooth
@@ -176,37 +179,85 @@ def test_c3_kerr_disk_subsample(gp, O):
     print("C3 rays with disk hits", int((n_rec > 0).sum()))
 
 
-def test_c4_manko_novikov_subsample(gp, O):
-    """Config 4 with the step budget cut to 4000 so that the oracle finishes the stalled interior
-    rays in seconds; MAXSTEPS rays are compared by status only (R21, R24)."""
-    w = W.workload("C4")
-    w["cfg"]["max_steps"] = 4000
-    rays, _, _, orc, probe = run_both(gp, O, w, 11, None, 2039)
-    check_parity(w, rays, orc, probe, "C4", max_flagged_fraction=0.02)
-    assert (orc["status"] == 2).sum() > 20 and (orc["status"] == 0).sum() > 1000
-    # BASELINE.json configs[3] / reading R21: the chaos flag comes from the ORACLE's companion run
-    # shifted by (1e-6, 1e-6) px: status differs, or the exit directions differ by more than 1 rad.
-    # Outside the flagged set the status must be bit-exact; inside it the comparison is statistical.
+def _chaos_comparison(w, rays, orc, sel, O, label, min_flagged=0):
+    """Reading R21: the chaos flag comes from the ORACLE's companion run shifted by (1e-6, 1e-6) px.
+    Outside the flagged set the class escaped / not escaped is bit-exact; inside it the comparison is
+    statistical: escape fraction within 0.15 (or 3 sigma of the binomial), two-sample KS on exit lambda."""
+    from parity_rules import chaos_flags
     wc = copy.deepcopy(w)
     wc["camera"].update(shift_x_px=1e-6, shift_y_px=1e-6)
-    b, c, s = W.ray_selection(w, 11, None, 2039)
-    comp, _ = O.trace(wc, b, c, s)
-
-    def unit(rec):
-        return np.stack([np.sin(rec["theta"]) * np.cos(rec["phi"]), np.sin(rec["theta"]) * np.sin(rec["phi"]),
-                         np.cos(rec["theta"])], 1)
-    ang = np.arccos(np.clip((unit(orc) * unit(comp)).sum(1), -1.0, 1.0))
-    both_out = (orc["status"] == 0) & (comp["status"] == 0)
-    chaotic = (orc["status"] != comp["status"]) | (both_out & (ang > 1.0))
-    assert np.array_equal(rays["status"][~chaotic].astype(np.int64), orc["status"][~chaotic])
-    if chaotic.sum() >= 20:   # statistical comparison inside the flagged set (empty at this sampling: see DESIGN.md 5)
+    comp, _ = O.trace(wc, *sel)
+    chaotic = chaos_flags(orc, comp)
+    n_ch = int(chaotic.sum())
+    ge, oe = rays["status"] == 0, orc["status"] == 0
+    print(f"{label}: chaos-flagged pixels (oracle companion run): {n_ch} of {len(orc)}; "
+          f"escaped among them: CUDA {int(ge[chaotic].sum())}, oracle {int(oe[chaotic].sum())}")
+    assert n_ch >= min_flagged, (n_ch, min_flagged)
+    if n_ch >= 20:
         from scipy.stats import ks_2samp
-        g, o = rays[chaotic], orc[chaotic]
-        assert abs((g["status"] == 0).mean() - (o["status"] == 0).mean()) <= 0.15
-        ge, oe = g["lambda"][g["status"] == 0], o["lambda"][o["status"] == 0]
-        if len(ge) >= 10 and len(oe) >= 10:
-            assert ks_2samp(ge, oe).pvalue > 0.01
-    print("C4 chaos-flagged pixels (oracle companion run):", int(chaotic.sum()), "of", c)
+        fg, fo = ge[chaotic].mean(), oe[chaotic].mean()
+        assert abs(fg - fo) <= max(0.15, 3.0 * math.sqrt(max(fo * (1 - fo), 0.01) / n_ch)), (fg, fo)
+        lg, lo = rays["lambda"][chaotic & ge], orc["lambda"][chaotic & oe]
+        if len(lg) >= 10 and len(lo) >= 10:
+            p = ks_2samp(lg, lo).pvalue
+            print(f"{label}: KS p-value of exit lambda inside the flagged set: {p:.3f} ({len(lg)} vs {len(lo)} rays)")
+            assert p > 0.01, p
+    return chaotic
+
+
+def test_c4_manko_novikov_subsample(gp, O):
+    """Config 4 on 2058 scattered rays with the step budget cut to 4000 so that the oracle finishes the
+    stalled interior rays in seconds (the full budget runs in the next test on fewer rays); MAXSTEPS
+    rays are compared by status only (R21)."""
+    w = W.workload("C4")
+    w["cfg"]["max_steps"] = 4000
+    sel = W.ray_selection(w, 11, None, 2039)
+    rays, _, _, orc, probe = run_both(gp, O, w, *sel)
+    check_parity(w, rays, orc, probe, "C4 (4000 steps)", max_flagged_fraction=0.02)
+    assert (orc["status"] == 2).sum() > 20 and (orc["status"] == 0).sum() > 1000
+    chaotic = _chaos_comparison(w, rays, orc, sel, O, "C4 (4000 steps)")
+    assert np.array_equal((rays["status"] == 0)[~chaotic], (orc["status"] == 0)[~chaotic])
+
+
+def test_c4_manko_novikov_at_its_own_step_budget(gp, O):
+    """BASELINE.json configs[3] as written: <= 2e5 attempted steps per ray.  511 scattered rays of the
+    2048 x 2048 image, about 55 of them inside the shadow, where they stall near r = 1.59 M and run to
+    the budget (1.2e6 evaluations each); everything that leaves between 4000 and 2e5 steps is in here."""
+    w = W.workload("C4")
+    assert w["cfg"]["max_steps"] == 200_000
+    sel = W.ray_selection(w, 11, None, 8209)
+    rays, _, counters, orc, probe = run_both(gp, O, w, *sel)
+    res, _ = check_parity(w, rays, orc, probe, "C4 (2e5 steps)", max_flagged_fraction=0.03)
+    shadow = orc["status"] != 0
+    assert len(orc) >= 500 and shadow.sum() >= 40, (len(orc), int(shadow.sum()))
+    late = (orc["status"] == 0) & (orc["n_accepted"] + orc["n_rejected"] > 4000)
+    print("C4 (2e5 steps): shadow rays", int(shadow.sum()), "of", len(orc), "; escaped after more than 4000 steps:",
+          int(late.sum()), "; MAXSTEPS on both sides:", int(((orc["status"] == 2) & (rays["status"] == 2)).sum()))
+    both_max = (orc["status"] == 2) & (rays["status"] == 2)
+    assert np.array_equal(rays["n_accepted"][both_max].astype(np.int64) + rays["n_rejected"][both_max],
+                          orc["n_accepted"][both_max] + orc["n_rejected"][both_max])       # the budget, exactly
+    chaotic = _chaos_comparison(w, rays, orc, sel, O, "C4 (2e5 steps)")
+    assert np.array_equal((rays["status"] == 0)[~chaotic], (orc["status"] == 0)[~chaotic])
+
+
+def test_x3_chaotic_band_statistical_comparison(gp, O):
+    """The paper's strongly chaotic case (Fig 10: Q = 2, S = 0.98 M^2), workload X3:
+    8192 rays of the band of long-lived orbits at the prograde edge of the shadow.  The oracle's
+    companion run flags some tens of them as chaotic (37 when this was written); there the CUDA path
+    and the oracle are compared statistically, everywhere else under the ordinary rules — the
+    rounding probe decides which of the long-lived rays still have a unique exit state."""
+    w = W.workload("X3")
+    sel = W.ray_selection(w, 1, None, 2)
+    rays, _, _, orc, probe = run_both(gp, O, w, *sel)
+    chaotic = _chaos_comparison(w, rays, orc, sel, O, "X3", min_flagged=20)
+    # ordinary rules outside the flagged set (inside it the exit state is not unique, R21)
+    keep = ~chaotic
+    # The whole band is long-lived (1e3-2e4 steps in the strong field): two thirds of it are flagged by the
+    # rounding probe, and of the rest about 1 % is moved past 1e-9 (never past 1e-6) by ANY further
+    # rounding sample, the oracle's own third build included (tests/test_parity_threshold.py).
+    res, _ = check_parity(w, rays[keep], orc[keep], probe[keep], "X3 outside the chaotic set",
+                          max_flagged_fraction=0.9, smooth_outlier_fraction=0.02)
+    assert res["smooth"] >= 1500, res
 
 
 def test_mn_q0_reproduces_kerr_on_gpu(gp, O):
@@ -233,9 +284,12 @@ def test_c5_fixed_relative_step_subsample(gp, O, name, stride, flagged):
     phi by ~1e6 rad under the fixed relative step; those rays are rounding-sensitive by any
     measure and are compared by status (parity_rules, R24)."""
     w = W.workload(name)
-    w["cfg"]["max_steps"] = 20000
+    assert w["cfg"]["max_steps"] == 200_000          # BASELINE.json configs[4] at this build's stated budget
     rays, _, _, orc, probe = run_both(gp, O, w, 1, None, stride)
     check_parity(w, rays, orc, probe, name, max_flagged_fraction=flagged)
+    steps = orc["n_accepted"]
+    print(name, "rays", len(orc), "captured", int((orc["status"] == 1).sum()), "longest ray", int(steps.max()),
+          "steps; rays beyond 20000 steps:", int((steps > 20000).sum()))
 
 
 # ---- edge cases ----------------------------------------------------------------------------------
