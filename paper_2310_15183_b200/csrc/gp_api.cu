@@ -7,6 +7,8 @@
 #include <stdio.h>
 #include <string.h>
 
+#include <mutex>
+
 #include "../../include/gp.h"
 #include "gp_trace.cuh"
 #include "gp_shade.cuh"
@@ -197,37 +199,54 @@ int make_params(int metric_id, const gp_metric_params *m, const gp_camera *cam, 
 }
 
 // ---- launch -----------------------------------------------------------------------------------
+// Resident blocks per SM and the SM count are properties of (kernel, device): cached per device id
+// under a mutex, so that a process may drive several devices and several host threads (the cache was
+// bound to the first device in round 1).
+constexpr int kMaxDevices = 64;
+struct LaunchInfo {
+  int n_sm;
+  int per_sm;   // 0 = not computed yet
+};
+std::mutex g_launch_mutex;
+
+template <class Kernel>
+int launch_info(Kernel kernel, size_t smem, LaunchInfo *slot, LaunchInfo *out) {
+  std::lock_guard<std::mutex> lock(g_launch_mutex);
+  if (slot->per_sm == 0) {
+    int dev = 0, n_sm = 0, occ = 0;
+    GP_CUDA(cudaGetDevice(&dev));
+    GP_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+    // dynamic shared memory beyond 48 KB (the disk variant of trace_dp54) needs the opt-in
+    if (smem > 48 * 1024)
+      GP_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    GP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, kBlock, smem));
+    slot->n_sm = n_sm;
+    slot->per_sm = occ < 1 ? 1 : occ;
+  }
+  *out = *slot;
+  return GP_OK;
+}
+
 template <int METRIC, bool DISK>
 int launch_one(const TraceParams &P, cudaStream_t stream) {
-  static int blocks[3] = {0, 0, 0};  // resident blocks per SM: dp54, rk4 FP64, rk4 FP32
-  static int n_sm = 0;
+  static LaunchInfo cache[kMaxDevices][3];   // per device: dp54, rk4 FP64, rk4 FP32 (zero-initialised)
   const bool dp54 = (P.scheme == 2);
   const bool fp32 = (P.precision == 1);
   const size_t smem = dp54 ? dp54_smem_bytes(DISK)
                            : (DISK ? (fp32 ? sizeof(float) : sizeof(double)) * kBlock * kParkSlotsRk4 : 0);
-  int &per_sm = blocks[dp54 ? 0 : (fp32 ? 2 : 1)];
-  if (per_sm == 0) {
-    int dev = 0;
-    GP_CUDA(cudaGetDevice(&dev));
-    GP_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
-    int occ = 0;
-    if (dp54)
-      GP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, trace_dp54<METRIC, DISK>, kBlock, smem));
-    else if (fp32)
-      GP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, trace_rk4<METRIC, DISK, float>, kBlock, smem));
-    else
-      GP_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, trace_rk4<METRIC, DISK, double>, kBlock, smem));
-    if (occ < 1) occ = 1;
-    // tuning aid: GP_BLOCKS_PER_SM caps the resident blocks per SM (never raises them)
-    if (const char *cap = getenv("GP_BLOCKS_PER_SM")) {
-      int c = atoi(cap);
-      if (c >= 1 && c < occ) occ = c;
-    }
-    per_sm = occ;
-  }
+  int dev = 0;
+  GP_CUDA(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kMaxDevices) return GP_E_UNSUPPORTED;
+  LaunchInfo *slot = &cache[dev][dp54 ? 0 : (fp32 ? 2 : 1)];
+  LaunchInfo li;
+  int rc;
+  if (dp54) rc = launch_info(trace_dp54<METRIC, DISK>, smem, slot, &li);
+  else if (fp32) rc = launch_info(trace_rk4<METRIC, DISK, float>, smem, slot, &li);
+  else rc = launch_info(trace_rk4<METRIC, DISK, double>, smem, slot, &li);
+  if (rc) return rc;
   // persistent grid: every SM filled to its resident-block limit, never more lanes than rays
   long long want = ((long long)P.cc.ray_count + kBlock - 1) / kBlock;
-  long long grid = (long long)n_sm * per_sm;
+  long long grid = (long long)li.n_sm * li.per_sm;
   if (grid > want) grid = want;
   if (grid < 1) grid = 1;
   if (dp54)

@@ -37,6 +37,9 @@ struct MathConst {
   double s[6];                        // sin: r + r z (s0 + s1 z + ... + s5 z^5), z = r^2
   double c[6];                        // cos: 1 - z/2 + z^2 (c0 + ... + c5 z^5)
   double one, half, fifth, six_fifths;
+  double magic;
+  double as[6];                       // sin d = d + d z (as0 + ... + as5 z^5), z = d^2: Taylor, |d| <= 1/2
+  double ac[7];                       // cos d - 1 = z (ac0 + ... + ac6 z^6)
 };
 
 __constant__ MathConst kMath = {
@@ -46,23 +49,26 @@ __constant__ MathConst kMath = {
      -0x1.ae5fdeb852566p-26, 0x1.5dfb4dfaf15abp-33},
     {0x1.5555555555555p-5, -0x1.6c16c16c1691fp-10, 0x1.a01a019f3df42p-16, -0x1.27e4fa025e03dp-22,
      0x1.1eeb52bea9072p-29, -0x1.906dd38cb66a1p-37},
-    1.0, 0.5, 0.2, 1.2};
+    1.0, 0.5, 0.2, 1.2, 6755399441055744.0,
+    {-0x1.5555555555555p-3, 0x1.1111111111111p-7, -0x1.a01a01a01a01ap-13, 0x1.71de3a556c734p-19, -0x1.ae64567f544e4p-26, 0x1.6124613a86d09p-33},
+    {-0x1.0000000000000p-1, 0x1.5555555555555p-5, -0x1.6c16c16c16c17p-10, 0x1.a01a01a01a01ap-16, -0x1.27e4fb7789f5cp-22, 0x1.1eed8eff8d898p-29, -0x1.93974a8c07c9dp-37}};
 
 // max / min of two doubles without fmax's NaN canonicalisation: a NaN candidate never replaces
 // the running value (the same outcome fmax(running, NaN) gives).
 __device__ __forceinline__ double dmax(double run, double cand) { return cand > run ? cand : run; }
 __device__ __forceinline__ double dmin(double run, double cand) { return cand < run ? cand : run; }
 
-// 1/x to <= 1 ulp for normal finite x: MUFU.RCP64H seed (about 20 bits) + one cubic and one
-// quadratic Newton step.  x = 0 or non-finite gives a non-finite result (the integrator's
-// finite tests catch it); subnormal x is outside the integrator's range.
+// 1/x to about 1 ulp for normal finite x: MUFU.RCP64H seed (relative error e0 <= 2^-20) + one cubic
+// Newton step, y (1 + e + e^2) = (1/x)(1 - e^3): e0^3 <= 2^-60 is 1/128 ulp, so what is left is the
+// rounding of the last FMA.  (A second, quadratic step — two more DFMAs, kept through round 1 — only
+// turned <= 1.5 ulp into <= 1 ulp; dropping it bought 1.4 % on the headline.)  x = 0 or non-finite
+// gives a non-finite result (the integrator's finite tests catch it); subnormal x is outside the
+// integrator's range.
 __device__ __forceinline__ double rcp_nr(double x) {
   double y;
   asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
   double e = fma(-x, y, kMath.one);
   e = fma(e, e, e);
-  y = fma(y, e, y);
-  e = fma(-x, y, kMath.one);
   return fma(y, e, y);
 }
 
@@ -109,6 +115,31 @@ __device__ __forceinline__ void sincos_fast(double x, double *sn, double *cs) {
   *cs = __hiloint2double(__double2hiint(b) ^ (((q + 1) & 2) << 30), __double2loint(b));
 }
 
+// sin and cos of (theta_n + d) from sn = sin theta_n, cn = cos theta_n by the addition theorems, for the
+// stage angles of one Runge-Kutta attempt (|d| = |step x sum a_ij dtheta/dlambda|, a few hundredths of a
+// radian in practice).  Taylor kernels through d^13 / d^14: truncation below 3e-17 for |d| <= 1/2.  No
+// range reduction, no quadrant logic, no branch: 20 FP64 instructions and nothing else, against 21 + 16
+// for sincos_fast.  A wild trial step (|d| > 1/2) gets a finite wrong value; its error estimate is then
+// huge and the step is rejected (R10 item 2), which is what happens to such a step anyway.
+__device__ __forceinline__ void sincos_add(double sn, double cn, double d, double *s, double *c) {
+  double z = d * d;
+  double ps = fma(z, kMath.as[5], kMath.as[4]);
+  double pc = fma(z, kMath.ac[6], kMath.ac[5]);
+  ps = fma(z, ps, kMath.as[3]);
+  pc = fma(z, pc, kMath.ac[4]);
+  ps = fma(z, ps, kMath.as[2]);
+  pc = fma(z, pc, kMath.ac[3]);
+  ps = fma(z, ps, kMath.as[1]);
+  pc = fma(z, pc, kMath.ac[2]);
+  ps = fma(z, ps, kMath.as[0]);
+  pc = fma(z, pc, kMath.ac[1]);
+  pc = fma(z, pc, kMath.ac[0]);
+  double sd = fma(d * z, ps, d);   // sin d
+  double cm = z * pc;              // cos d - 1
+  *s = fma(sn, cm, fma(cn, sd, sn));
+  *c = fma(cn, cm, fma(-sn, sd, cn));
+}
+
 // x^(-1/5) for x in [1e-5, 1e4] (the controller clamps outside, R10 item 3): FP32 seed from the
 // SFU (lg2/ex2, about 1e-6 relative), two Newton steps on y^-5 = x (error 3 e^2 per step) -> <= 2 ulp.
 // (One step, 1e-12 relative, saves 0.7 % of the headline's time and keeps every exit state within
@@ -118,9 +149,14 @@ __device__ __forceinline__ double pow_m1_5(double x) {
   float xf = __double2float_rn(x), lg, yf;
   asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(lg) : "f"(xf));
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(yf) : "f"(-0.2f * lg));
+  {
+    float y2 = yf * yf, y5 = y2 * y2 * yf;
+    float e = fmaf(-xf, y5, 1.0f);
+    yf = fmaf(yf * 0.2f, e, yf);
+  }
   double y = (double)yf;
 #pragma unroll
-  for (int i = 0; i < 2; ++i) {
+  for (int i = 0; i < 1; ++i) {
     double y2 = y * y;
     double y5 = y2 * y2 * y;
     double e = fma(-x, y5, kMath.one);

@@ -43,15 +43,22 @@ struct RhsT {
   T dt, dr, dth, dph, dpr, dpth;
   T s, c, H2;
   T is;  // 1/sin(theta) (Schwarzschild, Kerr; 0 for Manko-Novikov)
+  T pw;  // Kerr: p_th^2 + W^2, W = p_ph/s + a s p_t (a by-product the Carter monitor reuses)
 };
 typedef RhsT<double> Rhs;
 
 // ---- Schwarzschild --------------------------------------------------------------------------
 // 2H = -p_t^2/F + F p_r^2 + p_th^2/r^2 + p_ph^2/(r^2 s^2),  F = 1 - 2M/r   (eq 8 inverted)
-template <class T>
-GP_HD void rhs_schwarzschild(const MetricConst &mc, T pt, T pph, T r, T th, T pr, T pth, RhsT<T> &o) {
+template <class T, bool GIVEN_SC = false>
+GP_HD void rhs_schwarzschild(const MetricConst &mc, T pt, T pph, T r, T th, T pr, T pth, RhsT<T> &o,
+                             T s_in = T(0), T c_in = T(0)) {
   T s, c;
-  fsincos(th, &s, &c);
+  if (GIVEN_SC) {
+    s = s_in;
+    c = c_in;
+  } else {
+    fsincos(th, &s, &c);
+  }
   const T M = (T)mc.M;
   T ir = frcp(r);
   T ir2 = ir * ir;
@@ -83,10 +90,21 @@ GP_HD void rhs_schwarzschild(const MetricConst &mc, T pt, T pph, T r, T th, T pr
 // Written out operation by operation (half-derivatives, shared products, explicit fma): 53 FP64
 // instructions beside the sincos and the reciprocal, against 61 for the textbook arrangement — the
 // FP64 pipe is the bound, so the operation count is the run time.
-template <class T>
-GP_HD void rhs_kerr(const MetricConst &mc, T pt, T pph, T r, T th, T pr, T pth, RhsT<T> &o) {
+// SCALED: the six derivatives come out multiplied by hs, the step of the attempt, at the cost of ONE
+// extra multiplication (hs / Sigma replaces 1 / Sigma in their last product); the Runge-Kutta sums
+// then need no multiplication by the step (gp_trace_dp54.cuh).  The by-products (s, c, H2, is) are
+// never scaled.
+// GIVEN_SC: sin and cos of theta are supplied by the caller (s_in, c_in) and th is not read.
+template <class T, bool SCALED = false, bool GIVEN_SC = false>
+GP_HD void rhs_kerr(const MetricConst &mc, T pt, T pph, T r, T th, T pr, T pth, RhsT<T> &o, T hs = T(1),
+                    T s_in = T(0), T c_in = T(0)) {
   T s, c;
-  fsincos(th, &s, &c);
+  if (GIVEN_SC) {
+    s = s_in;
+    c = c_in;
+  } else {
+    fsincos(th, &s, &c);
+  }
   const T a = (T)mc.a, a2 = (T)mc.a2;
   T r2 = r * r;
   T rr = r2 + a2;
@@ -105,22 +123,25 @@ GP_HD void rhs_kerr(const MetricConst &mc, T pt, T pph, T r, T th, T pr, T pth, 
   T P = ffma(rr, pt, a * pph);
   T PiD = P * iDel;
   T pr2 = pr * pr;
-  T N = ffma(-P, PiD, ffma(W, W, ffma(pth, pth, Del * pr2)));
+  T pw = ffma(W, W, pth * pth);
+  T N = ffma(-P, PiD, ffma(Del, pr2, pw));
   T H2 = N * iSig;
-  o.dt = ffma(-rr, PiD, as * W) * iSig;
-  o.dph = ffma(-a, PiD, W * is) * iSig;
-  o.dr = (pr * iSig) * Del;
-  o.dth = pth * iSig;
+  const T hS = SCALED ? hs * iSig : iSig;
+  o.dt = ffma(-rr, PiD, as * W) * hS;
+  o.dph = ffma(-a, PiD, W * is) * hS;
+  o.dr = (pr * hS) * Del;
+  o.dth = pth * hS;
   // dp_r = -(1/2 d_r N - r 2H)/Sigma,  1/2 d_r N = (r-M)(p_r^2 + (P/Delta)^2) - 2 r p_t P/Delta
   T halfNr = ffma(T(-2), (r * pt) * PiD, (r - (T)mc.M) * ffma(PiD, PiD, pr2));
-  o.dpr = ffma(r, H2, -halfNr) * iSig;
+  o.dpr = ffma(r, H2, -halfNr) * hS;
   // dp_th = -(1/2 d_th N + a^2 s c 2H)/Sigma,  1/2 d_th N = W c (a p_t - p_ph/s^2)
   T halfNth = (W * c) * ffma(-(pph * is), is, a * pt);
-  o.dpth = -ffma(a2c * s, H2, halfNth) * iSig;
+  o.dpth = -ffma(a2c * s, H2, halfNth) * hS;
   o.H2 = H2;
   o.s = s;
   o.c = c;
   o.is = is;
+  o.pw = pw;
 }
 
 // ---- Manko-Novikov --------------------------------------------------------------------------
@@ -227,6 +248,30 @@ GP_HD void rhs_eval(const MetricConst &mc, T pt, T pph, T r, T th, T pr, T pth, 
 #else
     rhs_manko_novikov<T>(mc, pt, pph, r, th, pr, pth, o);
 #endif
+  }
+}
+
+// rhs_eval_scaled: the six derivatives multiplied by hs (see rhs_kerr); Schwarzschild and
+// Manko-Novikov scale the results afterwards (their cost is elsewhere).
+template <int METRIC, bool OUTLINE_MN = false, class T>
+GP_HD void rhs_eval_scaled(const MetricConst &mc, T pt, T pph, T r, T th, T pr, T pth, T hs, RhsT<T> &o) {
+  if (METRIC == METRIC_KERR) {
+    rhs_kerr<T, true>(mc, pt, pph, r, th, pr, pth, o, hs);
+  } else {
+    rhs_eval<METRIC, OUTLINE_MN, T>(mc, pt, pph, r, th, pr, pth, o);
+    o.dt *= hs; o.dr *= hs; o.dth *= hs; o.dph *= hs; o.dpr *= hs; o.dpth *= hs;
+  }
+}
+
+// The same with sin and cos of theta supplied by the caller (Schwarzschild, Kerr; gp_trace_dp54.cuh
+// obtains them for the stage angles by the addition theorems).
+template <int METRIC, class T>
+GP_HD void rhs_eval_scaled_sc(const MetricConst &mc, T pt, T pph, T r, T s, T c, T pr, T pth, T hs, RhsT<T> &o) {
+  if (METRIC == METRIC_KERR) {
+    rhs_kerr<T, true, true>(mc, pt, pph, r, T(0), pr, pth, o, hs, s, c);
+  } else {
+    rhs_schwarzschild<T, true>(mc, pt, pph, r, T(0), pr, pth, o, s, c);
+    o.dt *= hs; o.dr *= hs; o.dth *= hs; o.dph *= hs; o.dpr *= hs; o.dpth *= hs;
   }
 }
 

@@ -245,9 +245,14 @@ __device__ __forceinline__ bool finite_d(float x) { return fabsf(x) <= 3.4028234
 template <int METRIC, class T>
 __device__ __forceinline__ T carter_q(const MetricConst &mc, T pt, T pph, T pth, const RhsT<T> &o) {
   if (METRIC == METRIC_MN) return T(0);
-  const T a2 = (METRIC == METRIC_KERR) ? (T)mc.a2 : T(0);
+  if (METRIC == METRIC_KERR) {
+    // c^2 (p_ph^2/s^2 - a^2 p_t^2) = W^2 - (p_ph + a p_t)^2 with W = p_ph/s + a s p_t, and p_th^2 + W^2 is
+    // a by-product of rhs_kerr: five operations instead of eleven, every step
+    T l = ffma((T)mc.a, pt, pph);
+    return ffma(-((T)mc.a2 * o.c) * o.c, o.H2, o.pw - l * l);
+  }
   T c2 = o.c * o.c;
-  return pth * pth + c2 * (pph * pph * o.is * o.is - a2 * pt * pt) - a2 * c2 * o.H2;
+  return pth * pth + c2 * (pph * pph * o.is * o.is);
 }
 
 template <int METRIC, class T>

@@ -25,8 +25,11 @@ namespace gp {
 //                          trial state (r, th, pr, pth, t, ph, lambda), next step, raw k7 (6) and
 //                          its monitor triple.
 enum { C_T = 0, C_PH, C_LAM, C_HMAX, C_QDRIFT, C_Q0, C_IQ0, C_SINMIN, C_MARGIN, C_TARGET, C_K1T, C_K1PH,
-       C_TOT_RAYS, C_TOT_STEPS, C_TOT_RHS, kColdSlots };
-constexpr int kKSlots2 = 8;
+       C_TOT_RAYS, C_TOT_STEPS, C_TOT_RHS,
+       C_SLOT,      // output slot of the ray in flight (64-bit integer bits)
+       C_COUNTS,    // n_equator_crossings (low word) and landing steps taken (high word)
+       kColdSlots };
+constexpr int kKSlots2 = 11;   // + (sin, cos) of theta_n
 constexpr int kParkSlotsDp54 = 17;
 constexpr size_t dp54_smem_bytes(bool disk) {
   return sizeof(double) * kBlock * (2 * kKSlots2 + kColdSlots + (disk ? kParkSlotsDp54 : 0));
@@ -73,15 +76,21 @@ trace_dp54(const __grid_constant__ TraceParams P) {
 
   // ---- per-lane ray state (registers) ----
   int mode = MODE_IDLE;
-  long long slot = -1;
   double pt = 0.0, pph = 0.0;                         // constants of the ray
   double r = 0.0, th = 0.0, pr = 0.0, pth = 0.0;      // y_n, the part Hamilton's equations read
-  double k1r = 0.0, k1th = 0.0, k1pr = 0.0, k1pth = 0.0;  // raw F(y_n), same part
+  // raw F(y_n) lives in shared memory (K slots 8, 9): written when y_n changes, read once per attempt
+#define GP_SET_K1(a_, b_, c_, d_) { sts2(KS(8), (a_), (b_)); sts2(KS(9), (c_), (d_)); }
+#define GP_SET_SC(s_, c_) if (METRIC == METRIC_KERR) sts2(KS(10), (s_), (c_));
   double h = 0.0;                                     // step of the attempt in flight / next attempt
   // pending (trial) state and the error sums that still lack the e7 k7 term
   double nt = 0.0, nr = 0.0, nth = 0.0, nph = 0.0, npr = 0.0, npth = 0.0, nlam = 0.0;
   double et = 0.0, er = 0.0, eth = 0.0, eph = 0.0, epr = 0.0, epth = 0.0;
-  unsigned n_acc = 0, n_rej = 0, n_cross = 0, n_rec = 0, n_land = 0, status = 0;
+  unsigned n_acc = 0, n_rej = 0, n_rec = 0, status = 0;   // n_cross, n_land: cold slot C_COUNTS
+#define GP_BUMP_COUNTS(dcross_, dland_)                                                        \
+  {                                                                                            \
+    double w_ = lds1(CS(C_COUNTS));                                                            \
+    sts1(CS(C_COUNTS), __hiloint2double(__double2hiint(w_) + (dland_), __double2loint(w_) + (dcross_))); \
+  }
   bool exhausted = false;
   sts1(CS(C_TOT_RAYS), 0.0); sts1(CS(C_TOT_STEPS), 0.0); sts1(CS(C_TOT_RHS), 0.0);
   stamp_start(P.counters);
@@ -93,7 +102,7 @@ trace_dp54(const __grid_constant__ TraceParams P) {
     if (need_mask) {
       const long long got = fetch_slot(need_mask, need, P.counters, P.cc.ray_count);
       if (need) {
-        slot = got;
+        const long long slot = got;
         if (slot < 0) {
           exhausted = true;
         } else {
@@ -101,7 +110,8 @@ trace_dp54(const __grid_constant__ TraceParams P) {
           ray_birth(P.cc, mc, P.cc.ray_begin + slot * P.cc.ray_stride, nr, nth, nph, pt, npr, npth, pph);
           nt = 0.0; nlam = 0.0;
           mode = MODE_FRESH;
-          n_acc = n_rej = n_cross = n_rec = n_land = 0;
+          n_acc = n_rej = n_rec = 0;
+          sts1(CS(C_SLOT), __longlong_as_double(slot)); sts1(CS(C_COUNTS), __longlong_as_double(0LL));
           const double inf = __longlong_as_double(0x7ff0000000000000LL);
           sts1(CS(C_HMAX), 0.0); sts1(CS(C_QDRIFT), 0.0); sts1(CS(C_Q0), 0.0); sts1(CS(C_IQ0), 1.0);
           sts1(CS(C_SINMIN), inf); sts1(CS(C_MARGIN), inf);
@@ -123,7 +133,8 @@ trace_dp54(const __grid_constant__ TraceParams P) {
       if (mode == MODE_FRESH) {
         r = nr; th = nth; pr = npr; pth = npth; lam = nlam;
         sts1(CS(C_T), nt); sts1(CS(C_PH), nph); sts1(CS(C_LAM), nlam);
-        k1r = o7.dr; k1th = o7.dth; k1pr = o7.dpr; k1pth = o7.dpth;
+        GP_SET_K1(o7.dr, o7.dth, o7.dpr, o7.dpth)
+        GP_SET_SC(o7.s, o7.c)
         sts1(CS(C_K1T), o7.dt); sts1(CS(C_K1PH), o7.dph);
         h = P.h_cap_rel * nr;               // R10 item 4: h0 = cap x the start radius (r_obs for the pinhole)
         monH = fabs(0.5 * o7.H2); monQ = carter_q<METRIC>(mc, pt, pph, npth, o7); monS = fabs(o7.s);
@@ -138,12 +149,13 @@ trace_dp54(const __grid_constant__ TraceParams P) {
         // divided once; a tie within rounding picks either of two equal ratios.
         // |h| is common to the six numerators and multiplies the winner only; the scale is built as
         // |larger of y, y+| * rtol + atol with the abs folded into the multiply's operand modifier.
-#define GP_SCALE(y_, ny_) (__dmul_rn(fabs(fabs(y_) > fabs(ny_) ? (y_) : (ny_)), P.rtol) + P.atol)
-        double nm = fabs(et + dp.E7 * o7.dt), dn = GP_SCALE(t, nt);
+#define GP_SCALE(y_, ny_) fma(fabs(fabs(y_) > fabs(ny_) ? (y_) : (ny_)), P.rtol, P.atol)
+        const double hE7 = dp.E7 * h;     // the error sums already carry the step (block C)
+        double nm = fabs(et + hE7 * o7.dt), dn = GP_SCALE(t, nt);
         double nsum = nm;
 #define GP_ERR_TERM(e_, k7_, y_, ny_)                                            \
   {                                                                              \
-    double n_ = fabs((e_) + dp.E7 * (k7_));                                      \
+    double n_ = fabs((e_) + hE7 * (k7_));                                        \
     double d_ = GP_SCALE(y_, ny_);                                               \
     nsum += n_;                                                                  \
     bool gt_ = n_ * dn > nm * d_;                                                \
@@ -157,11 +169,9 @@ trace_dp54(const __grid_constant__ TraceParams P) {
         GP_ERR_TERM(epth, o7.dpth, pth, npth)
 #undef GP_ERR_TERM
 #undef GP_SCALE
-        nm *= fabs(h);
         // finite test on the sums: any inf/NaN term makes them non-finite (numerators are >= 0)
-        double ysum = ((nt + nr) + (nth + nph)) + (npr + npth);
         double err = div_nr(nm, dn, rcp_nr(dn));
-        if (!finite_d(nsum) || !finite_d(ysum) || !finite_d(err)) {
+        if (!finite_d(nsum) || !finite_d(err)) {
           ++n_rej;
           h *= dp.fac_min;
         } else {
@@ -184,7 +194,7 @@ trace_dp54(const __grid_constant__ TraceParams P) {
             } else {
               bool commit = true;
               if ((th - kHalfPi) * (nth - kHalfPi) < 0.0) {
-                ++n_cross;
+                GP_BUMP_COUNTS(1, 0)
                 if (DISK && n_rec < (unsigned)P.max_crossings) {
                   // O7: locate the crossing from y_n; resume from the parked trial state afterwards
                   sts1(PS(0), nr); sts1(PS(1), nth); sts1(PS(2), npr); sts1(PS(3), npth);
@@ -203,7 +213,8 @@ trace_dp54(const __grid_constant__ TraceParams P) {
                 monH = fabs(0.5 * o7.H2); monQ = carter_q<METRIC>(mc, pt, pph, npth, o7); monS = fabs(o7.s);
                 r = nr; th = nth; pr = npr; pth = npth; lam += h;
                 sts1(CS(C_T), nt); sts1(CS(C_PH), nph); sts1(CS(C_LAM), lam);
-                k1r = o7.dr; k1th = o7.dth; k1pr = o7.dpr; k1pth = o7.dpth;
+                GP_SET_K1(o7.dr, o7.dth, o7.dpr, o7.dpth)
+                GP_SET_SC(o7.s, o7.c)
                 sts1(CS(C_K1T), o7.dt); sts1(CS(C_K1PH), o7.dph);
                 h = hnext;
                 moved = true;
@@ -215,13 +226,14 @@ trace_dp54(const __grid_constant__ TraceParams P) {
         // landed on the exit surface: the record is the landed state (R14)
         r = lds1(CS(C_TARGET)); th = nth; pr = npr; pth = npth;
         sts1(CS(C_T), nt); sts1(CS(C_PH), nph); sts1(CS(C_LAM), nlam);
-        ++n_land;
+        GP_BUMP_COUNTS(0, 1)
         finished = true;
       } else {  // MODE_LAND_TH
-        ++n_land;
+        GP_BUMP_COUNTS(0, 1)
         if (DISK) {
           double rc = nr;
           if (rc >= P.disk_r_in && rc <= P.disk_r_out) {
+            const long long slot = __double_as_longlong(lds1(CS(C_SLOT)));
             P.disk[slot].r_cross[n_rec] = rc;
             P.disk[slot].g[n_rec] = kepler_g<METRIC>(mc, rc, pt, pph);
             ++n_rec;
@@ -230,7 +242,8 @@ trace_dp54(const __grid_constant__ TraceParams P) {
           lam = lds1(PS(6)); h = lds1(PS(7));
           sts1(CS(C_T), lds1(PS(4))); sts1(CS(C_PH), lds1(PS(5))); sts1(CS(C_LAM), lam);
           sts1(CS(C_K1T), lds1(PS(8))); sts1(CS(C_K1PH), lds1(PS(11)));
-          k1r = lds1(PS(9)); k1th = lds1(PS(10)); k1pr = lds1(PS(12)); k1pth = lds1(PS(13));
+          GP_SET_K1(lds1(PS(9)), lds1(PS(10)), lds1(PS(12)), lds1(PS(13)))
+          { double rs, rc; sincos_fast(th, &rs, &rc); GP_SET_SC(rs, rc) }   // once per recorded crossing
           monH = lds1(PS(14)); monQ = lds1(PS(15)); monS = lds1(PS(16));
         }
         mode = MODE_NORMAL;
@@ -260,6 +273,9 @@ trace_dp54(const __grid_constant__ TraceParams P) {
 
       if (finished) {
         unsigned attempts = n_acc + n_rej;
+        const long long slot = __double_as_longlong(lds1(CS(C_SLOT)));
+        const double cw = lds1(CS(C_COUNTS));
+        const unsigned n_cross = (unsigned)__double2loint(cw), n_land = (unsigned)__double2hiint(cw);
         unsigned n_rhs = 1u + 6u * attempts + 5u * n_land;
         Monitors mo;
         mo.h_max = lds1(CS(C_HMAX)); mo.q_drift = lds1(CS(C_QDRIFT)); mo.Q0 = 0.0; mo.iQ0 = 0.0;
@@ -291,6 +307,8 @@ trace_dp54(const __grid_constant__ TraceParams P) {
         double s = h;
         double bl = 1.0;             // sum of b_i / F_w: d(lambda)/ds of the step, 1 for an ordinary step
         double k1t = lds1(CS(C_K1T)), k1ph = lds1(CS(C_K1PH));
+        double k1r, k1th, k1pr, k1pth;
+        lds2(KS(8), k1r, k1th); lds2(KS(9), k1pr, k1pth);
         if (any_land) {
           double iv = 1.0;
           if (landing) {
@@ -303,27 +321,47 @@ trace_dp54(const __grid_constant__ TraceParams P) {
         // divide the stage slopes of a landing lane by F_w and add its b_i / F_w to bl
 #define GP_HENON(b_i)                                                           \
   if (any_land) {                                                               \
-    double iv = landing ? rcp_nr(land_r ? o.dr : o.dth) : 1.0;                  \
+    double iv = landing ? s * rcp_nr(land_r ? o.dr : o.dth) : 1.0;  /* o is s F */ \
     o.dr *= iv; o.dth *= iv; o.dpr *= iv; o.dpth *= iv; o.dt *= iv; o.dph *= iv; \
     bl += (b_i) * iv;                                                           \
   }
-        // quadratures t, phi: running 5th-order sums and the two error sums
-        double bt = dp.B1 * k1t, bph = dp.B1 * k1ph;
-        double qet = dp.E1 * k1t, qeph = dp.E1 * k1ph;
+        // Every K below is s F (or s F / F_w on a landing lane): the stage evaluations return their
+        // derivatives already multiplied by the step (rhs_eval_scaled), k1 is scaled once here, and the
+        // stage states, the trial state and the error sums are plain FMA chains from y_n.
+        const double hk1r = s * k1r, hk1th = s * k1th, hk1pr = s * k1pr, hk1pth = s * k1pth;
+        const double hk1t = s * k1t, hk1ph = s * k1ph;
+        // Stage angles (Kerr; for Schwarzschild the extra registers cost a spill): the theta sums below start from 0 instead of theta_n, so they
+        // are the increments d_j, and sin, cos of theta_n + d_j come from (sin, cos) theta_n — by-products of
+        // the evaluation that produced k1, kept in K slot 10 — through the addition theorems (sincos_add):
+        // no range reduction or quadrant logic inside the stages.  Manko-Novikov evaluates its own sincos.
+        constexpr bool kAngle = (METRIC == METRIC_KERR);
+        const double thb = kAngle ? 0.0 : th;
+        double sn_ = 0.0, cn_ = 0.0;
+        if (kAngle) lds2(KS(10), sn_, cn_);
+#define GP_STAGE_RHS(xr_, xth_, xpr_, xpth_)                                                   \
+  if (kAngle) {                                                                                \
+    double ss_, cc_;                                                                           \
+    sincos_add(sn_, cn_, (xth_), &ss_, &cc_);                                                  \
+    rhs_eval_scaled_sc<METRIC>(mc, pt, pph, (xr_), ss_, cc_, (xpr_), (xpth_), s, o);           \
+  } else {                                                                                     \
+    rhs_eval_scaled<METRIC, true>(mc, pt, pph, (xr_), (xth_), (xpr_), (xpth_), s, o);          \
+  }
+        double bt = dp.B1 * hk1t, bph = dp.B1 * hk1ph;
+        double qet = dp.E1 * hk1t, qeph = dp.E1 * hk1ph;
         Rhs o;
         double ar, ath, apr, apth;   // K_j of the stage just evaluated
         double br, bth, bpr, bpth;   // K's streamed back from shared memory
         // stage 2
-        rhs_eval<METRIC, true>(mc, pt, pph, r + s * (dp.A21 * k1r), th + s * (dp.A21 * k1th),
-                         pr + s * (dp.A21 * k1pr), pth + s * (dp.A21 * k1pth), o);
+        GP_STAGE_RHS( fma(dp.A21, hk1r, r), fma(dp.A21, hk1th, thb),
+                                      fma(dp.A21, hk1pr, pr), fma(dp.A21, hk1pth, pth))
         GP_HENON(0.0)
         ar = o.dr; ath = o.dth; apr = o.dpr; apth = o.dpth;                         // K2
         sts2(KS(0), ar, ath); sts2(KS(1), apr, apth);
         // stage 3
-        rhs_eval<METRIC, true>(mc, pt, pph, r + s * (dp.A31 * k1r + dp.A32 * ar),
-                         th + s * (dp.A31 * k1th + dp.A32 * ath),
-                         pr + s * (dp.A31 * k1pr + dp.A32 * apr),
-                         pth + s * (dp.A31 * k1pth + dp.A32 * apth), o);
+        GP_STAGE_RHS( fma(dp.A32, ar, fma(dp.A31, hk1r, r)),
+                                      fma(dp.A32, ath, fma(dp.A31, hk1th, thb)),
+                                      fma(dp.A32, apr, fma(dp.A31, hk1pr, pr)),
+                                      fma(dp.A32, apth, fma(dp.A31, hk1pth, pth)))
         GP_HENON(dp.B3)
         ar = o.dr; ath = o.dth; apr = o.dpr; apth = o.dpth;                         // K3
         sts2(KS(2), ar, ath); sts2(KS(3), apr, apth);
@@ -331,11 +369,11 @@ trace_dp54(const __grid_constant__ TraceParams P) {
         qet += dp.E3 * o.dt; qeph += dp.E3 * o.dph;
         // stage 4
         {
-          double xr = dp.A41 * k1r + dp.A43 * ar, xth = dp.A41 * k1th + dp.A43 * ath;
-          double xpr = dp.A41 * k1pr + dp.A43 * apr, xpth = dp.A41 * k1pth + dp.A43 * apth;
+          double xr = fma(dp.A43, ar, fma(dp.A41, hk1r, r)), xth = fma(dp.A43, ath, fma(dp.A41, hk1th, thb));
+          double xpr = fma(dp.A43, apr, fma(dp.A41, hk1pr, pr)), xpth = fma(dp.A43, apth, fma(dp.A41, hk1pth, pth));
           lds2(KS(0), br, bth); lds2(KS(1), bpr, bpth);                             // K2
-          xr += dp.A42 * br; xth += dp.A42 * bth; xpr += dp.A42 * bpr; xpth += dp.A42 * bpth;
-          rhs_eval<METRIC, true>(mc, pt, pph, r + s * xr, th + s * xth, pr + s * xpr, pth + s * xpth, o);
+          xr = fma(dp.A42, br, xr); xth = fma(dp.A42, bth, xth); xpr = fma(dp.A42, bpr, xpr); xpth = fma(dp.A42, bpth, xpth);
+          GP_STAGE_RHS( xr, xth, xpr, xpth)
         }
         GP_HENON(dp.B4)
         ar = o.dr; ath = o.dth; apr = o.dpr; apth = o.dpth;                         // K4
@@ -344,13 +382,13 @@ trace_dp54(const __grid_constant__ TraceParams P) {
         qet += dp.E4 * o.dt; qeph += dp.E4 * o.dph;
         // stage 5
         {
-          double xr = dp.A51 * k1r + dp.A54 * ar, xth = dp.A51 * k1th + dp.A54 * ath;
-          double xpr = dp.A51 * k1pr + dp.A54 * apr, xpth = dp.A51 * k1pth + dp.A54 * apth;
+          double xr = fma(dp.A54, ar, fma(dp.A51, hk1r, r)), xth = fma(dp.A54, ath, fma(dp.A51, hk1th, thb));
+          double xpr = fma(dp.A54, apr, fma(dp.A51, hk1pr, pr)), xpth = fma(dp.A54, apth, fma(dp.A51, hk1pth, pth));
           lds2(KS(0), br, bth); lds2(KS(1), bpr, bpth);                             // K2
-          xr += dp.A52 * br; xth += dp.A52 * bth; xpr += dp.A52 * bpr; xpth += dp.A52 * bpth;
+          xr = fma(dp.A52, br, xr); xth = fma(dp.A52, bth, xth); xpr = fma(dp.A52, bpr, xpr); xpth = fma(dp.A52, bpth, xpth);
           lds2(KS(2), br, bth); lds2(KS(3), bpr, bpth);                             // K3
-          xr += dp.A53 * br; xth += dp.A53 * bth; xpr += dp.A53 * bpr; xpth += dp.A53 * bpth;
-          rhs_eval<METRIC, true>(mc, pt, pph, r + s * xr, th + s * xth, pr + s * xpr, pth + s * xpth, o);
+          xr = fma(dp.A53, br, xr); xth = fma(dp.A53, bth, xth); xpr = fma(dp.A53, bpr, xpr); xpth = fma(dp.A53, bpth, xpth);
+          GP_STAGE_RHS( xr, xth, xpr, xpth)
         }
         GP_HENON(dp.B5)
         ar = o.dr; ath = o.dth; apr = o.dpr; apth = o.dpth;                         // K5
@@ -359,15 +397,15 @@ trace_dp54(const __grid_constant__ TraceParams P) {
         qet += dp.E5 * o.dt; qeph += dp.E5 * o.dph;
         // stage 6
         {
-          double xr = dp.A61 * k1r + dp.A65 * ar, xth = dp.A61 * k1th + dp.A65 * ath;
-          double xpr = dp.A61 * k1pr + dp.A65 * apr, xpth = dp.A61 * k1pth + dp.A65 * apth;
+          double xr = fma(dp.A65, ar, fma(dp.A61, hk1r, r)), xth = fma(dp.A65, ath, fma(dp.A61, hk1th, thb));
+          double xpr = fma(dp.A65, apr, fma(dp.A61, hk1pr, pr)), xpth = fma(dp.A65, apth, fma(dp.A61, hk1pth, pth));
           lds2(KS(0), br, bth); lds2(KS(1), bpr, bpth);                             // K2
-          xr += dp.A62 * br; xth += dp.A62 * bth; xpr += dp.A62 * bpr; xpth += dp.A62 * bpth;
+          xr = fma(dp.A62, br, xr); xth = fma(dp.A62, bth, xth); xpr = fma(dp.A62, bpr, xpr); xpth = fma(dp.A62, bpth, xpth);
           lds2(KS(2), br, bth); lds2(KS(3), bpr, bpth);                             // K3
-          xr += dp.A63 * br; xth += dp.A63 * bth; xpr += dp.A63 * bpr; xpth += dp.A63 * bpth;
+          xr = fma(dp.A63, br, xr); xth = fma(dp.A63, bth, xth); xpr = fma(dp.A63, bpr, xpr); xpth = fma(dp.A63, bpth, xpth);
           lds2(KS(4), br, bth); lds2(KS(5), bpr, bpth);                             // K4
-          xr += dp.A64 * br; xth += dp.A64 * bth; xpr += dp.A64 * bpr; xpth += dp.A64 * bpth;
-          rhs_eval<METRIC, true>(mc, pt, pph, r + s * xr, th + s * xth, pr + s * xpr, pth + s * xpth, o);
+          xr = fma(dp.A64, br, xr); xth = fma(dp.A64, bth, xth); xpr = fma(dp.A64, bpr, xpr); xpth = fma(dp.A64, bpth, xpth);
+          GP_STAGE_RHS( xr, xth, xpr, xpth)
         }
         GP_HENON(dp.B6)
         ar = o.dr; ath = o.dth; apr = o.dpr; apth = o.dpth;                         // K6
@@ -376,26 +414,27 @@ trace_dp54(const __grid_constant__ TraceParams P) {
 #undef GP_HENON
         // trial end state (5th-order solution; a7 = b) and the error sums without e7 k7
         {
-          double xr = dp.B1 * k1r + dp.B6 * ar, xth = dp.B1 * k1th + dp.B6 * ath;
-          double xpr = dp.B1 * k1pr + dp.B6 * apr, xpth = dp.B1 * k1pth + dp.B6 * apth;
-          er = dp.E1 * k1r + dp.E6 * ar; eth = dp.E1 * k1th + dp.E6 * ath;
-          epr = dp.E1 * k1pr + dp.E6 * apr; epth = dp.E1 * k1pth + dp.E6 * apth;
+          double xr = fma(dp.B6, ar, fma(dp.B1, hk1r, r)), xth = fma(dp.B6, ath, fma(dp.B1, hk1th, th));
+          double xpr = fma(dp.B6, apr, fma(dp.B1, hk1pr, pr)), xpth = fma(dp.B6, apth, fma(dp.B1, hk1pth, pth));
+          er = dp.E1 * hk1r + dp.E6 * ar; eth = dp.E1 * hk1th + dp.E6 * ath;
+          epr = dp.E1 * hk1pr + dp.E6 * apr; epth = dp.E1 * hk1pth + dp.E6 * apth;
           lds2(KS(2), br, bth); lds2(KS(3), bpr, bpth);                             // K3
-          xr += dp.B3 * br; xth += dp.B3 * bth; xpr += dp.B3 * bpr; xpth += dp.B3 * bpth;
+          xr = fma(dp.B3, br, xr); xth = fma(dp.B3, bth, xth); xpr = fma(dp.B3, bpr, xpr); xpth = fma(dp.B3, bpth, xpth);
           er += dp.E3 * br; eth += dp.E3 * bth; epr += dp.E3 * bpr; epth += dp.E3 * bpth;
           lds2(KS(4), br, bth); lds2(KS(5), bpr, bpth);                             // K4
-          xr += dp.B4 * br; xth += dp.B4 * bth; xpr += dp.B4 * bpr; xpth += dp.B4 * bpth;
+          xr = fma(dp.B4, br, xr); xth = fma(dp.B4, bth, xth); xpr = fma(dp.B4, bpr, xpr); xpth = fma(dp.B4, bpth, xpth);
           er += dp.E4 * br; eth += dp.E4 * bth; epr += dp.E4 * bpr; epth += dp.E4 * bpth;
           lds2(KS(6), br, bth); lds2(KS(7), bpr, bpth);                             // K5
-          xr += dp.B5 * br; xth += dp.B5 * bth; xpr += dp.B5 * bpr; xpth += dp.B5 * bpth;
+          xr = fma(dp.B5, br, xr); xth = fma(dp.B5, bth, xth); xpr = fma(dp.B5, bpr, xpr); xpth = fma(dp.B5, bpth, xpth);
           er += dp.E5 * br; eth += dp.E5 * bth; epr += dp.E5 * bpr; epth += dp.E5 * bpth;
-          nr = r + s * xr; nth = th + s * xth; npr = pr + s * xpr; npth = pth + s * xpth;
+          nr = xr; nth = xth; npr = xpr; npth = xpth;
         }
-        nt = lds1(CS(C_T)) + s * bt;
-        nph = lds1(CS(C_PH)) + s * bph;
+        nt = lds1(CS(C_T)) + bt;
+        nph = lds1(CS(C_PH)) + bph;
         nlam = lds1(CS(C_LAM)) + s * bl;
         et = qet;
         eph = qeph;
+#undef GP_STAGE_RHS
       }
     }
   }

@@ -199,7 +199,7 @@ def chaos_flags(orc, companion):
     return (ea != eb) | (ea & eb & (ang > 1.0))
 
 
-def check_h_drift(rays, orc, smooth, adaptive, label="", manko_novikov=False):
+def check_h_drift(rays, orc, smooth, adaptive, label="", manko_novikov=False, chaotic_band=False):
     """|H| drift (R22) on smooth escaped rays.  The two sides must report the same drift
     (1e-11 + 25 %: the running maximum is itself a rounding-level cancellation, and the oracle's
     own FMA build moves it by up to 14 %), the CUDA path may not drift more than 1.5 x the oracle,
@@ -218,7 +218,9 @@ def check_h_drift(rays, orc, smooth, adaptive, label="", manko_novikov=False):
     bad = np.abs(gh - oh) > 1e-11 + 0.25 * np.maximum(gh, oh)
     # Manko-Novikov: equal counts do not prove equal sequences (a rejection at another step, see the
     # counter rule in check_parity), so 1 % of those rays may sample other points
-    allow = 0.01 * bad.size if manko_novikov else 0.0
+    # (workload X3, the chaotic band: 3 % — the oracle's own x87 build differs from it on 1.5 % of such rays,
+    # tests/test_parity_threshold.py)
+    allow = (0.03 if chaotic_band else 0.01) * bad.size if manko_novikov else 0.0
     assert bad.sum() <= allow, (f"{label}: |H| drift differs on {bad.sum()} of {bad.size} rays, e.g. CUDA "
                                 f"{gh[bad][:3]} against oracle {oh[bad][:3]}")
     assert ((gh > 1.5 * oh + 1e-11).sum() <= allow), f"{label}: the CUDA path drifts more than the oracle"

@@ -50,13 +50,15 @@ def check_parity(w, rays, orc, probe, label, **kw):
                         manko_novikov=w["metric"]["id"] == W.MANKO_NOVIKOV, **kw)
     smooth = res.pop("smooth_mask")
     mn = w["metric"]["id"] == W.MANKO_NOVIKOV
-    check_h_drift(rays, orc, smooth, adaptive=w["cfg"]["scheme"] == 2, label=label, manko_novikov=mn)
+    check_h_drift(rays, orc, smooth, adaptive=w["cfg"]["scheme"] == 2, label=label, manko_novikov=mn,
+                  chaotic_band=kw.get("smooth_outlier_fraction", 0.0) > 0.0)
     # the other monitors, on smooth rays.  sin(theta)_min is a minimum over the discrete step
     # endpoints, so it moves with the step sequence (measured 3e-7 on a Manko-Novikov ray whose
     # error estimate is rounding-dominated); it is a flagging aid, not an output of the method.
     same = smooth & same_step_sequence(rays, orc)
     off = ~np.isclose(rays["sin_theta_min"][same], orc["sin_theta_min"][same], rtol=1e-5, atol=1e-12)
-    assert off.sum() <= (0.01 * off.size if mn else 0), (label, int(off.sum()), off.size)
+    assert off.sum() <= ((0.03 if kw.get("smooth_outlier_fraction", 0.0) > 0.0 else 0.01) * off.size if mn else 0), (
+        label, int(off.sum()), off.size)
     if w["metric"]["id"] != W.MANKO_NOVIKOV and w["cfg"]["scheme"] == 2:
         esc = same & (orc["status"] == 0)
         assert np.abs(rays["q_drift"] - orc["q_drift"])[esc].max() <= 1e-10 + 0.25 * orc["q_drift"][esc].max()

@@ -80,6 +80,13 @@ def test_chaotic_band_x3_outlier_fraction_is_a_property_of_the_workload():
     assert smooth.sum() >= 300
     assert past.sum() <= 0.02 * smooth.sum()
     assert third[smooth].max() <= 1e-6
+    # the running maximum of |H| is sampled at the step end points: even with equal step COUNTS the two
+    # builds step through different sequences on 1-2 % of these rays (parity_rules.check_h_drift allows 3 %)
+    same = smooth & (orc["n_accepted"] == x87["n_accepted"]) & (orc["n_rejected"] == x87["n_rejected"])
+    gh, oh = x87["h_max"][same], orc["h_max"][same]
+    other_points = np.abs(gh - oh) > 1e-11 + 0.25 * np.maximum(gh, oh)
+    print("X3 sample: |H| maxima differ on", int(other_points.sum()), "of", int(same.sum()), "equal-count rays")
+    assert other_points.mean() <= 0.03
 
 
 if __name__ == "__main__":
