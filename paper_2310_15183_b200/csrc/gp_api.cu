@@ -113,6 +113,8 @@ int make_camera(int metric_id, const MetricConst &mc, const gp_camera *c, double
   cc->shift_y_px = c->shift_y_px;
   cc->jitter_seed = c->jitter_seed;
   cc->Wt = Wt;
+  cc->inv_Wt = 1.0 / (double)Wt;
+  cc->inv_S = ((S & (S - 1)) == 0) ? 1.0 / (double)S : 0.0;
   cc->ray_begin = c->ray_begin;
   cc->ray_count = c->ray_count;
   cc->ray_stride = c->ray_stride;

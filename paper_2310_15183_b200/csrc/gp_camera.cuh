@@ -21,6 +21,9 @@ struct CameraConst {
   double jitter_amp_px, shift_x_px, shift_y_px;
   unsigned long long jitter_seed;
   long long Wt;                  // width * S
+  double inv_Wt;                 // 1 / Wt (seed of the row / column split of the ray index)
+  double inv_S;                  // 1 / S when S is a power of two (the division by S is then an exact
+                                 // multiplication), else 0: IEEE division
   long long ray_begin, ray_count, ray_stride;
   // observer (R12): position and ZAMO tetrad constants from the covariant metric there
   double r_obs, theta_obs, phi_obs;
@@ -51,8 +54,12 @@ __device__ __forceinline__ double jitter_unit(unsigned long long seed, unsigned 
 // Row a2.  ray = index in the supersampled image, row-major, J = 0 <-> beta_min.
 __device__ __forceinline__ void alpha_beta(const CameraConst &cc, long long ray, double &alpha,
                                            double &beta) {
-  long long J = ray / cc.Wt;
+  // row J = ray div Wt, column I = ray mod Wt: quotient estimated in FP64 (exact to +-1 for ray < 2^52),
+  // corrected with integers — a 64-bit integer division is ~80 instructions, once per ray
+  long long J = (long long)__dmul_rn((double)ray, cc.inv_Wt);
   long long I = ray - J * cc.Wt;
+  if (I < 0) { J -= 1; I += cc.Wt; }
+  else if (I >= cc.Wt) { J += 1; I -= cc.Wt; }
   double jx = 0.0, jy = 0.0;
   if (cc.jitter_amp_px > 0.0) {
     double ux = jitter_unit(cc.jitter_seed, (unsigned long long)ray, 0ULL);
@@ -60,8 +67,17 @@ __device__ __forceinline__ void alpha_beta(const CameraConst &cc, long long ray,
     jx = __dmul_rn(__dadd_rn(__dmul_rn(2.0, ux), -1.0), cc.jitter_amp_px);
     jy = __dmul_rn(__dadd_rn(__dmul_rn(2.0, uy), -1.0), cc.jitter_amp_px);
   }
-  double X = __dadd_rn(__dadd_rn(__ddiv_rn(__dadd_rn((double)I, 0.5), cc.supersample_d), jx), cc.shift_x_px);
-  double Y = __dadd_rn(__dadd_rn(__ddiv_rn(__dadd_rn((double)J, 0.5), cc.supersample_d), jy), cc.shift_y_px);
+  // (I + 0.5)/S: S = 2^k makes x * (1/S) the same double as x / S
+  double xs = __dadd_rn((double)I, 0.5), ys = __dadd_rn((double)J, 0.5);
+  if (cc.inv_S != 0.0) {
+    xs = __dmul_rn(xs, cc.inv_S);
+    ys = __dmul_rn(ys, cc.inv_S);
+  } else {
+    xs = __ddiv_rn(xs, cc.supersample_d);
+    ys = __ddiv_rn(ys, cc.supersample_d);
+  }
+  double X = __dadd_rn(__dadd_rn(xs, jx), cc.shift_x_px);
+  double Y = __dadd_rn(__dadd_rn(ys, jy), cc.shift_y_px);
   alpha = __dadd_rn(cc.alpha_min, __dmul_rn(X, cc.dalpha));
   beta = __dadd_rn(cc.beta_min, __dmul_rn(Y, cc.dbeta));
 }
@@ -73,7 +89,7 @@ __device__ __forceinline__ void alpha_beta(const CameraConst &cc, long long ray,
 __device__ __forceinline__ void initial_momentum(const CameraConst &cc, double alpha, double beta,
                                                  double &pt, double &pr, double &pth, double &pph) {
   double ro = cc.r_obs;
-  double iD = 1.0 / sqrt(ro * ro + alpha * alpha + beta * beta);
+  double iD = rsqrt(ro * ro + alpha * alpha + beta * beta);
   pr = cc.sq_grr * (-ro * iD);
   pth = cc.sq_gthth * (-beta * iD);
   pph = cc.sq_gpp * (alpha * iD);

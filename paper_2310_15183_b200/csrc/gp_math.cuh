@@ -82,11 +82,17 @@ __device__ __forceinline__ double div_nr(double a, double b, double y) {
 // sin and cos of x for |x| < 1e5 (the polar angle never leaves a few multiples of pi); the
 // library routine takes over beyond that.  Cody-Waite reduction to |r| <= pi/4 with a three-part
 // pi/2, then the two kernels, then the quadrant swap.
-__device__ __noinline__ void sincos_library(double x, double *sn, double *cs) { sincos(x, sn, cs); }
+__device__ __noinline__ double2 sincos_library(double x) {
+  double2 r;
+  sincos(x, &r.x, &r.y);
+  return r;   // by value: the results come back in registers, not through the caller's stack frame
+}
 
 __device__ __forceinline__ void sincos_fast(double x, double *sn, double *cs) {
   if (!(fabs(x) < 1.0e5)) {
-    sincos_library(x, sn, cs);
+    double2 sc = sincos_library(x);
+    *sn = sc.x;
+    *cs = sc.y;
     return;
   }
   double qd = rint(x * kMath.two_over_pi);

@@ -28,6 +28,7 @@ enum { C_T = 0, C_PH, C_LAM, C_HMAX, C_QDRIFT, C_Q0, C_IQ0, C_SINMIN, C_MARGIN, 
        C_TOT_RAYS, C_TOT_STEPS, C_TOT_RHS,
        C_SLOT,      // output slot of the ray in flight (64-bit integer bits)
        C_COUNTS,    // n_equator_crossings (low word) and landing steps taken (high word)
+       C_STATE,     // status of the ray once decided (low word) and disk crossings recorded (high word)
        kColdSlots };
 constexpr int kKSlots2 = 11;   // + (sin, cos) of theta_n
 constexpr int kParkSlotsDp54 = 17;
@@ -85,7 +86,12 @@ trace_dp54(const __grid_constant__ TraceParams P) {
   // pending (trial) state and the error sums that still lack the e7 k7 term
   double nt = 0.0, nr = 0.0, nth = 0.0, nph = 0.0, npr = 0.0, npth = 0.0, nlam = 0.0;
   double et = 0.0, er = 0.0, eth = 0.0, eph = 0.0, epr = 0.0, epth = 0.0;
-  unsigned n_acc = 0, n_rej = 0, n_rec = 0, status = 0;   // n_cross, n_land: cold slot C_COUNTS
+  unsigned n_acc = 0, n_rej = 0;   // n_cross, n_land: cold slot C_COUNTS; status, n_rec: C_STATE
+#define GP_SET_STATUS(code_)                                                                   \
+  {                                                                                            \
+    double w_ = lds1(CS(C_STATE));                                                             \
+    sts1(CS(C_STATE), __hiloint2double(__double2hiint(w_), (int)(code_)));                     \
+  }
 #define GP_BUMP_COUNTS(dcross_, dland_)                                                        \
   {                                                                                            \
     double w_ = lds1(CS(C_COUNTS));                                                            \
@@ -110,8 +116,9 @@ trace_dp54(const __grid_constant__ TraceParams P) {
           ray_birth(P.cc, mc, P.cc.ray_begin + slot * P.cc.ray_stride, nr, nth, nph, pt, npr, npth, pph);
           nt = 0.0; nlam = 0.0;
           mode = MODE_FRESH;
-          n_acc = n_rej = n_rec = 0;
+          n_acc = n_rej = 0;
           sts1(CS(C_SLOT), __longlong_as_double(slot)); sts1(CS(C_COUNTS), __longlong_as_double(0LL));
+          sts1(CS(C_STATE), __longlong_as_double(0LL));
           const double inf = __longlong_as_double(0x7ff0000000000000LL);
           sts1(CS(C_HMAX), 0.0); sts1(CS(C_QDRIFT), 0.0); sts1(CS(C_Q0), 0.0); sts1(CS(C_IQ0), 1.0);
           sts1(CS(C_SINMIN), inf); sts1(CS(C_MARGIN), inf);
@@ -188,14 +195,14 @@ trace_dp54(const __grid_constant__ TraceParams P) {
             double hnext = dmin(h * fac, P.h_cap_rel * nr);
             if (nr > P.r_esc || nr < P.r_cap) {
               // O8: discard the step, land on the surface from y_n
-              status = (nr > P.r_esc) ? GP_RAY_ESCAPED : GP_RAY_CAPTURED;
+              GP_SET_STATUS((nr > P.r_esc) ? GP_RAY_ESCAPED : GP_RAY_CAPTURED)
               sts1(CS(C_TARGET), (nr > P.r_esc) ? P.r_esc : P.r_cap);
               mode = MODE_LAND_R;
             } else {
               bool commit = true;
               if ((th - kHalfPi) * (nth - kHalfPi) < 0.0) {
                 GP_BUMP_COUNTS(1, 0)
-                if (DISK && n_rec < (unsigned)P.max_crossings) {
+                if (DISK && (unsigned)__double2hiint(lds1(CS(C_STATE))) < (unsigned)P.max_crossings) {
                   // O7: locate the crossing from y_n; resume from the parked trial state afterwards
                   sts1(PS(0), nr); sts1(PS(1), nth); sts1(PS(2), npr); sts1(PS(3), npth);
                   sts1(PS(4), nt); sts1(PS(5), nph); sts1(PS(6), lam + h); sts1(PS(7), hnext);
@@ -234,9 +241,11 @@ trace_dp54(const __grid_constant__ TraceParams P) {
           double rc = nr;
           if (rc >= P.disk_r_in && rc <= P.disk_r_out) {
             const long long slot = __double_as_longlong(lds1(CS(C_SLOT)));
+            const double sw = lds1(CS(C_STATE));
+            const unsigned n_rec = (unsigned)__double2hiint(sw);
             P.disk[slot].r_cross[n_rec] = rc;
             P.disk[slot].g[n_rec] = kepler_g<METRIC>(mc, rc, pt, pph);
-            ++n_rec;
+            sts1(CS(C_STATE), __hiloint2double((int)(n_rec + 1u), __double2loint(sw)));
           }
           r = lds1(PS(0)); th = lds1(PS(1)); pr = lds1(PS(2)); pth = lds1(PS(3));
           lam = lds1(PS(6)); h = lds1(PS(7));
@@ -254,10 +263,10 @@ trace_dp54(const __grid_constant__ TraceParams P) {
       if (mode == MODE_NORMAL) {
         // max_steps <= 5e8 (validated by the host) fits the 32-bit counters; lambda_max is +inf when off
         if (n_acc + n_rej >= (unsigned)P.max_steps || lam >= P.lambda_max) {
-          status = GP_RAY_MAXSTEPS;
+          GP_SET_STATUS(GP_RAY_MAXSTEPS)
           finished = true;
         } else if (h < dp.h_floor || h < dp.h_floor * fabs(lam)) {   // h < h_floor max(1, |lambda|)
-          status = GP_RAY_STEP_UNDERFLOW;
+          GP_SET_STATUS(GP_RAY_STEP_UNDERFLOW)
           finished = true;
         } else if (moved) {
           Monitors mo;
@@ -276,6 +285,8 @@ trace_dp54(const __grid_constant__ TraceParams P) {
         const long long slot = __double_as_longlong(lds1(CS(C_SLOT)));
         const double cw = lds1(CS(C_COUNTS));
         const unsigned n_cross = (unsigned)__double2loint(cw), n_land = (unsigned)__double2hiint(cw);
+        const double sw = lds1(CS(C_STATE));
+        const unsigned status = (unsigned)__double2loint(sw), n_rec = (unsigned)__double2hiint(sw);
         unsigned n_rhs = 1u + 6u * attempts + 5u * n_land;
         Monitors mo;
         mo.h_max = lds1(CS(C_HMAX)); mo.q_drift = lds1(CS(C_QDRIFT)); mo.Q0 = 0.0; mo.iQ0 = 0.0;
