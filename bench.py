@@ -30,10 +30,22 @@ if ROOT not in sys.path:
 
 import gp_workloads as W  # noqa: E402
 
-# ---- algorithmic FP64 flop model (+,-,x = 1, FMA = 2, 1/x, sqrt, sin, cos,
-# exp, pow = 1 each), counted from the formulas of SURVEY.md appendix A/B as implemented ----------
-F_RHS = {W.SCHWARZSCHILD: 40.0, W.KERR: 81.0, W.MANKO_NOVIKOV: 760.0}
-F_STEP = {0: 56.0, 1: 57.0, 2: 324.0}
+# ---- algorithmic FP64 flop models (+,-,x = 1, FMA = 2, 1/x, sqrt, sin, cos,
+# exp, pow = 1 each).  `roofline.frac` uses SURVEY.md section 8(d)'s per-unit figures (30 / 70 per
+# Schwarzschild / Kerr RHS, 55 per RK4 step, 330 per DP5(4) step; for Manko-Novikov the survey gives a
+# range, 600-1000, "builder to count": 760).  The builder's own count of the formulas of SURVEY.md
+# appendix A/B as written out in csrc/gp_metric.cuh is printed beside it (`frac_builder_model`). ------
+F_RHS = {W.SCHWARZSCHILD: 30.0, W.KERR: 70.0, W.MANKO_NOVIKOV: 760.0}
+F_STEP = {0: 55.0, 1: 55.0, 2: 330.0}
+F_RHS_BUILDER = {W.SCHWARZSCHILD: 40.0, W.KERR: 81.0, W.MANKO_NOVIKOV: 760.0}
+F_STEP_BUILDER = {0: 56.0, 1: 57.0, 2: 324.0}
+# Counter evidence that one timed run cannot produce (ncu replays kernels; a number printed under ncu is
+# never a bench value): hardware-counted FP64 flops / cycle as a fraction of the FMA peak, and DRAM bytes
+# per launch, of the SAME kernel build on the SAME workload, each with the profiles/ file it comes from.
+# Workloads without a capture report null and say so.
+PROFILED = {
+    ("headline", "fp64"): {"hw_fp64_frac": 0.488, "traffic": 8.41e7, "source": "profiles/trace_dp54_r02b.md"},
+}
 # nominal FP64 FMA peak: 148 SMs x 64 FP64 FMA lanes x 2 flop x 1.965 GHz
 FP64_LANES_PER_SM = 64
 FP32_LANES_PER_SM = 128
@@ -52,6 +64,11 @@ def _args():
                     help="fp32: the single-precision variant (fixed-step RK4 workloads only)")
     ap.add_argument("--stage", default="trace", choices=["trace", "shade"],
                     help="shade: time the image-formation kernel gp_shade on the records of a 2048^2 frame")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: weak = one frame per rank; strong = ONE frame split cyclically over the ranks "
+                         "(gp_workloads.shard, DESIGN.md section 8)")
+    ap.add_argument("--back-to-back", type=int, default=8,
+                    help="images of the extra back-to-back measurement on two streams (0 = skip)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -110,9 +127,10 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def alg_flops(w, attempts, n_rhs):
+def alg_flops(w, attempts, n_rhs, builder=False):
     """Algorithmic FP64 flops of a trace from its step and RHS counts."""
-    return F_RHS[w["metric"]["id"]] * float(n_rhs) + F_STEP[w["cfg"]["scheme"]] * float(attempts)
+    fr, fs = (F_RHS_BUILDER, F_STEP_BUILDER) if builder else (F_RHS, F_STEP)
+    return fr[w["metric"]["id"]] * float(n_rhs) + fs[w["cfg"]["scheme"]] * float(attempts)
 
 
 def config_of(w, n_gpus, extra=None):
@@ -132,7 +150,7 @@ def config_of(w, n_gpus, extra=None):
 
 
 # ---- the oracle, timed (cpu_baseline leg and --impl reference) --------------------------------------
-def oracle_sample(w, seconds):
+def oracle_sample(w, seconds, single_thread_seconds=0.0):
     """Time the oracle on a scattered subsample of the workload sized for about `seconds`."""
     from oracle import oracle as O
     total = W.n_rays(w)
@@ -150,10 +168,20 @@ def oracle_sample(w, seconds):
     t0 = time.perf_counter()
     rec, used = O.trace(w, b, c, s, n_threads=cores)
     dt = time.perf_counter() - t0
-    return {"value": c / dt, "unit": "geodesics/s", "cores": int(used), "kind": "oracle",
-            "sample": f"{c} rays of {w['name']} (ray stride {s} from ray {b}), {dt:.2f} s wall, "
-                      f"OpenMP dynamic over rays, g++ -O2 -ffp-contract=off",
-            "rhs_evals_per_s": float(rec["n_rhs"].sum()) / dt, "seconds": dt, "rays": c}
+    out = {"value": c / dt, "unit": "geodesics/s", "cores": int(used), "kind": "oracle",
+           "sample": f"{c} rays of {w['name']} (ray stride {s} from ray {b}), {dt:.2f} s wall, "
+                     f"OpenMP dynamic over rays, g++ -O2 -ffp-contract=off",
+           "rhs_evals_per_s": float(rec["n_rhs"].sum()) / dt, "seconds": dt, "rays": c}
+    if single_thread_seconds > 0:
+        # "also the single-thread rate" — a smaller sample of the same kind, one thread
+        c1 = int(max(256, min(c, out["value"] / max(1, used) * single_thread_seconds)))
+        b1, c1, s1 = W.ray_selection(w, 0, c1, (-(-total // c1)) | 1)
+        t0 = time.perf_counter()
+        O.trace(w, b1, c1, s1, n_threads=1)
+        dt1 = time.perf_counter() - t0
+        out["single_thread"] = {"value": c1 / dt1, "unit": "geodesics/s",
+                                "sample": f"{c1} rays (stride {s1}), {dt1:.2f} s wall, 1 thread"}
+    return out
 
 
 def run_reference(args):
@@ -201,18 +229,24 @@ def run_b200(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
 
-    # weak scaling: every rank traces its own frame of the workload (its own jitter seed); rays are
-    # independent, so there is no exchange step
+    # Rays are independent, so there is no exchange step.  weak: every rank traces
+    # its own frame of the workload (its own jitter seed).  strong: ONE frame, rank g takes the rays
+    # g, g + G, g + 2G, ... (gp_workloads.shard: cost per ray varies strongly over the image, cyclic
+    # interleave balances it); each rank runs its own work counter into its own buffers.
     w = W.workload(args.workload)
-    w["camera"]["jitter_seed"] = int(w["camera"].get("jitter_seed", 0)) + rank
+    strong = args.scaling == "strong" and world > 1
+    if not strong:
+        w["camera"]["jitter_seed"] = int(w["camera"].get("jitter_seed", 0)) + rank
     fp32 = args.precision == "fp32"
     if fp32:
         if w["cfg"]["scheme"] == 2:
             raise SystemExit("bench.py: --precision fp32 exists for the fixed-step RK4 workloads only")
         w["cfg"]["precision"] = 1
-    n = W.n_rays(w)
+    n_frame = W.n_rays(w)
+    sel = W.shard(w, rank, world) if strong else W.ray_selection(w)
+    n = sel[1]                      # rays this rank traces per step
     mid = w["metric"]["id"]
-    ms, cs, gs = gp.api.metric_struct(w["metric"]), gp.api.camera_struct(w["camera"]), gp.api.cfg_struct(w["cfg"])
+    ms, cs, gs = gp.api.metric_struct(w["metric"]), gp.api.camera_struct(w["camera"], *sel), gp.api.cfg_struct(w["cfg"])
     disk_on = gs.max_crossings > 0
     rays = torch.empty(n * 128, dtype=torch.uint8, device=dev)
     disk = torch.empty(n * 48, dtype=torch.uint8, device=dev) if disk_on else None
@@ -263,7 +297,7 @@ def run_b200(args):
     barrier()
     clocks = sampler.stop() if rank == 0 else None
     total_ms = ev[0].elapsed_time(ev[-1])
-    per_launch_ms = [ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps)]
+    per_launch_ms = sorted(ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps))
     cnt = counters.cpu().numpy().view("<u8")
     assert int(cnt[1]) == n, "every ray must finish exactly once"
     attempts, n_rhs = int(cnt[2]), int(cnt[3])
@@ -271,6 +305,32 @@ def run_b200(args):
     if world > 1:
         dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
     total_ms_max = float(tmax.item())
+
+    # ---- back to back ("also time 8 back-to-back images"): the same frame traced B
+    # times on two streams into two sets of buffers, so that the end-of-image tail of one launch (lanes
+    # going idle once the work counter is exhausted, `tail` below) overlaps the start of the next.
+    # Reported beside `value`, which stays the one-launch-at-a-time figure. ----
+    b2b = None
+    if args.back_to_back >= 2 and world == 1:
+        streams = [stream, torch.cuda.Stream(device=dev)]
+        bufs = [(rays, disk, counters),
+                (torch.empty_like(rays), torch.empty_like(disk) if disk_on else None, torch.zeros_like(counters))]
+        torch.cuda.synchronize(dev)
+        for rep in range(2):            # first pass warms the second stream
+            t_ev0, t_ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            t_ev0.record(streams[0])
+            streams[1].wait_event(t_ev0)
+            for i in range(args.back_to_back):
+                r_, d_, c_ = bufs[i % 2]
+                gp.gp_trace(mid, ms, cs, gs, r_, d_, c_, streams[i % 2])
+            streams[0].wait_stream(streams[1])
+            t_ev1.record(streams[0])
+            t_ev1.synchronize()
+            b2b_ms = t_ev0.elapsed_time(t_ev1) / args.back_to_back
+        for _, _, c_ in bufs:
+            assert int(c_.cpu().numpy().view("<u8")[1]) == n
+        b2b = {"images": args.back_to_back, "streams": 2, "ms_per_image": b2b_ms,
+               "geodesics_per_s": n / (b2b_ms * 1e-3)}
 
     # ---- end to end: gp_trace_host into pinned host buffers (alloc + kernel + D2H + sync) ----
     e2e = None
@@ -291,7 +351,7 @@ def run_b200(args):
         if world > 1:
             dist.all_reduce(dt, op=dist.ReduceOp.MAX)
         assert int(h_cnt[1]) == n and int((h_rays["status"] <= 4).sum()) == n
-        e2e = {"value": world * n * k_e2e / float(dt.item()), "unit": "geodesics/s",
+        e2e = {"value": (n_frame if strong else world * n) * k_e2e / float(dt.item()), "unit": "geodesics/s",
                "h2d_bytes_per_step": 24 + 120 + 112,  # the three parameter structs, as kernel arguments
                "d2h_bytes_per_step": n * 128 + (n * 48 if disk_on else 0) + 64,
                "steps": k_e2e, "call": "gp_trace_host (pinned host records, stream sync inside)"}
@@ -302,10 +362,15 @@ def run_b200(args):
         return
 
     sec = total_ms_max * 1e-3
-    value = world * n * args.steps / sec
+    n_job = n_frame if strong else world * n          # rays all ranks trace per step
+    value = n_job * args.steps / sec
     kern_ms = sum(per_launch_ms) / len(per_launch_ms)
     flops = alg_flops(w, attempts, n_rhs)
     achieved = flops / (kern_ms * 1e-3) / 1e12
+    achieved_builder = alg_flops(w, attempts, n_rhs, builder=True) / (kern_ms * 1e-3) / 1e12
+    prof = PROFILED.get((args.workload, args.precision),
+                        {"hw_fp64_frac": None, "traffic": None,
+                         "source": "no ncu capture of this workload / precision under profiles/"})
     props = torch.cuda.get_device_properties(dev)
     sm_max = (clocks or {}).get("sm_max_mhz") or 1965.0
     lanes = FP32_LANES_PER_SM if fp32 else FP64_LANES_PER_SM
@@ -315,36 +380,46 @@ def run_b200(args):
                   else f"geodesics/sec ({args.workload})",
         "value": value, "unit": "geodesics/s", "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": total_ms_max / args.steps,
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32" if fp32 else "f64",
-        "data": "synthetic", "config": config_of(w, world),
-        "rhs_evals_per_s": world * n_rhs * args.steps / sec,
+        # per-launch CUDA-event times of this rank over the timed region (best and median)
+        "ms_per_step_best": per_launch_ms[0], "ms_per_step_median": per_launch_ms[len(per_launch_ms) // 2],
+        "higher_is_better": True, "scaling": "strong" if strong else "weak", "vs_baseline": None,
+        "dtype": "f32" if fp32 else "f64",
+        "data": "synthetic",
+        "config": config_of(w, world, {"parallelism": f"cyclic_shards{world}", "rays_per_step_per_gpu": n} if strong else None),
+        "rhs_evals_per_s": world * n_rhs * args.steps / sec,      # rank 0's count x ranks
         "steps_per_ray": attempts / n, "rhs_per_ray": n_rhs / n,
         "roofline": {"bound": "alu", "kernel": "trace_dp54" if gs.scheme == 2 else "trace_rk4",
                      "achieved": achieved, "peak": peak_nominal, "unit": "TFLOP/s",
                      "frac": achieved / peak_nominal,
-                     # dram__bytes_read.sum + dram__bytes_write.sum of one headline launch, from the
-                     # ncu --set full capture summarised in profiles/trace_dp54_r01f.md
-                     "traffic": 8.32e7 if args.workload == "headline" else None,
+                     "flop_model": f"SURVEY.md 8(d): {F_RHS[mid]:.0f}/RHS + {F_STEP[gs.scheme]:.0f}/step",
+                     "frac_builder_model": achieved_builder / peak_nominal,
+                     "builder_model": f"{F_RHS_BUILDER[mid]:.0f}/RHS + {F_STEP_BUILDER[gs.scheme]:.0f}/step (DESIGN.md 6.2)",
+                     # not measurable inside a timed run: from the ncu --set full capture named in `profile`
+                     # (dram__bytes_read.sum + dram__bytes_write.sum per launch; (2 DFMA + DMUL + DADD) / cycle
+                     # over 148 SMs x 128 flop / cycle)
+                     "traffic": prof["traffic"], "hw_fp64_frac": prof["hw_fp64_frac"], "profile": prof["source"],
                      "peak_kind": f"nominal {'FP32' if fp32 else 'FP64'} FMA: {props.multi_processor_count} SMs x "
                                   f"{lanes} lanes x 2 x {sm_max:.0f} MHz",
                      "peak_probe": None if fp32 else peak_probe,
                      "frac_of_probe": None if fp32 else (achieved / peak_probe if peak_probe else None),
                      "probe_kind": "gp_probe_fp64_fma: register-resident DFMA chains, same process",
-                     "alg_flops_per_launch": flops, "kernel_ms": kern_ms,
-                     "flop_model": f"{F_RHS[mid]:.0f}/RHS + {F_STEP[gs.scheme]:.0f}/step (DESIGN.md 6.2)"},
+                     "alg_flops_per_launch": flops, "kernel_ms": kern_ms},
         "clocks": clocks, "gpu_launches": args.steps,
         # end-of-image tail of the persistent kernel, from the device time stamps of the last launch
         # (gp.h counters[4..7]): steady-state rate = 99 % of the rays / time until they had finished
         "tail": {"kernel_ms": (int(cnt[7]) - int(cnt[4])) * 1e-6,
                  "t99_ms": (int(cnt[5]) - int(cnt[4])) * 1e-6 if int(cnt[5]) else None,
-                 "steady_geodesics_per_s": (world * (n - n // 100) / ((int(cnt[5]) - int(cnt[4])) * 1e-9)
+                 "steady_geodesics_per_s": ((n - n // 100) / ((int(cnt[5]) - int(cnt[4])) * 1e-9)
                                             if int(cnt[5]) > int(cnt[4]) else None)},
     }
+    if b2b:
+        out["back_to_back"] = b2b
     if e2e:
         out["e2e"] = e2e
     if not args.no_cpu_baseline and world == 1:
-        cpu = oracle_sample(w, args.cpu_seconds)
-        out["cpu_baseline"] = {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample", "rhs_evals_per_s")}
+        cpu = oracle_sample(w, args.cpu_seconds, single_thread_seconds=3.0)
+        out["cpu_baseline"] = {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample", "rhs_evals_per_s",
+                                                   "single_thread")}
     print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()

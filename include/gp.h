@@ -176,7 +176,10 @@ enum {
 
 /* The hot path (BASELINE.json north_star): trace camera->ray_count rays and write one
  * gp_ray_record (and gp_disk_record) per ray.  out->* are DEVICE pointers.
- * Returns GP_OK or a GP_E_* code; on error nothing has been enqueued.                   */
+ * Returns GP_OK or a GP_E_* code.  On a validation error (every code but GP_E_CUDA) nothing has
+ * been enqueued; GP_E_CUDA (the launch itself was refused) may leave the 64-byte memset of
+ * `counters` enqueued.  Occupancy and SM count are cached per device id under a mutex: any
+ * number of devices and host threads may call concurrently.                              */
 int gp_trace(int metric_id, const gp_metric_params *metric, const gp_camera *camera,
              const gp_integrator_cfg *cfg, const gp_out_buffers *out, void *cuda_stream);
 
@@ -185,9 +188,10 @@ int gp_trace(int metric_id, const gp_metric_params *metric, const gp_camera *cam
  * by the kernel itself, record by record as the rays end, so the transfer overlaps the tracing;
  * pageable buffers are staged through device scratch from a library-owned stream-ordered pool and
  * copied back.  Either way the stream is SYNCHRONISED before returning.  This is the end-to-end
- * call bench.py times.  (One device per process and one call at a time: the scratch pool and the
- * 64-byte device counters are library-owned and belong to the device current at the first call;
- * gp_trace itself owns nothing and may run concurrently on different streams and buffers.)      */
+ * call bench.py times.  Re-entrant: the 64-byte device counters (and the staging scratch) are
+ * allocated per call, stream-ordered, from a library-owned pool that exists once per device
+ * (created under a mutex on first use, kept for the life of the process), so concurrent calls
+ * on different streams, host threads and devices are independent.                               */
 int gp_trace_host(int metric_id, const gp_metric_params *metric, const gp_camera *camera,
                   const gp_integrator_cfg *cfg, const gp_out_buffers *out, void *cuda_stream);
 
@@ -259,6 +263,8 @@ typedef struct gp_shade_cfg {
   double g_lo, g_hi;
 } gp_shade_cfg;
 
+/* Alignment (GP_E_BAD_PARAM otherwise): rays 16 bytes (128-bit loads; the buffers gp_trace accepts are
+ * 32-byte aligned), disk 8 bytes, rgba8 4 bytes (one 32-bit store per pixel).                      */
 int gp_shade(const gp_shade_cfg *cfg, const void *rays, size_t rays_bytes, const void *disk,
              size_t disk_bytes, void *rgba8, size_t rgba_bytes, void *cuda_stream);
 
@@ -274,7 +280,9 @@ int gp_shade(const gp_shade_cfg *cfg, const void *rays, size_t rays_bytes, const
  * (t, r, theta, phi, p_r, p_theta, 2H, lambda), NaN after an orbit ended early.  status: DEVICE n
  * uint32 (GP_RAY_ESCAPED = reached lambda_end, GP_RAY_CAPTURED = r < r_H (1 + eps_capture),
  * GP_RAY_MAXSTEPS, GP_RAY_STEP_UNDERFLOW).  n_steps: DEVICE n uint64 attempted steps.
- * GP_E_BAD_PARAM on non-positive rtol, h0, h_max, lambda_end, n_samples, negative atol / max_steps. */
+ * GP_E_BAD_PARAM on non-positive rtol, h0, h_max, lambda_end, n_samples, negative atol / max_steps,
+ * and on misaligned buffers: samples must be 32-byte aligned (written with 256-bit stores), states8 and
+ * n_steps 8-byte, status 4-byte.                                                                      */
 typedef struct gp_orbit_cfg {
   double rtol, atol, h0, h_max, lambda_end, eps_capture;
   int64_t n_samples, max_steps;

@@ -200,6 +200,32 @@ int make_params(int metric_id, const gp_metric_params *m, const gp_camera *cam, 
   return GP_OK;
 }
 
+// ---- library-owned scratch for gp_trace_host -----------------------------------------------------
+// One stream-ordered pool per device that keeps its memory between calls (release threshold = max): the
+// default pool would hand 128 MiB back to the driver at every synchronisation and pay cudaMalloc again
+// on the next call.  Created on first use under a mutex; allocations from it are per call.
+int scratch_pool(cudaMemPool_t *out) {
+  static cudaMemPool_t pools[64] = {};
+  static std::mutex mu;
+  int dev = 0;
+  GP_CUDA(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= 64) return GP_E_UNSUPPORTED;
+  std::lock_guard<std::mutex> lock(mu);
+  if (!pools[dev]) {
+    cudaMemPoolProps props = {};
+    props.allocType = cudaMemAllocationTypePinned;
+    props.location.type = cudaMemLocationTypeDevice;
+    props.location.id = dev;
+    cudaMemPool_t p = nullptr;
+    GP_CUDA(cudaMemPoolCreate(&p, &props));
+    unsigned long long keep = ~0ull;
+    GP_CUDA(cudaMemPoolSetAttribute(p, cudaMemPoolAttrReleaseThreshold, &keep));
+    pools[dev] = p;
+  }
+  *out = pools[dev];
+  return GP_OK;
+}
+
 // ---- launch -----------------------------------------------------------------------------------
 // Resident blocks per SM and the SM count are properties of (kernel, device): cached per device id
 // under a mutex, so that a process may drive several devices and several host threads (the cache was
@@ -377,69 +403,39 @@ int gp_trace_host(int metric_id, const gp_metric_params *metric, const gp_camera
   }
   if (out->counters && out->counters_bytes < 64) return GP_E_SIZE;
   cudaStream_t stream = (cudaStream_t)cuda_stream;
+  cudaMemPool_t pool = nullptr;
+  rc = scratch_pool(&pool);
+  if (rc) return rc;
   // Pinned (page-locked, mapped) host buffers are written by the kernel itself: a lane stores its
   // 128-byte record once, when its ray ends, so the records cross PCIe while the other rays are still
   // being integrated and no device-to-host copy remains after the kernel.  Pageable buffers take the
   // staged path below (device scratch + cudaMemcpyAsync).
-  {
-    cudaPointerAttributes ar, ad;
-    bool direct = n > 0 && cudaPointerGetAttributes(&ar, out->rays) == cudaSuccess &&
-                  ar.type == cudaMemoryTypeHost && ar.devicePointer != nullptr;
-    if (direct && disk)
-      direct = cudaPointerGetAttributes(&ad, out->disk) == cudaSuccess && ad.type == cudaMemoryTypeHost &&
-               ad.devicePointer != nullptr;
-    cudaGetLastError();  // a pageable pointer leaves cudaErrorInvalidValue behind on old drivers
-    if (direct) {
-      static unsigned long long *dcount = nullptr;   // 64-byte device counters (the work counter stays on the device)
-      if (!dcount) GP_CUDA(cudaMalloc((void **)&dcount, 64));
-      gp_out_buffers dev;
-      dev.counters = dcount;
-      dev.counters_bytes = 64;
-      dev.rays = ar.devicePointer;
-      dev.rays_bytes = rays_b;
-      dev.disk = disk ? ad.devicePointer : nullptr;
-      dev.disk_bytes = disk_b;
-      rc = gp_trace(metric_id, metric, camera, cfg, &dev, cuda_stream);
-      if (rc != GP_OK) return rc;
-      cudaError_t e = cudaSuccess;
-      if (out->counters) e = cudaMemcpyAsync(out->counters, dcount, 64, cudaMemcpyDeviceToHost, stream);
-      cudaError_t e3 = cudaStreamSynchronize(stream);
-      if (e != cudaSuccess) return cuda_fail(e);
-      if (e3 != cudaSuccess) return cuda_fail(e3);
-      return GP_OK;
-    }
-  }
-  // one scratch allocation: counters | ray records | disk records
+  cudaPointerAttributes ar, ad;
+  bool direct = n > 0 && cudaPointerGetAttributes(&ar, out->rays) == cudaSuccess &&
+                ar.type == cudaMemoryTypeHost && ar.devicePointer != nullptr;
+  if (direct && disk)
+    direct = cudaPointerGetAttributes(&ad, out->disk) == cudaSuccess && ad.type == cudaMemoryTypeHost &&
+             ad.devicePointer != nullptr;
+  cudaGetLastError();  // a pageable pointer leaves cudaErrorInvalidValue behind on old drivers
+  // one scratch allocation per call, stream-ordered: counters | ray records | disk records (the last two
+  // only on the staged path).  Nothing is shared between calls, so concurrent calls on different streams
+  // and host threads are independent.
   const size_t off_rays = 64, off_disk = off_rays + ((rays_b + 63) & ~(size_t)63);
-  // The scratch comes from a library-owned stream-ordered pool that keeps its memory between
-  // calls (release threshold = max): the default pool would hand 128 MiB back to the driver at
-  // every synchronisation and pay cudaMalloc again on the next call.
-  static cudaMemPool_t pool = nullptr;
-  if (!pool) {
-    int dev = 0;
-    GP_CUDA(cudaGetDevice(&dev));
-    cudaMemPoolProps props = {};
-    props.allocType = cudaMemAllocationTypePinned;
-    props.location.type = cudaMemLocationTypeDevice;
-    props.location.id = dev;
-    GP_CUDA(cudaMemPoolCreate(&pool, &props));
-    unsigned long long keep = ~0ull;
-    GP_CUDA(cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep));
-  }
+  const size_t scratch_b = direct ? 64 : off_disk + disk_b + 64;
   char *scratch = nullptr;
-  GP_CUDA(cudaMallocFromPoolAsync((void **)&scratch, off_disk + disk_b + 64, pool, stream));
+  GP_CUDA(cudaMallocFromPoolAsync((void **)&scratch, scratch_b, pool, stream));
   gp_out_buffers dev;
   dev.counters = scratch;
   dev.counters_bytes = 64;
-  dev.rays = scratch + off_rays;
+  dev.rays = direct ? ar.devicePointer : (void *)(scratch + off_rays);
   dev.rays_bytes = rays_b;
-  dev.disk = disk ? scratch + off_disk : nullptr;
+  dev.disk = disk ? (direct ? ad.devicePointer : (void *)(scratch + off_disk)) : nullptr;
   dev.disk_bytes = disk_b;
   rc = gp_trace(metric_id, metric, camera, cfg, &dev, cuda_stream);
   cudaError_t e = cudaSuccess;
   if (rc == GP_OK) {
-    if (n > 0) e = cudaMemcpyAsync(out->rays, dev.rays, rays_b, cudaMemcpyDeviceToHost, stream);
-    if (e == cudaSuccess && disk && n > 0)
+    if (!direct && n > 0) e = cudaMemcpyAsync(out->rays, dev.rays, rays_b, cudaMemcpyDeviceToHost, stream);
+    if (!direct && e == cudaSuccess && disk && n > 0)
       e = cudaMemcpyAsync(out->disk, dev.disk, disk_b, cudaMemcpyDeviceToHost, stream);
     if (e == cudaSuccess && out->counters)
       e = cudaMemcpyAsync(out->counters, dev.counters, 64, cudaMemcpyDeviceToHost, stream);
@@ -467,6 +463,7 @@ int gp_init_conditions(int metric_id, const gp_metric_params *metric, const gp_c
   if (!states8) return GP_E_NULL;
   if (states_bytes < n * 64) return GP_E_SIZE;
   if (alpha_beta2 && ab_bytes < n * 16) return GP_E_SIZE;
+  if (((uintptr_t)states8 & 7u) != 0 || ((uintptr_t)alpha_beta2 & 7u) != 0) return GP_E_BAD_PARAM;
   const unsigned grid = (unsigned)((n + 255) / 256);
   k_init_conditions<<<grid, 256, 0, (cudaStream_t)cuda_stream>>>(cc, mc, (double *)states8, (double *)alpha_beta2);
   GP_CUDA(cudaGetLastError());
@@ -483,6 +480,7 @@ int gp_eval_metric(int metric_id, const gp_metric_params *metric, const void *r_
   if (n == 0) return GP_OK;
   if (!r_theta2 || !out15) return GP_E_NULL;
   if (out_bytes < (size_t)n * 15 * sizeof(double)) return GP_E_SIZE;
+  if (((uintptr_t)r_theta2 & 7u) != 0 || ((uintptr_t)out15 & 7u) != 0) return GP_E_BAD_PARAM;
   const unsigned grid = (unsigned)((n + 127) / 128);
   k_eval_metric<<<grid, 128, 0, (cudaStream_t)cuda_stream>>>(metric_id, mc, (const double *)r_theta2, n,
                                                              (double *)out15);
@@ -500,6 +498,7 @@ int gp_eval_rhs(int metric_id, const gp_metric_params *metric, const void *state
   if (n == 0) return GP_OK;
   if (!states8 || !rhs6) return GP_E_NULL;
   if (rhs_bytes < (size_t)n * 6 * sizeof(double)) return GP_E_SIZE;
+  if (((uintptr_t)states8 & 7u) != 0 || ((uintptr_t)rhs6 & 7u) != 0) return GP_E_BAD_PARAM;
   const unsigned grid = (unsigned)((n + 127) / 128);
   cudaStream_t st = (cudaStream_t)cuda_stream;
   if (metric_id == GP_SCHWARZSCHILD)
@@ -545,6 +544,10 @@ int gp_integrate_orbits(int metric_id, const gp_metric_params *metric, const gp_
   if (samples_bytes < (size_t)n * (size_t)cfg->n_samples * 64 || status_bytes < (size_t)n * 4 ||
       n_steps_bytes < (size_t)n * 8)
     return GP_E_SIZE;
+  // samples are written with 256-bit stores, states read as doubles, status / n_steps as 32 / 64-bit words
+  if (((uintptr_t)samples & 31u) != 0 || ((uintptr_t)states8 & 7u) != 0 || ((uintptr_t)status & 3u) != 0 ||
+      ((uintptr_t)n_steps & 7u) != 0)
+    return GP_E_BAD_PARAM;
   P.rtol = cfg->rtol; P.atol = cfg->atol; P.h0 = cfg->h0; P.h_max = cfg->h_max; P.lambda_end = cfg->lambda_end;
   P.r_cap = P.mc.r_horizon * (1.0 + cfg->eps_capture);
   P.n = n; P.n_samples = cfg->n_samples; P.max_steps = cfg->max_steps;
@@ -584,6 +587,9 @@ int gp_shade(const gp_shade_cfg *cfg, const void *rays, size_t rays_bytes, const
   if (rays_bytes < n * sizeof(gp_ray_record)) return GP_E_SIZE;
   if (cfg->disk_overlay && disk_bytes < n * sizeof(gp_disk_record)) return GP_E_SIZE;
   if (rgba_bytes < npix * 4) return GP_E_SIZE;
+  // records are read with 128-bit loads, disk records as doubles, pixels written as 32-bit words
+  if (((uintptr_t)rays & 15u) != 0 || ((uintptr_t)rgba8 & 3u) != 0 || (cfg->disk_overlay && ((uintptr_t)disk & 7u) != 0))
+    return GP_E_BAD_PARAM;
   ShadeParams P;
   memset(&P, 0, sizeof(P));
   P.W = cfg->width; P.H = cfg->height; P.S = S;

@@ -196,3 +196,45 @@ def test_shade_and_orbit_validation_is_synchronous():
     assert orb(good, metric=api.gp_metric_params(1.0, 1.5, 0.0)) == api.GP_E_BAD_PARAM
     assert orb(good, n=0) == api.GP_OK            # nothing to do, nothing enqueued
     assert orb(good, n=-1) == api.GP_E_BAD_PARAM
+
+
+def test_alignment_is_validated_before_anything_is_enqueued():
+    """A misaligned caller buffer would raise a sticky misaligned-address fault inside a kernel that uses
+    vector loads / stores; every entry point refuses it synchronously instead (GP_E_BAD_PARAM)."""
+    vp = C.c_void_p
+    ok = api.shade_struct(dict(width=4, height=4, mode=0))
+    shade = lambda rays=0x1000, disk=None, out=0x2000, cfg=ok: api.lib.gp_shade(
+        C.byref(cfg), vp(rays), 16 * 128, vp(disk) if disk else None, 16 * 48 if disk else 0, vp(out), 64, None)
+    assert shade(rays=0x1008) == api.GP_E_BAD_PARAM            # records are read with 128-bit loads
+    assert shade(out=0x2002) == api.GP_E_BAD_PARAM             # one 32-bit store per pixel
+    ov = api.shade_struct(dict(width=4, height=4, mode=0, disk_overlay=1))
+    assert shade(disk=0x3004, cfg=ov) == api.GP_E_BAD_PARAM
+    m = api.gp_metric_params(1.0, 0.9, 0.0)
+    good = api.orbit_struct(dict(rtol=1e-9, atol=1e-9, h0=0.1, h_max=1.0, lambda_end=10.0, n_samples=4))
+    orb = lambda st=0x1000, sa=0x2000, stat=0x3000, ns=0x4000: api.lib.gp_integrate_orbits(
+        api.GP_KERR, C.byref(m), C.byref(good), vp(st), 2, vp(sa), 2 * 4 * 64, vp(stat), 8, vp(ns), 16, None)
+    assert orb(sa=0x2010) == api.GP_E_BAD_PARAM                # samples: st.global.v4.f64, 32-byte aligned
+    assert orb(sa=0x2008) == api.GP_E_BAD_PARAM
+    assert orb(st=0x1004) == api.GP_E_BAD_PARAM
+    assert orb(stat=0x3002) == api.GP_E_BAD_PARAM
+    assert orb(ns=0x4004) == api.GP_E_BAD_PARAM
+    # step-level entry points
+    w = W.workload("C2")
+    cam = api.camera_struct(w["camera"], 0, 8, 1)
+    assert api.lib.gp_init_conditions(1, C.byref(m), C.byref(cam), vp(0x1004), 8 * 64, None, 0, None) == api.GP_E_BAD_PARAM
+    assert api.lib.gp_init_conditions(1, C.byref(m), C.byref(cam), vp(0x1000), 8 * 64, vp(0x2004), 8 * 16, None) == api.GP_E_BAD_PARAM
+    assert api.lib.gp_eval_metric(1, C.byref(m), vp(0x1004), 4, vp(0x2000), 4 * 120, None) == api.GP_E_BAD_PARAM
+    assert api.lib.gp_eval_rhs(1, C.byref(m), vp(0x1000), 4, vp(0x2004), 4 * 48, None) == api.GP_E_BAD_PARAM
+    # gp_trace: records 32-byte, disk and counters 8-byte
+    for out in (api.gp_out_buffers(vp(0x1010), 64 * 128, vp(0x2000), 64 * 48, vp(0x3000), 64),
+                api.gp_out_buffers(vp(0x1000), 64 * 128, vp(0x2004), 64 * 48, vp(0x3000), 64),
+                api.gp_out_buffers(vp(0x1000), 64 * 128, vp(0x2000), 64 * 48, vp(0x3004), 64)):
+        assert _call(W.workload("C3"), out=out) == api.GP_E_BAD_PARAM
+
+
+def test_no_tuning_hooks_or_process_wide_device_state_in_the_product():
+    """The launch path reads no environment variable, and what it caches is keyed by device id."""
+    src = open(os.path.join(ROOT, "paper_2310_15183_b200", "csrc", "gp_api.cu")).read()
+    assert "getenv" not in src
+    assert "static unsigned long long *dcount" not in src and "static cudaMemPool_t pool =" not in src
+    assert "cache[kMaxDevices]" in src and "std::mutex" in src

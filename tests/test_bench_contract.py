@@ -38,7 +38,13 @@ def test_cuda_arm_line():
     assert BASE | {"roofline", "cpu_baseline", "clocks", "gpu_launches", "tail"} <= set(d)
     r = d["roofline"]
     assert r["bound"] == "alu" and r["unit"] == "TFLOP/s" and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12
-    assert r["traffic"] and d["gpu_launches"] == 3 and d["n_gpus"] == 1 and d["scaling"] == "weak"
+    assert d["gpu_launches"] == 3 and d["n_gpus"] == 1 and d["scaling"] == "weak"
+    # both flop models, best and median, the counter evidence with its source
+    assert "SURVEY.md 8(d): 70/RHS + 330/step" in r["flop_model"] and r["frac_builder_model"] > r["frac"]
+    assert r["profile"] and os.path.exists(os.path.join(ROOT, r["profile"])) and r["traffic"] and 0.3 < r["hw_fp64_frac"] < 1.0
+    assert d["ms_per_step_best"] <= d["ms_per_step_median"] <= 1.5 * d["ms_per_step"]
+    assert d["back_to_back"]["images"] == 8 and d["back_to_back"]["ms_per_image"] < 1.05 * d["ms_per_step"]
+    assert d["cpu_baseline"]["single_thread"]["value"] < d["cpu_baseline"]["value"]
     assert d["config"]["workload"] == "headline" and d["dtype"] == "f64"
     assert d["e2e"]["d2h_bytes_per_step"] >= 1024 * 1024 * 128 and d["e2e"]["value"] > 0.5 * d["value"]
     assert d["cpu_baseline"]["kind"] == "oracle" and d["value"] > 100 * d["cpu_baseline"]["value"]

@@ -675,3 +675,49 @@ def test_concurrent_traces_on_two_streams(gp):
         got = rays.cpu().numpy().view(gp.api.RAY_DTYPE)
         assert got.tobytes() == r.tobytes()
         assert cnt.cpu().numpy().view("<u8")[1] == len(r)
+
+
+def test_trace_host_is_reentrant_across_host_threads(gp):
+    """gp_trace_host allocates its device counters (and staging scratch) per call from a per-device pool:
+    two host threads on two streams, one with pinned and one with pageable buffers, get the records of
+    the same calls made one after the other (include/gp.h)."""
+    import threading
+    import torch
+    specs = [("C2", 3, 6000, 17, True), ("C3", 5, 6000, 53, False)]
+    ref, outs, errs = [], [None] * len(specs), []
+    for n, b, c, s, _ in specs:
+        r, d, _ = gp.api.trace_workload(W.workload(n), b, c, s)
+        ref.append((r, d))
+
+    def work(i):
+        try:
+            n, b, c, s, pinned = specs[i]
+            w = W.workload(n)
+            stream = torch.cuda.Stream()
+            disk = w["cfg"]["max_crossings"] > 0
+            for _ in range(3):
+                if pinned:
+                    rays = torch.zeros(c * 128, dtype=torch.uint8, pin_memory=True).numpy().view(gp.api.RAY_DTYPE)
+                    dsk = torch.zeros(c * 48, dtype=torch.uint8, pin_memory=True).numpy().view(gp.api.DISK_DTYPE) if disk else None
+                else:
+                    rays = np.zeros(c, dtype=gp.api.RAY_DTYPE)
+                    dsk = np.zeros(c, dtype=gp.api.DISK_DTYPE) if disk else None
+                cnt = np.zeros(8, dtype=np.uint64)
+                gp.gp_trace_host(w["metric"]["id"], gp.api.metric_struct(w["metric"]),
+                                 gp.api.camera_struct(w["camera"], b, c, s), gp.api.cfg_struct(w["cfg"]),
+                                 rays, dsk, cnt, stream)
+                outs[i] = (rays.copy(), None if dsk is None else dsk.copy(), cnt.copy())
+        except Exception as e:   # surfaced below
+            errs.append(e)
+
+    threads = [threading.Thread(target=work, args=(i,)) for i in range(len(specs))]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert not errs, errs
+    for (r, d), (gr, gd, cnt), (n, b, c, s, _) in zip(ref, outs, specs):
+        assert gr.tobytes() == r.tobytes()
+        if d is not None and gd is not None:
+            assert gd.tobytes() == d.tobytes()
+        assert cnt[1] == c
