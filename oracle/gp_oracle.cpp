@@ -640,8 +640,10 @@ void trace_ray(const orc_metric *m, const orc_camera *cam, const orc_cfg *cfg, d
   const double r_cap = horizon_radius(m) * (1.0 + cfg->eps_capture);
   const double r_esc = cfg->r_escape;
   const bool disk_on = cfg->max_crossings > 0;
+  const bool ring_on = cfg->ring_half_angle > 0.0;
+  const double ring_d = cfg->ring_half_angle;
   double r_in = cfg->disk_r_in, r_out = cfg->disk_r_out;
-  if (disk_on && r_in <= 0.0) r_in = isco_radius(m);
+  if ((disk_on || ring_on) && r_in <= 0.0) r_in = isco_radius(m);
   Monitors mo;
   mo.h_max = 0.0;
   mo.q_drift = 0.0;
@@ -737,6 +739,49 @@ void trace_ray(const orc_metric *m, const orc_camera *cam, const orc_cfg *cfg, d
       for (int i = 0; i < 6; ++i) y[i] = yl[i];
       lam = laml;
       break;
+    }
+    // Solid ring ("collision is based on the ray propagating to a point inside volume of the
+    // object"; reading R39).  Volume: r_in <= r <= r_out, |theta - pi/2| <= d, a box in (r, theta).
+    // An accepted, non-terminal step y_n -> y_{n+1} (y_n outside the volume) can meet it only if every
+    // coordinate that starts outside its interval ENTERS it during the step (ends inside it or beyond
+    // it).  Then the entry point is LOCATED with the landing step of R14 from y_n, on the face of each such
+    // coordinate on y_n's side: the theta-face first — a hit if the landed radius is in range — else the
+    // radial face — a hit if the landed theta is inside the slab.  (For a ray that enters the box, the
+    // later of the two face crossings is the entry and only there is the other coordinate in range.)
+    // This contains the paper's test (y_{n+1} inside) and does not depend on the step size for a slab
+    // or a corner crossed within one step.
+    if (ring_on) {
+      const double un = y[2] - kHalfPi, un1 = ynew[2] - kHalfPi;
+      const bool th_out = std::fabs(un) > ring_d;
+      const bool r_out_n = !(y[1] >= r_in && y[1] <= r_out);
+      const bool th_enters = std::fabs(un1) <= ring_d || un * un1 < 0.0;
+      const bool r_enters = (ynew[1] >= r_in && ynew[1] <= r_out) || (y[1] < r_in) != (ynew[1] < r_in);
+      double yl[6], laml;
+      bool hit = false;
+      if ((th_out || r_out_n) && (!th_out || th_enters) && (!r_out_n || r_enters)) {
+        if (th_out) {
+          landing_step(S, scheme, 2, y, lam, kHalfPi + (un > 0.0 ? ring_d : -ring_d), yl, &laml);
+          ++n_land;
+          hit = yl[1] >= r_in && yl[1] <= r_out;
+        }
+        if (!hit && r_out_n) {
+          landing_step(S, scheme, 1, y, lam, (y[1] < r_in) ? r_in : r_out, yl, &laml);
+          ++n_land;
+          hit = std::fabs(yl[2] - kHalfPi) <= ring_d;
+        }
+      }
+      if (hit) {
+        double kp[3] = {NaN, NaN, NaN};
+        if (m->id == 2) kepler_general(m, yl[1], S.pt, S.pphi, kp);
+        else kepler(m, yl[1], S.pt, S.pphi, kp);
+        rec->disk_r[0] = yl[1];
+        rec->disk_g[0] = kp[2];
+        n_rec = 1;
+        for (int i = 0; i < 6; ++i) y[i] = yl[i];
+        lam = laml;
+        status = 5;
+        break;
+      }
     }
     // O7: equator crossing on an accepted, non-terminal step (R19)
     if ((y[2] - kHalfPi) * (ynew[2] - kHalfPi) < 0.0) {
@@ -915,6 +960,10 @@ static int valid_run(const orc_metric *m, const orc_camera *cam, const orc_cfg *
   if (!valid_metric(m) || !cam || !cfg) return 0;
   if (cfg->scheme < 0 || cfg->scheme > 2) return 0;
   if (cfg->max_crossings < 0 || cfg->max_crossings > 3) return 0;
+  if (!(cfg->ring_half_angle >= 0.0) || cfg->ring_half_angle >= 1.5) return 0;
+  if (cfg->ring_half_angle > 0.0 && (cfg->max_crossings > 0 || cfg->scheme != 2 || !(cfg->disk_r_out >= cfg->disk_r_in)))
+    return 0;   // the ring replaces the thin disk; located hits are built for the adaptive scheme
+  if (cfg->ring_half_angle > 0.0 && m->id == 2 && !(cfg->disk_r_in > 0.0)) return 0;
   if (cfg->max_crossings > 0 && m->id == 2 && !(cfg->disk_r_in > 0.0)) return 0;  // no ISCO formula for Manko-Novikov
   if (cam->width <= 0 || cam->height <= 0 || cam->supersample <= 0) return 0;
   return 1;

@@ -51,9 +51,15 @@ typedef struct orc_cfg {
   double eps_capture, r_escape;
   double disk_r_in, disk_r_out;
   int64_t max_crossings;
+  /* > 0: a solid ring (Fig 15-17: "a region in space around the equator of non-zero
+   * thickness", hit when "the ray propagat[es] to a point inside the volume"): the set
+   * disk_r_in <= r <= disk_r_out, |theta - pi/2| <= ring_half_angle.  Opaque: the ray ends there with
+   * status 5, located on the face it entered through (see trace_ray); disk_r[0], disk_g[0] = hit radius
+   * and redshift factor of the circular equatorial emitter at that radius.  Needs max_crossings = 0. */
+  double ring_half_angle;
 } orc_cfg;
 
-/* status: 0 escaped, 1 captured, 2 max steps, 3 non-finite, 4 step underflow */
+/* status: 0 escaped, 1 captured, 2 max steps, 3 non-finite, 4 step underflow, 5 hit the ring */
 typedef struct orc_record {
   int64_t status, n_accepted, n_rejected, n_equator_crossings, n_disk_recorded, n_rhs;
   double alpha, beta;

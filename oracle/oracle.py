@@ -30,7 +30,7 @@ class OrcCfg(C.Structure):
     _fields_ = [("scheme", _i64), ("h", _f64), ("h_rel", _f64), ("rtol", _f64), ("atol", _f64),
                 ("h_cap_rel", _f64), ("max_steps", _i64), ("lambda_max", _f64),
                 ("eps_capture", _f64), ("r_escape", _f64), ("disk_r_in", _f64),
-                ("disk_r_out", _f64), ("max_crossings", _i64)]
+                ("disk_r_out", _f64), ("max_crossings", _i64), ("ring_half_angle", _f64)]
 
 
 RECORD_DTYPE = np.dtype([
@@ -120,7 +120,8 @@ def _cfg(d):
     return OrcCfg(d["scheme"], d.get("h", 0.0), d.get("h_rel", 0.0), d.get("rtol", 0.0),
                   d.get("atol", 0.0), d.get("h_cap_rel", 0.0), d["max_steps"],
                   d.get("lambda_max", 0.0), d["eps_capture"], d["r_escape"],
-                  d.get("disk_r_in", 0.0), d.get("disk_r_out", 0.0), d.get("max_crossings", 0))
+                  d.get("disk_r_in", 0.0), d.get("disk_r_out", 0.0), d.get("max_crossings", 0),
+                  d.get("ring_half_angle", 0.0))
 
 
 def _dp(a):
