@@ -25,7 +25,7 @@
 extern "C" {
 #endif
 
-#define GP_VERSION 101 /* major*10000 + minor*100 + patch */
+#define GP_VERSION 102 /* major*10000 + minor*100 + patch */
 
 /* ---- spacetimes (section 2.2) ------------------------------------------- */
 enum {
@@ -97,6 +97,21 @@ typedef struct gp_integrator_cfg {
   double disk_r_in, disk_r_out; /* thin equatorial disk; disk_r_in <= 0 -> prograde ISCO  */
   int32_t max_crossings;        /* 0..3 recorded disk crossings; 0 = disk off             */
   int32_t reserved_;
+  /* > 0: a SOLID RING instead of the thin disk (objects "cannot be infinitely thin, as
+   * their collision is based on the ray propagating to a point inside volume of the object"; L735-743,
+   * Figs 15-17: "a region in space around the equator" whose hits go "through the redshift
+   * calculation").  Volume: disk_r_in <= r <= disk_r_out, |theta - pi/2| <= ring_half_angle (a box in
+   * r, theta).  Opaque: the ray ends with status GP_RAY_HIT_RING at the point where it ENTERS the
+   * volume.  An accepted, non-terminal step y_n -> y_{n+1} is examined when every coordinate (r, theta)
+   * that starts outside its interval ends inside it or beyond it; the entry is located from y_n by the
+   * landing step of scheme 2 on the theta-face on y_n's side (a hit if the landed radius is in range),
+   * else on the radial face on y_n's side (a hit if the landed theta is in the slab); otherwise the ray
+   * goes on from y_{n+1} (reading R39).  The record holds the state at the hit; disk record
+   * slot 0 holds the hit radius and g of the circular equatorial emitter at that radius (eq 56-57), the
+   * other slots NaN.  Requires scheme 2, max_crossings = 0, a disk buffer; Manko-Novikov needs an explicit
+   * disk_r_in.  0 = no ring.  Values < 0 or >= 1.5 -> GP_E_BAD_PARAM; with scheme 0 / 1 or
+   * max_crossings > 0 -> GP_E_UNSUPPORTED.                                                              */
+  double ring_half_angle;
 } gp_integrator_cfg;
 
 /* ---- outputs ------------------------------------------------------------------------ */
@@ -105,7 +120,8 @@ enum {
   GP_RAY_CAPTURED = 1,
   GP_RAY_MAXSTEPS = 2,
   GP_RAY_NONFINITE = 3,
-  GP_RAY_STEP_UNDERFLOW = 4
+  GP_RAY_STEP_UNDERFLOW = 4,
+  GP_RAY_HIT_RING = 5 /* ended on the solid ring (cfg.ring_half_angle > 0) */
 };
 
 /* One per ray, 128 bytes.  theta and phi are raw (accumulated, not wrapped).  The traced
@@ -141,7 +157,7 @@ typedef struct gp_disk_record {
 } gp_disk_record;
 
 /* Device buffers, caller-owned.  rays: >= ray_count*sizeof(gp_ray_record), 32-byte
- * aligned.  disk: >= ray_count*sizeof(gp_disk_record) when max_crossings > 0, else may be
+ * aligned.  disk: >= ray_count*sizeof(gp_disk_record) when max_crossings > 0 or the ring is on, else may be
  * NULL.  counters: >= 64 bytes, 8-byte aligned; the library zeroes it on the stream, uses
  * word 0 as the atomic work counter and leaves totals behind:
  *   [0] work counter (>= ray_count at exit)  [1] rays finished  [2] attempted steps

@@ -14,7 +14,7 @@ from . import build as _build
 HERE = os.path.dirname(os.path.abspath(__file__))
 
 GP_SCHWARZSCHILD, GP_KERR, GP_MANKO_NOVIKOV = 0, 1, 2
-GP_RAY_ESCAPED, GP_RAY_CAPTURED, GP_RAY_MAXSTEPS, GP_RAY_NONFINITE, GP_RAY_STEP_UNDERFLOW = range(5)
+GP_RAY_ESCAPED, GP_RAY_CAPTURED, GP_RAY_MAXSTEPS, GP_RAY_NONFINITE, GP_RAY_STEP_UNDERFLOW, GP_RAY_HIT_RING = range(6)
 GP_OK, GP_E_BAD_METRIC, GP_E_BAD_PARAM, GP_E_NULL, GP_E_SIZE, GP_E_UNSUPPORTED, GP_E_CUDA = (
     0, -1, -2, -3, -4, -5, -6)
 
@@ -41,7 +41,7 @@ class gp_integrator_cfg(C.Structure):
                 ("max_steps", _i64), ("lambda_max", _f64),
                 ("eps_capture", _f64), ("r_escape", _f64),
                 ("disk_r_in", _f64), ("disk_r_out", _f64),
-                ("max_crossings", _i32), ("reserved_", _i32)]
+                ("max_crossings", _i32), ("reserved_", _i32), ("ring_half_angle", _f64)]
 
 
 class gp_shade_cfg(C.Structure):
@@ -148,7 +148,7 @@ def cfg_struct(g):
                              int(g["max_steps"]), g.get("lambda_max", 0.0),
                              g["eps_capture"], g["r_escape"],
                              g.get("disk_r_in", 0.0), g.get("disk_r_out", 0.0),
-                             int(g.get("max_crossings", 0)), 0)
+                             int(g.get("max_crossings", 0)), 0, g.get("ring_half_angle", 0.0))
 
 
 def _stream_ptr(stream):
@@ -289,7 +289,8 @@ def trace_workload(w, ray_begin=0, ray_count=None, ray_stride=1, stream=None, de
     n = cam.ray_count
     cfg = cfg_struct(w["cfg"])
     rays = torch.empty(max(n, 1) * 128, dtype=torch.uint8, device=device)
-    disk = torch.empty(max(n, 1) * 48, dtype=torch.uint8, device=device) if cfg.max_crossings > 0 else None
+    need_disk = cfg.max_crossings > 0 or cfg.ring_half_angle > 0.0
+    disk = torch.empty(max(n, 1) * 48, dtype=torch.uint8, device=device) if need_disk else None
     counters = torch.empty(64, dtype=torch.uint8, device=device)
     gp_trace(w["metric"]["id"], metric_struct(w["metric"]), cam, cfg, rays, disk, counters, stream)
     (stream or torch.cuda.current_stream()).synchronize()

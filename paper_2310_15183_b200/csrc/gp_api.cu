@@ -180,6 +180,11 @@ int make_params(int metric_id, const gp_metric_params *m, const gp_camera *cam, 
   // a Manko-Novikov disk needs an explicit inner radius: there is no ISCO formula for that metric
   if (cfg->max_crossings > 0 && metric_id == GP_MANKO_NOVIKOV && !(cfg->disk_r_in > 0.0)) return GP_E_BAD_PARAM;
   if (isnan(cfg->lambda_max)) return GP_E_BAD_PARAM;
+  // solid ring (gp.h): replaces the thin disk, located hits exist for the adaptive scheme
+  if (!(cfg->ring_half_angle >= 0.0) || !(cfg->ring_half_angle < 1.5)) return GP_E_BAD_PARAM;
+  const bool ring = cfg->ring_half_angle > 0.0;
+  if (ring && (cfg->scheme != 2 || cfg->max_crossings > 0)) return GP_E_UNSUPPORTED;
+  if (ring && metric_id == GP_MANKO_NOVIKOV && !(cfg->disk_r_in > 0.0)) return GP_E_BAD_PARAM;
   P->scheme = cfg->scheme;
   P->precision = cfg->precision;
   P->max_crossings = cfg->max_crossings;
@@ -192,7 +197,8 @@ int make_params(int metric_id, const gp_metric_params *m, const gp_camera *cam, 
   P->lambda_max = cfg->lambda_max > 0.0 ? cfg->lambda_max : (double)INFINITY;  // <= 0 = no affine budget
   P->r_cap = P->mc.r_horizon * (1.0 + cfg->eps_capture);
   P->r_esc = cfg->r_escape;
-  if (cfg->max_crossings > 0) {
+  P->ring_d = cfg->ring_half_angle;
+  if (cfg->max_crossings > 0 || ring) {
     P->disk_r_in = (cfg->disk_r_in > 0.0) ? cfg->disk_r_in : isco_prograde(metric_id, P->mc);
     P->disk_r_out = cfg->disk_r_out;
     if (!(P->disk_r_out >= P->disk_r_in)) return GP_E_BAD_PARAM;
@@ -255,12 +261,14 @@ int launch_info(Kernel kernel, size_t smem, LaunchInfo *slot, LaunchInfo *out) {
   return GP_OK;
 }
 
-template <int METRIC, bool DISK>
+// OBJ: 0 no object, 1 thin disk with recorded crossings, 2 solid ring (scheme 2 only)
+template <int METRIC, int OBJ>
 int launch_one(const TraceParams &P, cudaStream_t stream) {
+  constexpr bool DISK = (OBJ == 1);
   static LaunchInfo cache[kMaxDevices][3];   // per device: dp54, rk4 FP64, rk4 FP32 (zero-initialised)
   const bool dp54 = (P.scheme == 2);
   const bool fp32 = (P.precision == 1);
-  const size_t smem = dp54 ? dp54_smem_bytes(DISK)
+  const size_t smem = dp54 ? dp54_smem_bytes(OBJ != 0)
                            : (DISK ? (fp32 ? sizeof(float) : sizeof(double)) * kBlock * kParkSlotsRk4 : 0);
   int dev = 0;
   GP_CUDA(cudaGetDevice(&dev));
@@ -268,7 +276,7 @@ int launch_one(const TraceParams &P, cudaStream_t stream) {
   LaunchInfo *slot = &cache[dev][dp54 ? 0 : (fp32 ? 2 : 1)];
   LaunchInfo li;
   int rc;
-  if (dp54) rc = launch_info(trace_dp54<METRIC, DISK>, smem, slot, &li);
+  if (dp54) rc = launch_info(trace_dp54<METRIC, OBJ>, smem, slot, &li);
   else if (fp32) rc = launch_info(trace_rk4<METRIC, DISK, float>, smem, slot, &li);
   else rc = launch_info(trace_rk4<METRIC, DISK, double>, smem, slot, &li);
   if (rc) return rc;
@@ -278,7 +286,7 @@ int launch_one(const TraceParams &P, cudaStream_t stream) {
   if (grid > want) grid = want;
   if (grid < 1) grid = 1;
   if (dp54)
-    trace_dp54<METRIC, DISK><<<(unsigned)grid, kBlock, smem, stream>>>(P);
+    trace_dp54<METRIC, OBJ><<<(unsigned)grid, kBlock, smem, stream>>>(P);
   else if (fp32)
     trace_rk4<METRIC, DISK, float><<<(unsigned)grid, kBlock, smem, stream>>>(P);
   else
@@ -288,15 +296,15 @@ int launch_one(const TraceParams &P, cudaStream_t stream) {
 }
 
 int launch_trace(int metric_id, const TraceParams &P, cudaStream_t stream) {
-  const bool disk = P.max_crossings > 0;
+  const int obj = P.ring_d > 0.0 ? 2 : (P.max_crossings > 0 ? 1 : 0);
+#define GP_LAUNCH(M_)                                              \
+  (obj == 2 ? launch_one<M_, 2>(P, stream) : obj == 1 ? launch_one<M_, 1>(P, stream) : launch_one<M_, 0>(P, stream))
   switch (metric_id) {
-    case GP_SCHWARZSCHILD:
-      return disk ? launch_one<METRIC_SCHW, true>(P, stream) : launch_one<METRIC_SCHW, false>(P, stream);
-    case GP_KERR:
-      return disk ? launch_one<METRIC_KERR, true>(P, stream) : launch_one<METRIC_KERR, false>(P, stream);
-    default:
-      return disk ? launch_one<METRIC_MN, true>(P, stream) : launch_one<METRIC_MN, false>(P, stream);
+    case GP_SCHWARZSCHILD: return GP_LAUNCH(METRIC_SCHW);
+    case GP_KERR: return GP_LAUNCH(METRIC_KERR);
+    default: return GP_LAUNCH(METRIC_MN);
   }
+#undef GP_LAUNCH
 }
 
 // ---- step-level kernels (parity of rows a2-a5 in isolation) -------------------------------------
@@ -371,7 +379,7 @@ int gp_trace(int metric_id, const gp_metric_params *metric, const gp_camera *cam
     if (!out->rays) return GP_E_NULL;
     if (out->rays_bytes < n * sizeof(gp_ray_record)) return GP_E_SIZE;
     if (((uintptr_t)out->rays & 31u) != 0) return GP_E_BAD_PARAM;
-    if (cfg->max_crossings > 0) {
+    if (cfg->max_crossings > 0 || cfg->ring_half_angle > 0.0) {
       if (!out->disk) return GP_E_NULL;
       if (out->disk_bytes < n * sizeof(gp_disk_record)) return GP_E_SIZE;
       if (((uintptr_t)out->disk & 7u) != 0) return GP_E_BAD_PARAM;
@@ -393,7 +401,7 @@ int gp_trace_host(int metric_id, const gp_metric_params *metric, const gp_camera
   int rc = make_params(metric_id, metric, camera, cfg, &P);
   if (rc) return rc;
   const size_t n = (size_t)camera->ray_count;
-  const bool disk = cfg->max_crossings > 0;
+  const bool disk = cfg->max_crossings > 0 || cfg->ring_half_angle > 0.0;
   const size_t rays_b = n * sizeof(gp_ray_record), disk_b = disk ? n * sizeof(gp_disk_record) : 0;
   if (n > 0) {
     if (!out->rays) return GP_E_NULL;

@@ -30,6 +30,7 @@ struct TraceParams {
   double lambda_max;   // +inf when the configuration has no affine budget (cfg.lambda_max <= 0)
   double r_cap, r_esc;              // r_H (1 + eps_capture), r_escape
   double disk_r_in, disk_r_out;
+  double ring_d;                    // half opening angle of the solid ring (> 0: object kind 2)
   gp_ray_record *rays;
   gp_disk_record *disk;
   unsigned long long *counters;

@@ -62,9 +62,12 @@ __device__ __forceinline__ void lds2(unsigned a, double &x, double &y) {
   asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(x), "=d"(y) : "r"(a));
 }
 
-template <int METRIC, bool DISK>
+// OBJ: 0 no object; 1 thin disk, crossings located and recorded (R19); 2 solid ring, the ray ends where it
+// enters the volume (R39).  Both objects use the park area.
+template <int METRIC, int OBJ>
 __global__ void __launch_bounds__(kBlock, METRIC == METRIC_MN ? GP_DP54_MIN_BLOCKS_MN : GP_DP54_MIN_BLOCKS)
 trace_dp54(const __grid_constant__ TraceParams P) {
+  constexpr bool DISK = (OBJ == 1), RING = (OBJ == 2);
   extern __shared__ double2 smem2[];
   const MetricConst &mc = P.mc;
   const int tid = threadIdx.x;
@@ -91,6 +94,21 @@ trace_dp54(const __grid_constant__ TraceParams P) {
   {                                                                                            \
     double w_ = lds1(CS(C_STATE));                                                             \
     sts1(CS(C_STATE), __hiloint2double(__double2hiint(w_), (int)(code_)));                     \
+  }
+// the ray goes on from the trial state parked before a landing step (thin disk: always; ring: no hit);
+// the ring variant counts the equator crossing of that step here (the oracle counts it after its ring test)
+#define GP_RESUME_PARKED()                                                                     \
+  {                                                                                            \
+    if (RING && (th - kHalfPi) * (lds1(PS(1)) - kHalfPi) < 0.0) GP_BUMP_COUNTS(1, 0)           \
+    r = lds1(PS(0)); th = lds1(PS(1)); pr = lds1(PS(2)); pth = lds1(PS(3));                    \
+    lam = lds1(PS(6)); h = lds1(PS(7));                                                        \
+    sts1(CS(C_T), lds1(PS(4))); sts1(CS(C_PH), lds1(PS(5))); sts1(CS(C_LAM), lam);             \
+    sts1(CS(C_K1T), lds1(PS(8))); sts1(CS(C_K1PH), lds1(PS(11)));                              \
+    GP_SET_K1(lds1(PS(9)), lds1(PS(10)), lds1(PS(12)), lds1(PS(13)))                           \
+    { double rs_, rc_; sincos_fast(th, &rs_, &rc_); GP_SET_SC(rs_, rc_) }                      \
+    monH = lds1(PS(14)); monQ = lds1(PS(15)); monS = lds1(PS(16));                             \
+    mode = MODE_NORMAL;                                                                        \
+    moved = true;                                                                              \
   }
 #define GP_BUMP_COUNTS(dcross_, dland_)                                                        \
   {                                                                                            \
@@ -200,22 +218,53 @@ trace_dp54(const __grid_constant__ TraceParams P) {
               mode = MODE_LAND_R;
             } else {
               bool commit = true;
-              if ((th - kHalfPi) * (nth - kHalfPi) < 0.0) {
+              // park the accepted trial state (and F there) so that the ray can resume from it after a
+              // landing step located something on the way from y_n
+#define GP_PARK()                                                                        \
+  {                                                                                      \
+    sts1(PS(0), nr); sts1(PS(1), nth); sts1(PS(2), npr); sts1(PS(3), npth);              \
+    sts1(PS(4), nt); sts1(PS(5), nph); sts1(PS(6), lam + h); sts1(PS(7), hnext);         \
+    sts1(PS(8), o7.dt); sts1(PS(9), o7.dr); sts1(PS(10), o7.dth);                        \
+    sts1(PS(11), o7.dph); sts1(PS(12), o7.dpr); sts1(PS(13), o7.dpth);                   \
+    sts1(PS(14), fabs(0.5 * o7.H2));                                                     \
+    sts1(PS(15), carter_q<METRIC>(mc, pt, pph, npth, o7));                               \
+    sts1(PS(16), fabs(o7.s));                                                            \
+  }
+              bool ring_try = false;
+              if (RING) {
+                // R39: the step can meet the box r_in..r_out x |theta - pi/2| <= d only if every coordinate
+                // that starts outside its interval ends inside it or beyond it
+                const double un = th - kHalfPi, un1 = nth - kHalfPi;
+                const bool th_out = fabs(un) > P.ring_d;
+                const bool r_out_n = !(r >= P.disk_r_in && r <= P.disk_r_out);
+                const bool th_enters = fabs(un1) <= P.ring_d || un * un1 < 0.0;
+                const bool r_enters = (nr >= P.disk_r_in && nr <= P.disk_r_out) || ((r < P.disk_r_in) != (nr < P.disk_r_in));
+                ring_try = (th_out || r_out_n) && (!th_out || th_enters) && (!r_out_n || r_enters);
+                if (ring_try) {
+                  GP_PARK()
+                  if (th_out) {
+                    sts1(CS(C_TARGET), kHalfPi + (un > 0.0 ? P.ring_d : -P.ring_d));
+                    mode = MODE_LAND_TH;
+                  } else {
+                    GP_SET_STATUS(GP_RAY_HIT_RING)
+                    sts1(CS(C_TARGET), (r < P.disk_r_in) ? P.disk_r_in : P.disk_r_out);
+                    mode = MODE_LAND_R;
+                  }
+                  commit = false;
+                }
+              }
+              // (ring variant: a step under examination counts its equator crossing when it resumes)
+              if (!ring_try && (th - kHalfPi) * (nth - kHalfPi) < 0.0) {
                 GP_BUMP_COUNTS(1, 0)
                 if (DISK && (unsigned)__double2hiint(lds1(CS(C_STATE))) < (unsigned)P.max_crossings) {
                   // O7: locate the crossing from y_n; resume from the parked trial state afterwards
-                  sts1(PS(0), nr); sts1(PS(1), nth); sts1(PS(2), npr); sts1(PS(3), npth);
-                  sts1(PS(4), nt); sts1(PS(5), nph); sts1(PS(6), lam + h); sts1(PS(7), hnext);
-                  sts1(PS(8), o7.dt); sts1(PS(9), o7.dr); sts1(PS(10), o7.dth);
-                  sts1(PS(11), o7.dph); sts1(PS(12), o7.dpr); sts1(PS(13), o7.dpth);
-                  sts1(PS(14), fabs(0.5 * o7.H2));
-                  sts1(PS(15), carter_q<METRIC>(mc, pt, pph, npth, o7));
-                  sts1(PS(16), fabs(o7.s));
+                  GP_PARK()
                   sts1(CS(C_TARGET), kHalfPi);
                   mode = MODE_LAND_TH;
                   commit = false;
                 }
               }
+#undef GP_PARK
               if (commit) {
                 monH = fabs(0.5 * o7.H2); monQ = carter_q<METRIC>(mc, pt, pph, npth, o7); monS = fabs(o7.s);
                 r = nr; th = nth; pr = npr; pth = npth; lam += h;
@@ -230,13 +279,50 @@ trace_dp54(const __grid_constant__ TraceParams P) {
           }
         }
       } else if (mode == MODE_LAND_R) {
-        // landed on the exit surface: the record is the landed state (R14)
-        r = lds1(CS(C_TARGET)); th = nth; pr = npr; pth = npth;
-        sts1(CS(C_T), nt); sts1(CS(C_PH), nph); sts1(CS(C_LAM), nlam);
         GP_BUMP_COUNTS(0, 1)
-        finished = true;
+        bool resume = false;
+        if (RING && __double2loint(lds1(CS(C_STATE))) == GP_RAY_HIT_RING) {
+          // radial face of the ring: a hit if the landed theta is inside the slab, else the ray goes on
+          if (fabs(nth - kHalfPi) <= P.ring_d) {
+            const long long slot = __double_as_longlong(lds1(CS(C_SLOT)));
+            const double rc = lds1(CS(C_TARGET));
+            P.disk[slot].r_cross[0] = rc;
+            P.disk[slot].g[0] = kepler_g<METRIC>(mc, rc, pt, pph);
+            sts1(CS(C_STATE), __hiloint2double(1, GP_RAY_HIT_RING));
+          } else {
+            GP_SET_STATUS(0)
+            resume = true;
+          }
+        }
+        if (!resume) {
+          // landed on the exit surface (or the ring's radial face): the record is the landed state (R14)
+          r = lds1(CS(C_TARGET)); th = nth; pr = npr; pth = npth;
+          sts1(CS(C_T), nt); sts1(CS(C_PH), nph); sts1(CS(C_LAM), nlam);
+          finished = true;
+        } else {
+          GP_RESUME_PARKED()
+        }
       } else {  // MODE_LAND_TH
         GP_BUMP_COUNTS(0, 1)
+        if (RING) {
+          // theta-face of the ring: a hit if the landed radius is in range; else try the radial face on
+          // y_n's side when r_n is outside the range; else the ray goes on from the parked state
+          if (nr >= P.disk_r_in && nr <= P.disk_r_out) {
+            const long long slot = __double_as_longlong(lds1(CS(C_SLOT)));
+            P.disk[slot].r_cross[0] = nr;
+            P.disk[slot].g[0] = kepler_g<METRIC>(mc, nr, pt, pph);
+            sts1(CS(C_STATE), __hiloint2double(1, GP_RAY_HIT_RING));
+            r = nr; th = lds1(CS(C_TARGET)); pr = npr; pth = npth;
+            sts1(CS(C_T), nt); sts1(CS(C_PH), nph); sts1(CS(C_LAM), nlam);
+            finished = true;
+          } else if (!(r >= P.disk_r_in && r <= P.disk_r_out)) {
+            GP_SET_STATUS(GP_RAY_HIT_RING)
+            sts1(CS(C_TARGET), (r < P.disk_r_in) ? P.disk_r_in : P.disk_r_out);
+            mode = MODE_LAND_R;
+          } else {
+            GP_RESUME_PARKED()
+          }
+        }
         if (DISK) {
           double rc = nr;
           if (rc >= P.disk_r_in && rc <= P.disk_r_out) {
@@ -247,16 +333,12 @@ trace_dp54(const __grid_constant__ TraceParams P) {
             P.disk[slot].g[n_rec] = kepler_g<METRIC>(mc, rc, pt, pph);
             sts1(CS(C_STATE), __hiloint2double((int)(n_rec + 1u), __double2loint(sw)));
           }
-          r = lds1(PS(0)); th = lds1(PS(1)); pr = lds1(PS(2)); pth = lds1(PS(3));
-          lam = lds1(PS(6)); h = lds1(PS(7));
-          sts1(CS(C_T), lds1(PS(4))); sts1(CS(C_PH), lds1(PS(5))); sts1(CS(C_LAM), lam);
-          sts1(CS(C_K1T), lds1(PS(8))); sts1(CS(C_K1PH), lds1(PS(11)));
-          GP_SET_K1(lds1(PS(9)), lds1(PS(10)), lds1(PS(12)), lds1(PS(13)))
-          { double rs, rc; sincos_fast(th, &rs, &rc); GP_SET_SC(rs, rc) }   // once per recorded crossing
-          monH = lds1(PS(14)); monQ = lds1(PS(15)); monS = lds1(PS(16));
+          GP_RESUME_PARKED()
         }
-        mode = MODE_NORMAL;
-        moved = true;
+        if (!RING) {
+          mode = MODE_NORMAL;
+          moved = true;
+        }
       }
 
       // stop tests in the oracle's order (R18, R10 item 5), then the monitors of the new state (R22)
@@ -293,7 +375,7 @@ trace_dp54(const __grid_constant__ TraceParams P) {
         mo.sin_min = lds1(CS(C_SINMIN)); mo.err_margin = lds1(CS(C_MARGIN));
         store_record(P.rays + slot, lds1(CS(C_T)), r, th, lds1(CS(C_PH)), pr, pth, lds1(CS(C_LAM)), pt, pph, mo,
                      status, n_acc, n_rej, n_cross, n_rec, n_rhs);
-        if (DISK) {
+        if (OBJ != 0) {
           const double qnan = __longlong_as_double(0x7ff8000000000000LL);
           for (unsigned i = n_rec; i < 3u; ++i) {
             P.disk[slot].r_cross[i] = qnan;

@@ -50,12 +50,12 @@ def test_record_layouts():
     assert gp.gp_ray_record_size() == 128 == api.RAY_DTYPE.itemsize
     assert gp.gp_disk_record_size() == 48 == api.DISK_DTYPE.itemsize
     assert gp.gp_counters_size() == 64
-    assert gp.gp_version() == 101
+    assert gp.gp_version() == 102
     f = api.RAY_DTYPE.fields
     assert f["lambda"][1] == 32 and f["status"][1] == 40 and f["p_r"][1] == 48 and f["p_t"][1] == 64
     assert f["sin_theta_min"][1] == 96 and f["err_margin"][1] == 104 and f["n_rhs"][1] == 124
     assert C.sizeof(api.gp_camera) == 7 * 8 + 4 * 4 + 8 + 3 * 8 + 3 * 8 + 8
-    assert C.sizeof(api.gp_integrator_cfg) == 8 + 5 * 8 + 8 + 8 + 2 * 8 + 2 * 8 + 8
+    assert C.sizeof(api.gp_integrator_cfg) == 8 + 5 * 8 + 8 + 8 + 2 * 8 + 2 * 8 + 8 + 8
 
 
 def test_strerror():
@@ -107,6 +107,11 @@ BAD = [
     ("scheme 9", lambda m, c, g: setattr(g, "scheme", 9), None, api.GP_E_BAD_PARAM),
     ("r_escape inside r_obs", lambda m, c, g: setattr(g, "r_escape", 10.0), None, api.GP_E_BAD_PARAM),
     ("4 crossings", lambda m, c, g: setattr(g, "max_crossings", 4), None, api.GP_E_BAD_PARAM),
+    ("ring with the thin disk", lambda m, c, g: (setattr(g, "ring_half_angle", 0.05), setattr(g, "max_crossings", 1)),
+     None, api.GP_E_UNSUPPORTED),
+    ("ring with a fixed-step scheme", lambda m, c, g: (setattr(g, "ring_half_angle", 0.05), setattr(g, "scheme", 1),
+                                                       setattr(g, "h_rel", 0.02)), None, api.GP_E_UNSUPPORTED),
+    ("negative ring angle", lambda m, c, g: setattr(g, "ring_half_angle", -1.0), None, api.GP_E_BAD_PARAM),
     ("FP32 with the adaptive scheme", lambda m, c, g: setattr(g, "precision", 1), None, api.GP_E_UNSUPPORTED),
     ("precision 2", lambda m, c, g: setattr(g, "precision", 2), None, api.GP_E_UNSUPPORTED),
     ("projection 2", lambda m, c, g: setattr(c, "projection", 2), None, api.GP_E_UNSUPPORTED),

@@ -721,3 +721,100 @@ def test_trace_host_is_reentrant_across_host_threads(gp):
         if d is not None and gd is not None:
             assert gd.tobytes() == d.tobytes()
         assert cnt[1] == c
+
+
+# ---- solid ring objects (Figs 15-17; reading R39) ----------------
+def _ring(name, metric, d, r_in, r_out, **cam):
+    w = W.workload(name, **cam)
+    w["metric"] = metric
+    w["cfg"].update(max_crossings=0, disk_r_in=r_in, disk_r_out=r_out, ring_half_angle=d, max_steps=4000)
+    return w
+
+
+@pytest.mark.parametrize("label,metric,r_in,incl", [
+    ("Kerr a=0.98 (Fig 15)", dict(id=W.KERR, M=1.0, a=0.98, q=0.0), 0.0, 80.0),
+    ("Kerr a=0.98 from the equator", dict(id=W.KERR, M=1.0, a=0.98, q=0.0), 3.0, 90.0),
+    ("Manko-Novikov a=0.1 q=-2 (Figs 16-17)", dict(id=W.MANKO_NOVIKOV, M=1.0, a=0.1, q=-2.0), 5.0, 75.0)])
+def test_solid_ring_hits_match_the_oracle(gp, O, label, metric, r_in, incl):
+    """The ring is opaque: status 5 and the state at the point of entry, located on the face the ray
+    came in through; disk slot 0 = (hit radius, g).  Status bit-exact outside the flagged sets, hit
+    state 1e-9 on smooth rays, hit radius exactly on a face, g to 1e-9 (Kerr) / 1e-8 (eq 56 by duals vs
+    complex step)."""
+    w = _ring("C3", metric, 0.05, r_in, 14.0, width=256, height=256, theta_obs=math.radians(incl),
+              alpha_min=-18.0, alpha_max=18.0, beta_min=-18.0, beta_max=18.0)
+    b, c, s = W.ray_selection(w, 3, None, 5)
+    rays, disk, counters = gp.api.trace_workload(w, b, c, s)
+    orc, _ = O.trace(w, b, c, s)
+    probe, _ = O.trace(w, b, c, s, rounding_probe=True)
+    assert counters[1] == c
+    # the generic rules treat status 5 like any ended ray once it is mapped onto "ended on a surface"
+    from parity_rules import SENSITIVE_AT, flags, rel_err as re_
+    fl = flags(orc, probe)
+    gs, os_ = rays["status"].astype(np.int64), orc["status"]
+    # the hit point has its own conditioning (a ray grazing a face: dr/dtheta large), so the rounding probe
+    # is read on the hit radius and momenta as well
+    for f in ("r", "p_r", "p_theta"):
+        fl["sensitive"] = fl["sensitive"] | ((os_ == 5) & (probe["status"] == 5) & (re_(probe[f], orc[f]) > SENSITIVE_AT))
+    excused = fl["marginal"] | fl["sensitive"]
+    mism = gs != os_
+    if metric["id"] == W.MANKO_NOVIKOV:
+        mism &= ~((gs != 0) & (os_ != 0) & (gs != 5) & (os_ != 5))     # R38: which "shadow" code
+    assert not (mism & ~excused).any(), (label, int((mism & ~excused).sum()), np.flatnonzero(mism & ~excused)[:5])
+    hit = (gs == 5) & (os_ == 5)
+    assert hit.sum() > 1500, int(hit.sum())
+    smooth = hit & ~(fl["marginal"] | fl["near_axis"] | fl["sensitive"])
+    assert smooth.sum() >= 0.97 * hit.sum()
+    for f in FIELDS + ("r", "p_r", "p_theta"):
+        e = re_(rays[f], orc[f])[smooth]
+        assert e.max() <= TOL, (label, f, e.max())
+    # exactly on a face, and the face is the same one
+    on_th = np.abs(np.abs(orc["theta"] - math.pi / 2) - 0.05) <= 1e-15
+    assert np.array_equal(rays["theta"][smooth & on_th], orc["theta"][smooth & on_th])
+    assert np.array_equal(rays["r"][smooth & ~on_th], orc["r"][smooth & ~on_th])
+    assert (smooth & ~on_th).sum() >= 5 and (smooth & on_th).sum() > 1000
+    assert np.array_equal(disk["r_cross"][smooth, 0], rays["r"][smooth])
+    assert re_(disk["r_cross"][smooth, 0], orc["disk_r"][smooth, 0]).max() <= TOL
+    gtol = 1e-8 if metric["id"] == W.MANKO_NOVIKOV else TOL
+    assert re_(disk["g"][smooth, 0], orc["disk_g"][smooth, 0]).max() <= gtol
+    assert np.isnan(disk["r_cross"][:, 1:]).all() and np.isnan(disk["r_cross"][gs != 5, 0]).all()
+    assert np.array_equal(rays["n_disk_recorded"][smooth], np.ones(smooth.sum(), dtype=np.uint32))
+    for f in ("n_accepted", "n_rejected", "n_equator_crossings", "n_rhs"):
+        d_ = rays[f][smooth].astype(np.int64) != orc[f][smooth]
+        assert d_.sum() <= max(1.0, (0.02 if metric["id"] == W.MANKO_NOVIKOV else 1e-4) * d_.size), (label, f, int(d_.sum()))
+    # the rays that miss the ring are ordinary rays: the ordinary rules
+    miss = (os_ != 5) & (gs != 5)
+    check_parity(w, rays[miss], orc[miss], probe[miss], label + " (rays that miss)", max_flagged_fraction=0.05)
+    g = disk["g"][smooth, 0]
+    assert (g > 1.0).any() and (g < 1.0).any()
+    print(label, "hits", int(hit.sum()), "smooth", int(smooth.sum()), "radial-face hits", int((smooth & ~on_th).sum()),
+          "status mismatches (excused)", int(mism.sum()))
+
+
+def test_solid_ring_thin_limit_on_the_gpu(gp):
+    """A property that needs no oracle: as the half angle -> 0 the ring hit becomes the first thin-disk
+    crossing inside [r_in, r_out] recorded by the disk variant of the same kernel."""
+    metric = dict(id=W.KERR, M=1.0, a=0.98, q=0.0)
+    ring = _ring("C3", metric, 1e-11, 4.0, 14.0, width=200, height=200)
+    thin = copy.deepcopy(ring)
+    thin["cfg"].update(ring_half_angle=0.0, max_crossings=3)
+    a, ad, _ = gp.api.trace_workload(thin)
+    b, bd, _ = gp.api.trace_workload(ring)
+    hit = a["n_disk_recorded"] >= 1
+    assert hit.sum() > 3000
+    assert (b["status"][hit] == 5).all() and np.array_equal(b["status"][~hit], a["status"][~hit])
+    assert np.abs(bd["r_cross"][hit, 0] - ad["r_cross"][hit, 0]).max() <= 1e-8
+    assert np.abs(bd["g"][hit, 0] / ad["g"][hit, 0] - 1.0).max() <= 1e-8
+    for f in a.dtype.names:                                # untouched rays: the same bits, except the evaluation
+        if f != "n_rhs":                                   # count (the two variants locate different things on the way)
+            assert np.array_equal(a[f][~hit], b[f][~hit], equal_nan=True), f
+
+
+def test_ring_validation_on_the_gpu(gp):
+    w = _ring("C3", dict(id=W.KERR, M=1.0, a=0.9, q=0.0), 0.05, 0.0, 14.0)
+    for bad, code in ((dict(max_crossings=2), gp.api.GP_E_UNSUPPORTED), (dict(scheme=1, h_rel=0.02), gp.api.GP_E_UNSUPPORTED),
+                      (dict(ring_half_angle=-0.1), gp.api.GP_E_BAD_PARAM), (dict(ring_half_angle=2.0), gp.api.GP_E_BAD_PARAM)):
+        wb = copy.deepcopy(w)
+        wb["cfg"].update(bad)
+        with pytest.raises(gp.api.GpError) as e:
+            gp.api.trace_workload(wb, 0, 10, 1)
+        assert e.value.code == code, bad
