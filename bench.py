@@ -60,8 +60,9 @@ def _args():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--cpu-seconds", type=float, default=12.0,
                     help="target oracle time for the cpu_baseline sample")
-    ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32"],
-                    help="fp32: the single-precision variant (fixed-step RK4 workloads only)")
+    ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32", "mixed"],
+                    help="fp32: the single-precision variant (fixed-step RK4 workloads only); mixed: FP32 "
+                         "equations with an FP64 state (adaptive workloads run at rtol = atol = 1e-7)")
     ap.add_argument("--stage", default="trace", choices=["trace", "shade"],
                     help="shade: time the image-formation kernel gp_shade on the records of a 2048^2 frame")
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
@@ -237,11 +238,16 @@ def run_b200(args):
     strong = args.scaling == "strong" and world > 1
     if not strong:
         w["camera"]["jitter_seed"] = int(w["camera"].get("jitter_seed", 0)) + rank
-    fp32 = args.precision == "fp32"
-    if fp32:
+    mixed = args.precision == "mixed"
+    fp32 = args.precision == "fp32" or mixed        # which roofline: the equations run on the FP32 lanes
+    if args.precision == "fp32":
         if w["cfg"]["scheme"] == 2:
             raise SystemExit("bench.py: --precision fp32 exists for the fixed-step RK4 workloads only")
         w["cfg"]["precision"] = 1
+    if mixed:
+        w["cfg"]["precision"] = 2
+        if w["cfg"]["scheme"] == 2:
+            w["cfg"].update(rtol=1e-7, atol=1e-7)   # gp.h: the floor of the mixed adaptive variant
     n_frame = W.n_rays(w)
     sel = W.shard(w, rank, world) if strong else W.ray_selection(w)
     n = sel[1]                      # rays this rank traces per step
@@ -383,7 +389,7 @@ def run_b200(args):
         # per-launch CUDA-event times of this rank over the timed region (best and median)
         "ms_per_step_best": per_launch_ms[0], "ms_per_step_median": per_launch_ms[len(per_launch_ms) // 2],
         "higher_is_better": True, "scaling": "strong" if strong else "weak", "vs_baseline": None,
-        "dtype": "f32" if fp32 else "f64",
+        "dtype": "f32 equations + f64 state" if mixed else ("f32" if fp32 else "f64"),
         "data": "synthetic",
         "config": config_of(w, world, {"parallelism": f"cyclic_shards{world}", "rays_per_step_per_gpu": n} if strong else None),
         "rhs_evals_per_s": world * n_rhs * args.steps / sec,      # rank 0's count x ranks

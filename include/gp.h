@@ -87,9 +87,15 @@ typedef struct gp_camera {
  * lambda_max when lambda_max > 0), NONFINITE / STEP_UNDERFLOW on numerical failure.     */
 typedef struct gp_integrator_cfg {
   int32_t scheme;    /* 0, 1, 2 as above                                                 */
-  int32_t precision; /* 0 = FP64; 1 = FP32 state and equations, schemes 0 and 1 only (with
-                        scheme 2 -> GP_E_UNSUPPORTED); the ray is born and the record written in
-                        FP64 either way; others -> GP_E_UNSUPPORTED                             */
+  int32_t precision; /* 0 = FP64 (required path).
+                        1 = FP32 state and equations, schemes 0 and 1 only (scheme 2 -> GP_E_UNSUPPORTED).
+                        2 = mixed: Hamilton's equations in FP32 at the state
+                            rounded to FP32, state / Runge-Kutta sums / error norm / controller in FP64;
+                            all schemes; with scheme 2 rtol and atol must be >= 1e-7 (the error estimate
+                            carries the 6e-8 noise of an FP32 evaluation; below -> GP_E_BAD_PARAM) and no
+                            disk / ring (-> GP_E_UNSUPPORTED).  Stated tolerance of 1 and 2: DESIGN.md 7.6.
+                        The ray is born and the record written in FP64 in every case; other values ->
+                        GP_E_UNSUPPORTED                                                             */
   double h, h_rel, rtol, atol, h_cap_rel;
   int64_t max_steps; /* attempted steps (accepted + rejected), landing steps not counted */
   double lambda_max; /* <= 0: off                                                        */

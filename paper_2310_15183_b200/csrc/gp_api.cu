@@ -151,8 +151,13 @@ int make_params(int metric_id, const gp_metric_params *m, const gp_camera *cam, 
   memset(P, 0, sizeof(*P));
   int rc = make_metric(metric_id, m, &P->mc);
   if (rc) return rc;
-  if (cfg->precision != 0 && cfg->precision != 1) return GP_E_UNSUPPORTED;
+  if (cfg->precision < 0 || cfg->precision > 2) return GP_E_UNSUPPORTED;
   if (cfg->scheme < 0 || cfg->scheme > 2) return GP_E_BAD_PARAM;
+  // precision 2 (FP32 equations, FP64 state): every scheme; with the adaptive scheme the tolerances must
+  // stay above the noise of an FP32 evaluation of the equations in the error estimate (gp.h)
+  if (cfg->precision == 2 && cfg->scheme == 2 && (!(cfg->rtol >= 1e-7) || !(cfg->atol >= 1e-7))) return GP_E_BAD_PARAM;
+  if (cfg->precision == 2 && cfg->scheme == 2 && (cfg->max_crossings > 0 || cfg->ring_half_angle > 0.0))
+    return GP_E_UNSUPPORTED;   // the mixed adaptive kernel is built without objects
   // the single-precision variant exists for the fixed-step schemes only: a 1e-10 tolerance has no
   // meaning in FP32 arithmetic
   if (cfg->precision == 1 && cfg->scheme == 2) return GP_E_UNSUPPORTED;
@@ -265,32 +270,43 @@ int launch_info(Kernel kernel, size_t smem, LaunchInfo *slot, LaunchInfo *out) {
 template <int METRIC, int OBJ>
 int launch_one(const TraceParams &P, cudaStream_t stream) {
   constexpr bool DISK = (OBJ == 1);
-  static LaunchInfo cache[kMaxDevices][3];   // per device: dp54, rk4 FP64, rk4 FP32 (zero-initialised)
+  static LaunchInfo cache[kMaxDevices][5];   // per device: dp54, rk4 FP64 / FP32 / mixed, dp54 mixed (zero-initialised)
   const bool dp54 = (P.scheme == 2);
-  const bool fp32 = (P.precision == 1);
+  const int prec = P.precision;   // 0 FP64, 1 FP32, 2 FP32 equations + FP64 state
   const size_t smem = dp54 ? dp54_smem_bytes(OBJ != 0)
-                           : (DISK ? (fp32 ? sizeof(float) : sizeof(double)) * kBlock * kParkSlotsRk4 : 0);
+                           : (DISK ? (prec == 1 ? sizeof(float) : sizeof(double)) * kBlock * kParkSlotsRk4 : 0);
   int dev = 0;
   GP_CUDA(cudaGetDevice(&dev));
   if (dev < 0 || dev >= kMaxDevices) return GP_E_UNSUPPORTED;
-  LaunchInfo *slot = &cache[dev][dp54 ? 0 : (fp32 ? 2 : 1)];
+  LaunchInfo *slot = &cache[dev][dp54 ? (prec == 2 ? 4 : 0) : 1 + prec];
   LaunchInfo li;
   int rc;
-  if (dp54) rc = launch_info(trace_dp54<METRIC, OBJ>, smem, slot, &li);
-  else if (fp32) rc = launch_info(trace_rk4<METRIC, DISK, float>, smem, slot, &li);
-  else rc = launch_info(trace_rk4<METRIC, DISK, double>, smem, slot, &li);
-  if (rc) return rc;
   // persistent grid: every SM filled to its resident-block limit, never more lanes than rays
-  long long want = ((long long)P.cc.ray_count + kBlock - 1) / kBlock;
-  long long grid = (long long)li.n_sm * li.per_sm;
-  if (grid > want) grid = want;
-  if (grid < 1) grid = 1;
-  if (dp54)
-    trace_dp54<METRIC, OBJ><<<(unsigned)grid, kBlock, smem, stream>>>(P);
-  else if (fp32)
-    trace_rk4<METRIC, DISK, float><<<(unsigned)grid, kBlock, smem, stream>>>(P);
-  else
-    trace_rk4<METRIC, DISK, double><<<(unsigned)grid, kBlock, smem, stream>>>(P);
+#define GP_GO(kernel_)                                                            \
+  {                                                                               \
+    rc = launch_info(kernel_, smem, slot, &li);                                   \
+    if (rc) return rc;                                                            \
+    long long want = ((long long)P.cc.ray_count + kBlock - 1) / kBlock;           \
+    long long grid = (long long)li.n_sm * li.per_sm;                              \
+    if (grid > want) grid = want;                                                 \
+    if (grid < 1) grid = 1;                                                       \
+    kernel_<<<(unsigned)grid, kBlock, smem, stream>>>(P);                         \
+  }
+  if (dp54) {
+    if (prec == 2) {
+      if (OBJ != 0) return GP_E_UNSUPPORTED;
+      GP_GO((trace_dp54<METRIC, 0, float>))
+    } else {
+      GP_GO((trace_dp54<METRIC, OBJ>))
+    }
+  } else if (prec == 1) {
+    GP_GO((trace_rk4<METRIC, DISK, float>))
+  } else if (prec == 2) {
+    GP_GO((trace_rk4<METRIC, DISK, float, double>))
+  } else {
+    GP_GO((trace_rk4<METRIC, DISK, double>))
+  }
+#undef GP_GO
   GP_CUDA(cudaGetLastError());
   return GP_OK;
 }

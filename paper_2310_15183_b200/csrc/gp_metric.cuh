@@ -275,6 +275,19 @@ GP_HD void rhs_eval_scaled_sc(const MetricConst &mc, T pt, T pph, T r, T s, T c,
   }
 }
 
+// The mixed-precision form (cfg.precision = 2): the equations are evaluated in FP32 at the FP64 state
+// rounded to FP32, the six derivatives come back in FP64 multiplied by hs.
+template <int METRIC>
+GP_HD void rhs_eval_fp32_scaled(const MetricConst &mc, double pt, double pph, double r, double th, double pr,
+                                double pth, double hs, RhsT<double> &o) {
+  RhsT<float> f;
+  f.pw = 0.0f;
+  rhs_eval<METRIC, true, float>(mc, (float)pt, (float)pph, (float)r, (float)th, (float)pr, (float)pth, f);
+  o.dt = hs * (double)f.dt; o.dr = hs * (double)f.dr; o.dth = hs * (double)f.dth;
+  o.dph = hs * (double)f.dph; o.dpr = hs * (double)f.dpr; o.dpth = hs * (double)f.dpth;
+  o.s = (double)f.s; o.c = (double)f.c; o.H2 = (double)f.H2; o.is = (double)f.is; o.pw = (double)f.pw;
+}
+
 // ---- covariant metric at a point (host: observer tetrad, row a3) ------------------------------
 // out: g_tt, g_tphi, g_phiphi, g_rr, g_thth
 GP_HD void metric_cov(int metric, const MetricConst &mc, double r, double th, double g[5]) {

@@ -64,10 +64,13 @@ __device__ __forceinline__ void lds2(unsigned a, double &x, double &y) {
 
 // OBJ: 0 no object; 1 thin disk, crossings located and recorded (R19); 2 solid ring, the ray ends where it
 // enters the volume (R39).  Both objects use the park area.
-template <int METRIC, int OBJ>
+// TR: arithmetic type of Hamilton's equations.  double is the required path; float is the mixed variant
+// (cfg.precision = 2): FP32 equations at the rounded state, FP64 state, sums, error
+// norm and controller — the tolerance must then stay above the noise of an FP32 evaluation (gp.h).
+template <int METRIC, int OBJ, class TR = double>
 __global__ void __launch_bounds__(kBlock, METRIC == METRIC_MN ? GP_DP54_MIN_BLOCKS_MN : GP_DP54_MIN_BLOCKS)
 trace_dp54(const __grid_constant__ TraceParams P) {
-  constexpr bool DISK = (OBJ == 1), RING = (OBJ == 2);
+  constexpr bool DISK = (OBJ == 1), RING = (OBJ == 2), MIXED = (sizeof(TR) == 4);
   extern __shared__ double2 smem2[];
   const MetricConst &mc = P.mc;
   const int tid = threadIdx.x;
@@ -84,7 +87,7 @@ trace_dp54(const __grid_constant__ TraceParams P) {
   double r = 0.0, th = 0.0, pr = 0.0, pth = 0.0;      // y_n, the part Hamilton's equations read
   // raw F(y_n) lives in shared memory (K slots 8, 9): written when y_n changes, read once per attempt
 #define GP_SET_K1(a_, b_, c_, d_) { sts2(KS(8), (a_), (b_)); sts2(KS(9), (c_), (d_)); }
-#define GP_SET_SC(s_, c_) if (METRIC == METRIC_KERR) sts2(KS(10), (s_), (c_));
+#define GP_SET_SC(s_, c_) if (METRIC == METRIC_KERR && !MIXED) sts2(KS(10), (s_), (c_));
   double h = 0.0;                                     // step of the attempt in flight / next attempt
   // pending (trial) state and the error sums that still lack the e7 k7 term
   double nt = 0.0, nr = 0.0, nth = 0.0, nph = 0.0, npr = 0.0, npth = 0.0, nlam = 0.0;
@@ -148,7 +151,8 @@ trace_dp54(const __grid_constant__ TraceParams P) {
     if (mode != MODE_IDLE) {
       // ---- A: F at the pending state (stage 7 of the attempt in flight / k1 of a fresh ray) ----
       Rhs o7;
-      rhs_eval<METRIC, true>(mc, pt, pph, nr, nth, npr, npth, o7);
+      if (MIXED) rhs_eval_fp32_scaled<METRIC>(mc, pt, pph, nr, nth, npr, npth, 1.0, o7);
+      else rhs_eval<METRIC, true>(mc, pt, pph, nr, nth, npr, npth, o7);
 
       // ---- B: decisions ----
       bool finished = false;
@@ -427,7 +431,7 @@ trace_dp54(const __grid_constant__ TraceParams P) {
         // are the increments d_j, and sin, cos of theta_n + d_j come from (sin, cos) theta_n — by-products of
         // the evaluation that produced k1, kept in K slot 10 — through the addition theorems (sincos_add):
         // no range reduction or quadrant logic inside the stages.  Manko-Novikov evaluates its own sincos.
-        constexpr bool kAngle = (METRIC == METRIC_KERR);
+        constexpr bool kAngle = (METRIC == METRIC_KERR) && !MIXED;
         const double thb = kAngle ? 0.0 : th;
         double sn_ = 0.0, cn_ = 0.0;
         if (kAngle) lds2(KS(10), sn_, cn_);
@@ -436,6 +440,8 @@ trace_dp54(const __grid_constant__ TraceParams P) {
     double ss_, cc_;                                                                           \
     sincos_add(sn_, cn_, (xth_), &ss_, &cc_);                                                  \
     rhs_eval_scaled_sc<METRIC>(mc, pt, pph, (xr_), ss_, cc_, (xpr_), (xpth_), s, o);           \
+  } else if (MIXED) {                                                                          \
+    rhs_eval_fp32_scaled<METRIC>(mc, pt, pph, (xr_), (xth_), (xpr_), (xpth_), s, o);           \
   } else {                                                                                     \
     rhs_eval_scaled<METRIC, true>(mc, pt, pph, (xr_), (xth_), (xpr_), (xpth_), s, o);          \
   }

@@ -7,9 +7,12 @@
 // equations are evaluated at is first tested against the capture radius; the first hit ends the
 // ray as CAPTURED (then one landing step from y_n).
 //
-// T is the arithmetic type of the state and of Hamilton's equations: double, or float for the
-// single-precision variant BASELINE.json configs[4] asks for (cfg.precision = 1).  The ray is
-// always born in double (rows a2, a3) and the record is always written in double.
+// T is the arithmetic type of Hamilton's equations and S that of the state and of the Runge-Kutta sums:
+// (double, double) is the required path; (float, float) the single-precision variant BASELINE.json
+// configs[4] asks for (cfg.precision = 1); (float, double) the mixed variant of SURVEY.md section 8(f)
+// NEXT-1 (cfg.precision = 2): the equations are evaluated in FP32 at the state rounded to FP32, their
+// results are accumulated into an FP64 state, so that rounding no longer accumulates with the number of
+// steps.  The ray is always born in double (rows a2, a3) and the record is always written in double.
 #ifndef GP_TRACE_RK4_CUH_
 #define GP_TRACE_RK4_CUH_
 
@@ -18,19 +21,19 @@ namespace gp {
 
 constexpr int kParkSlotsRk4 = 7;  // trial state (r, th, pr, pth, t, ph, lambda) across an equator landing
 
-template <int METRIC, bool DISK, class T>
+template <int METRIC, bool DISK, class T, class S = T>
 __global__ void __launch_bounds__(kBlock) trace_rk4(const __grid_constant__ TraceParams P) {
-  extern __shared__ double park_raw[];  // [kParkSlotsRk4][kBlock] of T when DISK
-  T *park = reinterpret_cast<T *>(park_raw);
+  extern __shared__ double park_raw[];  // [kParkSlotsRk4][kBlock] of S when DISK
+  S *park = reinterpret_cast<S *>(park_raw);
   const MetricConst &mc = P.mc;
   const int tid = threadIdx.x;
-  const T r_cap = (T)P.r_cap, r_esc = (T)P.r_esc, half_pi = (T)kHalfPi;
+  const S r_cap = (S)P.r_cap, r_esc = (S)P.r_esc, half_pi = (S)kHalfPi;
 
   int mode = MODE_IDLE;
   long long slot = -1;
   T pt = T(0), pph = T(0);
-  T t = T(0), r = T(0), th = T(0), ph = T(0), pr = T(0), pth = T(0), lam = T(0);
-  T target = T(0);
+  S t = S(0), r = S(0), th = S(0), ph = S(0), pr = S(0), pth = S(0), lam = S(0);
+  S target = S(0);
   MonitorsT<T> mo = {T(0), T(0), T(0), T(1), T(0), T(0)};
   unsigned n_acc = 0, n_cross = 0, n_rec = 0, n_land = 0, status = 0;
   bool exhausted = false;
@@ -50,8 +53,8 @@ __global__ void __launch_bounds__(kBlock) trace_rk4(const __grid_constant__ Trac
         } else {
           double dr0, dth0, dph0, dpt, dpr, dpth, dpph;
           ray_birth(P.cc, mc, P.cc.ray_begin + slot * P.cc.ray_stride, dr0, dth0, dph0, dpt, dpr, dpth, dpph);
-          pt = (T)dpt; pr = (T)dpr; pth = (T)dpth; pph = (T)dpph;
-          t = T(0); r = (T)dr0; th = (T)dth0; ph = (T)dph0; lam = T(0);
+          pt = (T)dpt; pr = (S)dpr; pth = (S)dpth; pph = (T)dpph;
+          t = S(0); r = (S)dr0; th = (S)dth0; ph = (S)dph0; lam = S(0);
           mode = MODE_NORMAL;
           n_acc = n_cross = n_rec = n_land = 0;
           mo.h_max = T(0); mo.q_drift = T(0); mo.Q0 = T(0);
@@ -73,53 +76,54 @@ __global__ void __launch_bounds__(kBlock) trace_rk4(const __grid_constant__ Trac
       if (!finished) {
         const bool normal = (mode == MODE_NORMAL);
         const bool land_r = (mode == MODE_LAND_R);
-        const T s = normal ? (P.scheme == 0 ? (T)P.h : (T)P.h_rel * r) : (land_r ? (target - r) : (target - th));
+        const S s = normal ? (P.scheme == 0 ? (S)P.h : (S)P.h_rel * r) : (land_r ? (target - r) : (target - th));
         // Landing steps are 1 in several hundred: their divisor work (Henon's 1/F_w) sits behind a
         // warp-uniform branch taken only when some lane of this convergence group is landing.
         const bool any_land = __any_sync(__activemask(), !normal);
-        T sl = T(1);  // weighted sum of 1/F_w: d(lambda)/ds of a landing step (unused otherwise)
+        S sl = S(1);  // weighted sum of 1/F_w: d(lambda)/ds of a landing step (unused otherwise)
 #define GP_HENON(weight, first)                                                   \
   if (any_land) {                                                                 \
     T iv = normal ? T(1) : frcp(land_r ? o.dr : o.dth);                           \
     o.dt *= iv; o.dr *= iv; o.dth *= iv; o.dph *= iv; o.dpr *= iv; o.dpth *= iv;  \
-    sl = (first) ? iv : sl + T(weight) * iv;                                      \
+    sl = (first) ? (S)iv : sl + S(weight) * (S)iv;                                \
   }
         RhsT<T> o;
         // k1 = F(y_n)
-        rhs_eval<METRIC>(mc, pt, pph, r, th, pr, pth, o);
+        rhs_eval<METRIC>(mc, pt, pph, (T)r, (T)th, (T)pr, (T)pth, o);
         if (normal)
-          monitor_apply<METRIC>(mo, (T)fabs(T(0.5) * o.H2), carter_q<METRIC>(mc, pt, pph, pth, o), (T)fabs(o.s),
+          monitor_apply<METRIC>(mo, (T)fabs(T(0.5) * o.H2), carter_q<METRIC>(mc, pt, pph, (T)pth, o), (T)fabs(o.s),
                                 n_acc == 0);
         GP_HENON(1.0, true)
-        T st = o.dt, sr = o.dr, sth = o.dth, sph = o.dph, spr = o.dpr, spth = o.dpth;  // k1 + 2k2 + 2k3 + k4
-        const T hs = T(0.5) * s;
+        // k1 + 2k2 + 2k3 + k4, accumulated in the state's type
+        S st = (S)o.dt, sr = (S)o.dr, sth = (S)o.dth, sph = (S)o.dph, spr = (S)o.dpr, spth = (S)o.dpth;
+        const S hs = S(0.5) * s;
         // k2 = F(y_n + h/2 k1)
-        T yr = r + hs * o.dr;
+        S yr = r + hs * (S)o.dr;
         bool captured = normal && (yr < r_cap);
-        rhs_eval<METRIC>(mc, pt, pph, yr, th + hs * o.dth, pr + hs * o.dpr, pth + hs * o.dpth, o);
+        rhs_eval<METRIC>(mc, pt, pph, (T)yr, (T)(th + hs * (S)o.dth), (T)(pr + hs * (S)o.dpr), (T)(pth + hs * (S)o.dpth), o);
         GP_HENON(2.0, false)
-        st += T(2) * o.dt; sr += T(2) * o.dr; sth += T(2) * o.dth; sph += T(2) * o.dph; spr += T(2) * o.dpr;
-        spth += T(2) * o.dpth;
+        st += S(2) * (S)o.dt; sr += S(2) * (S)o.dr; sth += S(2) * (S)o.dth; sph += S(2) * (S)o.dph;
+        spr += S(2) * (S)o.dpr; spth += S(2) * (S)o.dpth;
         // k3 = F(y_n + h/2 k2)
-        yr = r + hs * o.dr;
+        yr = r + hs * (S)o.dr;
         captured = captured || (normal && (yr < r_cap));
-        rhs_eval<METRIC>(mc, pt, pph, yr, th + hs * o.dth, pr + hs * o.dpr, pth + hs * o.dpth, o);
+        rhs_eval<METRIC>(mc, pt, pph, (T)yr, (T)(th + hs * (S)o.dth), (T)(pr + hs * (S)o.dpr), (T)(pth + hs * (S)o.dpth), o);
         GP_HENON(2.0, false)
-        st += T(2) * o.dt; sr += T(2) * o.dr; sth += T(2) * o.dth; sph += T(2) * o.dph; spr += T(2) * o.dpr;
-        spth += T(2) * o.dpth;
+        st += S(2) * (S)o.dt; sr += S(2) * (S)o.dr; sth += S(2) * (S)o.dth; sph += S(2) * (S)o.dph;
+        spr += S(2) * (S)o.dpr; spth += S(2) * (S)o.dpth;
         // k4 = F(y_n + h k3)
-        yr = r + s * o.dr;
+        yr = r + s * (S)o.dr;
         captured = captured || (normal && (yr < r_cap));
-        rhs_eval<METRIC>(mc, pt, pph, yr, th + s * o.dth, pr + s * o.dpr, pth + s * o.dpth, o);
+        rhs_eval<METRIC>(mc, pt, pph, (T)yr, (T)(th + s * (S)o.dth), (T)(pr + s * (S)o.dpr), (T)(pth + s * (S)o.dpth), o);
         GP_HENON(1.0, false)
-        st += o.dt; sr += o.dr; sth += o.dth; sph += o.dph; spr += o.dpr; spth += o.dpth;
+        st += (S)o.dt; sr += (S)o.dr; sth += (S)o.dth; sph += (S)o.dph; spr += (S)o.dpr; spth += (S)o.dpth;
 #undef GP_HENON
-        const T w = s * (T)dp.sixth;
-        const T nt = t + w * st, nr = r + w * sr, nth = th + w * sth, nph = ph + w * sph,
+        const S w = s * (S)dp.sixth;
+        const S nt = t + w * st, nr = r + w * sr, nth = th + w * sth, nph = ph + w * sph,
                 npr = pr + w * spr, npth = pth + w * spth;
 
         if (normal) {
-          const T ysum = ((nt + nr) + (nth + nph)) + (npr + npth);
+          const S ysum = ((nt + nr) + (nth + nph)) + (npr + npth);
           const bool nonfinite = !captured && !finite_d(ysum);
           if (!nonfinite) ++n_acc;
           if (nonfinite) {
@@ -132,10 +136,10 @@ __global__ void __launch_bounds__(kBlock) trace_rk4(const __grid_constant__ Trac
             mode = MODE_LAND_R;
           } else {
             bool commit = true;
-            if ((th - half_pi) * (nth - half_pi) < T(0)) {
+            if ((th - half_pi) * (nth - half_pi) < S(0)) {
               ++n_cross;
               if (DISK && n_rec < (unsigned)P.max_crossings) {
-                T *pk = park + tid;
+                S *pk = park + tid;
                 pk[0 * kBlock] = nr; pk[1 * kBlock] = nth; pk[2 * kBlock] = npr; pk[3 * kBlock] = npth;
                 pk[4 * kBlock] = nt; pk[5 * kBlock] = nph; pk[6 * kBlock] = lam + s;
                 target = half_pi;
@@ -160,7 +164,7 @@ __global__ void __launch_bounds__(kBlock) trace_rk4(const __grid_constant__ Trac
               P.disk[slot].g[n_rec] = kepler_g<METRIC>(mc, rc, (double)pt, (double)pph);
               ++n_rec;
             }
-            const T *pk = park + tid;
+            const S *pk = park + tid;
             r = pk[0 * kBlock]; th = pk[1 * kBlock]; pr = pk[2 * kBlock]; pth = pk[3 * kBlock];
             t = pk[4 * kBlock]; ph = pk[5 * kBlock]; lam = pk[6 * kBlock];
           }
