@@ -57,6 +57,9 @@ def _args():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="headline")
+    ap.add_argument("--side", type=int, default=0,
+                    help="override the image size of the workload (side x side pixels); for profiling the "
+                         "Manko-Novikov configs at a size ncu can replay")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--cpu-seconds", type=float, default=12.0,
                     help="target oracle time for the cpu_baseline sample")
@@ -234,7 +237,7 @@ def run_b200(args):
     # its own frame of the workload (its own jitter seed).  strong: ONE frame, rank g takes the rays
     # g, g + G, g + 2G, ... (gp_workloads.shard: cost per ray varies strongly over the image, cyclic
     # interleave balances it); each rank runs its own work counter into its own buffers.
-    w = W.workload(args.workload)
+    w = W.workload(args.workload, **(dict(width=args.side, height=args.side) if args.side else {}))
     strong = args.scaling == "strong" and world > 1
     if not strong:
         w["camera"]["jitter_seed"] = int(w["camera"].get("jitter_seed", 0)) + rank

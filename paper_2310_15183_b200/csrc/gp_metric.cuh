@@ -231,9 +231,11 @@ GP_HD void rhs_manko_novikov(const MetricConst &mc, T pt, T pph, T r, T th, T pr
 // out-of-line copy keeps that kernel inside the instruction cache: measured +9 % on the DP5(4) kernel
 // and -4 % on the four-stage RK4 kernel, which therefore keeps the inlined form (OUTLINE_MN = false).
 template <class T>
-__device__ __noinline__ void rhs_manko_novikov_call(const MetricConst &mc, T pt, T pph, T r, T th, T pr, T pth,
-                                                    RhsT<T> &o) {
+__device__ __noinline__ RhsT<T> rhs_manko_novikov_call(const MetricConst &mc, T pt, T pph, T r, T th, T pr, T pth) {
+  RhsT<T> o;
   rhs_manko_novikov<T>(mc, pt, pph, r, th, pr, pth, o);
+  o.pw = T(0);
+  return o;   // by value: the ten results come back in registers, not through the caller's stack frame
 }
 #endif
 
@@ -243,7 +245,7 @@ GP_HD void rhs_eval(const MetricConst &mc, T pt, T pph, T r, T th, T pr, T pth, 
   else if (METRIC == METRIC_KERR) rhs_kerr<T>(mc, pt, pph, r, th, pr, pth, o);
   else {
 #if defined(__CUDA_ARCH__)
-    if (OUTLINE_MN) rhs_manko_novikov_call<T>(mc, pt, pph, r, th, pr, pth, o);
+    if (OUTLINE_MN) o = rhs_manko_novikov_call<T>(mc, pt, pph, r, th, pr, pth);
     else rhs_manko_novikov<T>(mc, pt, pph, r, th, pr, pth, o);
 #else
     rhs_manko_novikov<T>(mc, pt, pph, r, th, pr, pth, o);
