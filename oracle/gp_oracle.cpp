@@ -1021,38 +1021,51 @@ int orc_integrate_orbits(const orc_metric *m, const orc_orbit_cfg *cfg, const do
     S.pphi = st[7];
     auto f = [&](const double *yy, double *dy) { rhs(S, yy, dy); };
     double y[6] = {st[0], st[1], st[2], st[3], st[5], st[6]};
-    double lam = 0.0, h = cfg->h0;
+    // "Integrate to lambda_1, sample; integrate on to lambda_2, sample; ..." (gp_oracle.h): an outer loop over
+    // the sample times and, for each, the adaptive loop of R10 run until the affine parameter EQUALS the
+    // sample time.  `proposal` is the controller's current step suggestion; an attempt takes the smallest of
+    // the proposal, h_max and the distance left to the sample time; when it is the distance that binds, the
+    // attempt "arrives": lambda is set to the sample time itself and the proposal is not allowed to shrink
+    // because of the shortened step (it keeps the larger of its old value and the new suggestion).
+    double lam = 0.0, proposal = cfg->h0;
     double k[7][7];
     f(y, k[0]);
-    int64_t next = 0, steps = 0, stat = 0;
-    while (next < K) {
-      if (steps >= cfg->max_steps) { stat = 2; break; }
-      if (h < 1e-14 * std::fmax(1.0, std::fabs(lam))) { stat = 4; break; }
-      const double lam_next = (double)(next + 1) * cfg->lambda_end / (double)K;
-      const double room = lam_next - lam;
-      double hs = std::fmin(h, cfg->h_max);
-      const bool cut = !(hs < room);       // the step is cut short (or exactly fits) at the sample time
-      if (cut) hs = room;
-      double ynew[6], errvec[7];
-      dp54_step(f, 6, y, hs, k, ynew, errvec);
-      ++steps;
-      double err = error_norm(y, ynew, errvec, cfg->rtol, cfg->atol);
-      if (!std::isfinite(err) || !all_finite(ynew, 6)) { h = hs * 0.2; continue; }
-      double fac = (err == 0.0) ? 5.0 : 0.9 * std::pow(err, -0.2);
-      if (err > 1.0) { h = hs * std::fmax(0.2, fac); continue; }
-      double hnew = hs * std::fmin(5.0, std::fmax(0.2, fac));
-      h = cut ? std::fmax(h, hnew) : hnew;
-      for (int c = 0; c < 6; ++c) y[c] = ynew[c];
-      for (int c = 0; c < 6; ++c) k[0][c] = k[6][c];   // FSAL
-      lam = cut ? lam_next : lam + hs;
-      if (y[1] < r_cap) { stat = 1; break; }
-      if (cut) {
-        double *o = out + 8 * next;
-        // 2H = p_mu dq^mu/dlambda: p_t dt + p_r dr + p_th dth + p_ph dph with the FSAL slopes
-        double H2 = S.pt * k[0][0] + y[4] * k[0][1] + y[5] * k[0][2] + S.pphi * k[0][3];
-        o[0] = y[0]; o[1] = y[1]; o[2] = y[2]; o[3] = y[3]; o[4] = y[4]; o[5] = y[5]; o[6] = H2; o[7] = lam;
-        ++next;
+    int64_t steps = 0, stat = 0;
+    for (int64_t sample = 0; sample < K && stat == 0; ++sample) {
+      const double t_sample = (double)(sample + 1) * cfg->lambda_end / (double)K;
+      while (lam != t_sample) {
+        if (steps >= cfg->max_steps) { stat = 2; break; }
+        if (proposal < 1e-14 * std::fmax(1.0, std::fabs(lam))) { stat = 4; break; }
+        const double left = t_sample - lam;
+        double take = std::fmin(proposal, cfg->h_max);
+        const bool arrives = take >= left;
+        if (arrives) take = left;
+        double ynew[6], errvec[7];
+        dp54_step(f, 6, y, take, k, ynew, errvec);
+        ++steps;
+        const double err = error_norm(y, ynew, errvec, cfg->rtol, cfg->atol);
+        if (!std::isfinite(err) || !all_finite(ynew, 6)) {   // R10 item 2
+          proposal = 0.2 * take;
+          continue;
+        }
+        const double fac = (err == 0.0) ? 5.0 : 0.9 * std::pow(err, -0.2);
+        if (err > 1.0) {                                     // R10 item 3, rejected
+          proposal = take * std::fmax(0.2, fac);
+          continue;
+        }
+        const double suggestion = take * std::fmin(5.0, std::fmax(0.2, fac));
+        proposal = arrives ? std::fmax(proposal, suggestion) : suggestion;
+        for (int c = 0; c < 6; ++c) y[c] = ynew[c];
+        for (int c = 0; c < 6; ++c) k[0][c] = k[6][c];       // FSAL
+        lam = arrives ? t_sample : lam + take;
+        if (y[1] < r_cap) { stat = 1; break; }
       }
+      if (stat != 0) break;
+      // the sample: state, 2H = p_mu dq^mu/dlambda from the slopes at the new state, lambda
+      double *o = out + 8 * sample;
+      o[0] = y[0]; o[1] = y[1]; o[2] = y[2]; o[3] = y[3]; o[4] = y[4]; o[5] = y[5];
+      o[6] = S.pt * k[0][0] + y[4] * k[0][1] + y[5] * k[0][2] + S.pphi * k[0][3];
+      o[7] = lam;
     }
     status[i] = stat;
     n_steps[i] = steps;
