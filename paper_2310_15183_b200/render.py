@@ -34,7 +34,7 @@ def write_ppm(path, rgba):
 
 
 def render(workload, size=None, supersample=1, mode="grid", disk=False, inclination_deg=None, projection=0,
-           tex=(2048, 1024), time_period=25.0, device="cuda"):
+           tex=(2048, 1024), time_period=25.0, device="cuda", ring_half_angle=0.0):
     """Returns ((H, W, 4) uint8 image with row 0 at the top, dict of timings and counters)."""
     import numpy as np
     import torch
@@ -52,11 +52,16 @@ def render(workload, size=None, supersample=1, mode="grid", disk=False, inclinat
         w["cfg"].update(max_crossings=1, disk_r_out=20.0,
                         disk_r_in=(4.0 if w["metric"]["id"] == W.MANKO_NOVIKOV else 0.0))
         cfg = api.cfg_struct(w["cfg"])
+    if ring_half_angle > 0.0:      # the paper's solid ring (Figs 15-17) instead of the thin disk
+        w["cfg"].update(max_crossings=0, ring_half_angle=ring_half_angle, disk_r_out=14.0,
+                        disk_r_in=(5.0 if w["metric"]["id"] == W.MANKO_NOVIKOV else 0.0))
+        cfg = api.cfg_struct(w["cfg"])
     cam = api.camera_struct(w["camera"])
     n = cam.ray_count
     W_, H_ = w["camera"]["width"], w["camera"]["height"]
     rays = torch.empty(n * 128, dtype=torch.uint8, device=device)
-    drec = torch.empty(n * 48, dtype=torch.uint8, device=device) if cfg.max_crossings > 0 else None
+    need_disk = cfg.max_crossings > 0 or cfg.ring_half_angle > 0.0
+    drec = torch.empty(n * 48, dtype=torch.uint8, device=device) if need_disk else None
     counters = torch.empty(64, dtype=torch.uint8, device=device)
     out = torch.empty(W_ * H_ * 4, dtype=torch.uint8, device=device)
     stream = torch.cuda.current_stream()
@@ -85,11 +90,14 @@ def main(argv=None):
     ap.add_argument("--supersample", type=int, default=1)
     ap.add_argument("--mode", default="grid", choices=["grid", "texture", "time"])
     ap.add_argument("--disk", action="store_true", help="thin Keplerian disk coloured by its redshift factor")
+    ap.add_argument("--ring", type=float, default=0.0, metavar="HALF_ANGLE",
+                    help="solid ring of that half opening angle (rad) about the equator, coloured by redshift (adaptive workloads)")
     ap.add_argument("--inclination", type=float, default=None, help="observer polar angle in degrees")
     ap.add_argument("--screen-camera", action="store_true", help="the paper's Euclidean-screen camera (parallel rays)")
     ap.add_argument("--out", default="frame.png", help=".png or .ppm")
     a = ap.parse_args(argv)
-    img, info = render(a.workload, a.size, a.supersample, a.mode, a.disk, a.inclination, int(a.screen_camera))
+    img, info = render(a.workload, a.size, a.supersample, a.mode, a.disk, a.inclination, int(a.screen_camera),
+                       ring_half_angle=a.ring)
     (write_ppm if a.out.lower().endswith(".ppm") else write_png)(a.out, img)
     print(f"{a.out}: {img.shape[1]}x{img.shape[0]}, {info['rays']} rays, trace {info['trace_ms']:.2f} ms, "
           f"shade {info['shade_ms']:.3f} ms, {info['rhs_evaluations']} RHS evaluations", file=sys.stderr)

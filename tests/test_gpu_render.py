@@ -32,8 +32,9 @@ def _read_png(path):
 @pytest.mark.parametrize("args", [["--workload", "C2", "--mode", "grid"],
                                   ["--workload", "C3", "--mode", "texture", "--disk", "--supersample", "2"],
                                   ["--workload", "C4", "--mode", "time", "--disk", "--inclination", "80"],
-                                  ["--workload", "headline_rk4", "--mode", "grid", "--screen-camera"]],
-                         ids=["kerr_grid", "kerr_disk_texture_ss2", "mn_disk_time", "rk4_screen_camera"])
+                                  ["--workload", "headline_rk4", "--mode", "grid", "--screen-camera"],
+                                  ["--workload", "C3", "--mode", "grid", "--ring", "0.06", "--inclination", "78"]],
+                         ids=["kerr_grid", "kerr_disk_texture_ss2", "mn_disk_time", "rk4_screen_camera", "kerr_solid_ring"])
 def test_render_writes_an_image(tmp_path, args):
     from paper_2310_15183_b200 import render
     out = str(tmp_path / "frame.png")
