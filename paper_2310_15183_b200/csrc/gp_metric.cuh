@@ -277,6 +277,14 @@ GP_HD void rhs_eval_scaled_sc(const MetricConst &mc, T pt, T pph, T r, T s, T c,
   }
 }
 
+// Unscaled evaluation with sin and cos of theta supplied by the caller (Schwarzschild, Kerr): the stages of
+// trace_rk4 obtain them from (sin, cos) theta_n by the addition theorems (sincos_add).
+template <int METRIC, class T>
+GP_HD void rhs_eval_sc(const MetricConst &mc, T pt, T pph, T r, T s, T c, T pr, T pth, RhsT<T> &o) {
+  if (METRIC == METRIC_KERR) rhs_kerr<T, false, true>(mc, pt, pph, r, T(0), pr, pth, o, T(1), s, c);
+  else rhs_schwarzschild<T, true>(mc, pt, pph, r, T(0), pr, pth, o, s, c);
+}
+
 // The mixed-precision form (cfg.precision = 2): the equations are evaluated in FP32 at the FP64 state
 // rounded to FP32, the six derivatives come back in FP64 multiplied by hs.
 template <int METRIC>

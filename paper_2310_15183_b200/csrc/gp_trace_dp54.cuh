@@ -207,7 +207,7 @@ trace_dp54(const __grid_constant__ TraceParams P) {
           sts1(CS(C_MARGIN), dmin(lds1(CS(C_MARGIN)), fabs(err - 1.0)));
           // fac = 0.9 err^(-1/5), clamped to [0.2, 5] (err = 0 gives 5); the clamp of err keeps the
           // FP32 seed of pow_m1_5 in range and changes nothing: 0.9 (1e-5)^-0.2 = 9 > 5, 0.9 (1e4)^-0.2 = 0.14 < 0.2
-          double fac = dp.safety * pow_m1_5(dmin(dmax(dp.err_lo, err), dp.err_hi));
+          double fac = dp.safety * pow_m1_5_clamped(err);
           fac = dmin(dmax(dp.fac_min, fac), dp.fac_max);
           if (err > 1.0) {
             ++n_rej;

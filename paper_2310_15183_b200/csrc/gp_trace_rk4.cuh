@@ -21,8 +21,10 @@ namespace gp {
 
 constexpr int kParkSlotsRk4 = 7;  // trial state (r, th, pr, pth, t, ph, lambda) across an equator landing
 
+// (the disk variant of the FP64 Kerr kernel needs a few registers more than the 128 that four resident
+// blocks allow: it is held to three)
 template <int METRIC, bool DISK, class T, class S = T>
-__global__ void __launch_bounds__(kBlock) trace_rk4(const __grid_constant__ TraceParams P) {
+__global__ void __launch_bounds__(kBlock, (DISK && sizeof(T) == 8 && METRIC == METRIC_KERR) ? 3 : 0) trace_rk4(const __grid_constant__ TraceParams P) {
   extern __shared__ double park_raw[];  // [kParkSlotsRk4][kBlock] of S when DISK
   S *park = reinterpret_cast<S *>(park_raw);
   const MetricConst &mc = P.mc;
@@ -94,30 +96,45 @@ __global__ void __launch_bounds__(kBlock) trace_rk4(const __grid_constant__ Trac
           monitor_apply<METRIC>(mo, (T)fabs(T(0.5) * o.H2), carter_q<METRIC>(mc, pt, pph, (T)pth, o), (T)fabs(o.s),
                                 n_acc == 0);
         GP_HENON(1.0, true)
+        // Stage angles (Schwarzschild, Kerr): sin, cos of theta_n + d from (sin, cos) theta_n — by-products of
+        // k1 — through the addition theorems: no range reduction or quadrant logic in stages 2-4.  A fixed
+        // step has no error control to reject a stage that swings theta by more than the Taylor kernels
+        // cover (a ray grazing the polar axis does), so |d| > 1/4 takes the full evaluation.
+        constexpr bool kAngle = (METRIC != METRIC_MN);
+        const T sn_ = o.s, cn_ = o.c;
+#define GP_STAGE(yr_, dth_, ypr_, ypth_)                                                          \
+  if (kAngle && fabs((T)(dth_)) <= T(0.25)) {                                                     \
+    T ss_, cc_;                                                                                   \
+    sincos_add(sn_, cn_, (T)(dth_), &ss_, &cc_);                                                  \
+    rhs_eval_sc<METRIC>(mc, pt, pph, (T)(yr_), ss_, cc_, (T)(ypr_), (T)(ypth_), o);               \
+  } else {                                                                                        \
+    rhs_eval<METRIC>(mc, pt, pph, (T)(yr_), (T)(th + (dth_)), (T)(ypr_), (T)(ypth_), o);          \
+  }
         // k1 + 2k2 + 2k3 + k4, accumulated in the state's type
         S st = (S)o.dt, sr = (S)o.dr, sth = (S)o.dth, sph = (S)o.dph, spr = (S)o.dpr, spth = (S)o.dpth;
         const S hs = S(0.5) * s;
         // k2 = F(y_n + h/2 k1)
         S yr = r + hs * (S)o.dr;
         bool captured = normal && (yr < r_cap);
-        rhs_eval<METRIC>(mc, pt, pph, (T)yr, (T)(th + hs * (S)o.dth), (T)(pr + hs * (S)o.dpr), (T)(pth + hs * (S)o.dpth), o);
+        GP_STAGE(yr, hs * (S)o.dth, pr + hs * (S)o.dpr, pth + hs * (S)o.dpth)
         GP_HENON(2.0, false)
         st += S(2) * (S)o.dt; sr += S(2) * (S)o.dr; sth += S(2) * (S)o.dth; sph += S(2) * (S)o.dph;
         spr += S(2) * (S)o.dpr; spth += S(2) * (S)o.dpth;
         // k3 = F(y_n + h/2 k2)
         yr = r + hs * (S)o.dr;
         captured = captured || (normal && (yr < r_cap));
-        rhs_eval<METRIC>(mc, pt, pph, (T)yr, (T)(th + hs * (S)o.dth), (T)(pr + hs * (S)o.dpr), (T)(pth + hs * (S)o.dpth), o);
+        GP_STAGE(yr, hs * (S)o.dth, pr + hs * (S)o.dpr, pth + hs * (S)o.dpth)
         GP_HENON(2.0, false)
         st += S(2) * (S)o.dt; sr += S(2) * (S)o.dr; sth += S(2) * (S)o.dth; sph += S(2) * (S)o.dph;
         spr += S(2) * (S)o.dpr; spth += S(2) * (S)o.dpth;
         // k4 = F(y_n + h k3)
         yr = r + s * (S)o.dr;
         captured = captured || (normal && (yr < r_cap));
-        rhs_eval<METRIC>(mc, pt, pph, (T)yr, (T)(th + s * (S)o.dth), (T)(pr + s * (S)o.dpr), (T)(pth + s * (S)o.dpth), o);
+        GP_STAGE(yr, s * (S)o.dth, pr + s * (S)o.dpr, pth + s * (S)o.dpth)
         GP_HENON(1.0, false)
         st += (S)o.dt; sr += (S)o.dr; sth += (S)o.dth; sph += (S)o.dph; spr += (S)o.dpr; spth += (S)o.dpth;
 #undef GP_HENON
+#undef GP_STAGE
         const S w = s * (S)dp.sixth;
         const S nt = t + w * st, nr = r + w * sr, nth = th + w * sth, nph = ph + w * sph,
                 npr = pr + w * spr, npth = pth + w * spth;
