@@ -41,7 +41,7 @@ class gp_integrator_cfg(C.Structure):
                 ("max_steps", _i64), ("lambda_max", _f64),
                 ("eps_capture", _f64), ("r_escape", _f64),
                 ("disk_r_in", _f64), ("disk_r_out", _f64),
-                ("max_crossings", _i32), ("reserved_", _i32), ("ring_half_angle", _f64)]
+                ("max_crossings", _i32), ("segment_steps", _i32), ("ring_half_angle", _f64)]
 
 
 class gp_shade_cfg(C.Structure):
@@ -148,7 +148,8 @@ def cfg_struct(g):
                              int(g["max_steps"]), g.get("lambda_max", 0.0),
                              g["eps_capture"], g["r_escape"],
                              g.get("disk_r_in", 0.0), g.get("disk_r_out", 0.0),
-                             int(g.get("max_crossings", 0)), 0, g.get("ring_half_angle", 0.0))
+                             int(g.get("max_crossings", 0)), int(g.get("segment_steps", 0)),
+                             g.get("ring_half_angle", 0.0))
 
 
 def _stream_ptr(stream):

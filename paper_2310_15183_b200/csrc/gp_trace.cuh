@@ -34,9 +34,19 @@ struct TraceParams {
   gp_ray_record *rays;
   gp_disk_record *disk;
   unsigned long long *counters;
+  // Segmented tracing of long rays (Manko-Novikov, scheme 2): after seg_steps attempted
+  // steps a ray's state is parked in its own record and its slot appended to list_out; the next launch
+  // (round + 1) takes its work from that list.  seg_steps = 0: off.
+  long long seg_steps;
+  int round;
+  const long long *list_in;
+  const unsigned long long *list_in_count;
+  long long *list_out;
+  unsigned long long *list_out_count;
 };
 
-enum { MODE_IDLE = 0, MODE_FRESH = 1, MODE_NORMAL = 2, MODE_LAND_R = 3, MODE_LAND_TH = 4 };
+enum { MODE_IDLE = 0, MODE_FRESH = 1, MODE_NORMAL = 2, MODE_LAND_R = 3, MODE_LAND_TH = 4, MODE_RESUME = 5 };
+constexpr unsigned kRayParked = 255u;   // internal status of a record that holds a parked state (never left behind)
 
 #if defined(__CUDACC__)
 // Rows a2 + a3 for one ray: image-plane point, then the initial state of the selected camera.
@@ -221,7 +231,7 @@ __device__ __forceinline__ unsigned long long global_ns() {
   return t;
 }
 __device__ __forceinline__ void stamp_start(unsigned long long *counters) {
-  if (blockIdx.x == 0 && threadIdx.x == 0) counters[4] = global_ns();
+  if (blockIdx.x == 0 && threadIdx.x == 0 && counters[4] == 0ull) counters[4] = global_ns();   // first round only
 }
 __device__ __forceinline__ void stamp_ray_done(unsigned long long *counters, long long ray_count) {
   const unsigned long long done = atomicAdd(counters + 6, 1ull) + 1ull;

@@ -29,6 +29,7 @@ enum { C_T = 0, C_PH, C_LAM, C_HMAX, C_QDRIFT, C_Q0, C_IQ0, C_SINMIN, C_MARGIN, 
        C_SLOT,      // output slot of the ray in flight (64-bit integer bits)
        C_COUNTS,    // n_equator_crossings (low word) and landing steps taken (high word)
        C_STATE,     // status of the ray once decided (low word) and disk crossings recorded (high word)
+       C_SEG,       // attempted steps at the start of this segment (segmented tracing)
        kColdSlots };
 constexpr int kKSlots2 = 11;   // + (sin, cos) of theta_n
 constexpr int kParkSlotsDp54 = 17;
@@ -71,6 +72,7 @@ template <int METRIC, int OBJ, class TR = double>
 __global__ void __launch_bounds__(kBlock, METRIC == METRIC_MN ? GP_DP54_MIN_BLOCKS_MN : GP_DP54_MIN_BLOCKS)
 trace_dp54(const __grid_constant__ TraceParams P) {
   constexpr bool DISK = (OBJ == 1), RING = (OBJ == 2), MIXED = (sizeof(TR) == 4);
+  constexpr bool SEG = (METRIC == METRIC_MN);   // segmented tracing is built into the Manko-Novikov kernels only
   extern __shared__ double2 smem2[];
   const MetricConst &mc = P.mc;
   const int tid = threadIdx.x;
@@ -127,11 +129,32 @@ trace_dp54(const __grid_constant__ TraceParams P) {
     const bool need = (mode == MODE_IDLE) && !exhausted;
     const unsigned need_mask = __ballot_sync(kFull, need);
     if (need_mask) {
-      const long long got = fetch_slot(need_mask, need, P.counters, P.cc.ray_count);
+      const bool from_list = SEG && P.round > 0;
+      const long long n_work = from_list ? (long long)*P.list_in_count : P.cc.ray_count;
+      const long long got = fetch_slot(need_mask, need, P.counters, n_work);
       if (need) {
-        const long long slot = got;
+        const long long slot = (from_list && got >= 0) ? P.list_in[got] : got;
         if (slot < 0) {
           exhausted = true;
+        } else if (from_list) {
+          // resume a parked ray: its record holds y_n, the constants, the monitors and the counters; the
+          // step proposal sits in the q_drift field (unused by this metric) and the landing-step count in
+          // n_rhs.  F(y_n) is evaluated afresh in block A — the same bits the FSAL evaluation had.
+          const double *rec = reinterpret_cast<const double *>(P.rays + slot);
+          nt = rec[0]; nr = rec[1]; nth = rec[2]; nph = rec[3];
+          nlam = rec[4]; npr = rec[6]; npth = rec[7];
+          pt = rec[8]; pph = rec[9];
+          h = rec[11];
+          const double w0 = rec[5], w1 = rec[14], w2 = rec[15];
+          n_acc = (unsigned)__double2hiint(w0);
+          n_rej = (unsigned)__double2loint(w1);
+          sts1(CS(C_HMAX), rec[10]); sts1(CS(C_QDRIFT), 0.0); sts1(CS(C_Q0), 0.0); sts1(CS(C_IQ0), 1.0);
+          sts1(CS(C_SINMIN), rec[12]); sts1(CS(C_MARGIN), rec[13]);
+          sts1(CS(C_SLOT), __longlong_as_double(slot));
+          sts1(CS(C_COUNTS), __hiloint2double(__double2hiint(w2), __double2hiint(w1)));   // n_land | n_cross
+          sts1(CS(C_STATE), __hiloint2double(__double2loint(w2), 0));                      // n_rec | status
+          sts1(CS(C_SEG), (double)(n_acc + n_rej));
+          mode = MODE_RESUME;
         } else {
           // a2 + a3
           ray_birth(P.cc, mc, P.cc.ray_begin + slot * P.cc.ray_stride, nr, nth, nph, pt, npr, npth, pph);
@@ -140,6 +163,7 @@ trace_dp54(const __grid_constant__ TraceParams P) {
           n_acc = n_rej = 0;
           sts1(CS(C_SLOT), __longlong_as_double(slot)); sts1(CS(C_COUNTS), __longlong_as_double(0LL));
           sts1(CS(C_STATE), __longlong_as_double(0LL));
+          if (SEG) sts1(CS(C_SEG), 0.0);
           const double inf = __longlong_as_double(0x7ff0000000000000LL);
           sts1(CS(C_HMAX), 0.0); sts1(CS(C_QDRIFT), 0.0); sts1(CS(C_Q0), 0.0); sts1(CS(C_IQ0), 1.0);
           sts1(CS(C_SINMIN), inf); sts1(CS(C_MARGIN), inf);
@@ -159,13 +183,13 @@ trace_dp54(const __grid_constant__ TraceParams P) {
       bool moved = false;   // y_n changed: run the stop tests' monitor on the new state
       double monH = 0.0, monQ = 0.0, monS = 0.0;
       double lam = 0.0;     // lambda of y_n, valid after this block when mode == MODE_NORMAL
-      if (mode == MODE_FRESH) {
+      if (mode == MODE_FRESH || (SEG && mode == MODE_RESUME)) {
         r = nr; th = nth; pr = npr; pth = npth; lam = nlam;
         sts1(CS(C_T), nt); sts1(CS(C_PH), nph); sts1(CS(C_LAM), nlam);
         GP_SET_K1(o7.dr, o7.dth, o7.dpr, o7.dpth)
         GP_SET_SC(o7.s, o7.c)
         sts1(CS(C_K1T), o7.dt); sts1(CS(C_K1PH), o7.dph);
-        h = P.h_cap_rel * nr;               // R10 item 4: h0 = cap x the start radius (r_obs for the pinhole)
+        if (!SEG || mode == MODE_FRESH) h = P.h_cap_rel * nr;   // R10 item 4: h0 = cap x the start radius (r_obs for the pinhole); a resumed ray keeps its proposal
         monH = fabs(0.5 * o7.H2); monQ = carter_q<METRIC>(mc, pt, pph, npth, o7); monS = fabs(o7.s);
         mode = MODE_NORMAL;
         moved = true;
@@ -364,6 +388,21 @@ trace_dp54(const __grid_constant__ TraceParams P) {
             sts1(CS(C_QDRIFT), mo.q_drift); sts1(CS(C_Q0), mo.Q0); sts1(CS(C_IQ0), mo.iQ0);
           }
         }
+        // Segmented tracing: a ray that has used up its segment parks (y_n, constants, monitors, counters, step
+        // proposal) in its own record and hands its slot to the next round; any lane picks it up there.
+        if (SEG && P.seg_steps > 0 && !finished &&
+            (long long)(n_acc + n_rej) - (long long)lds1(CS(C_SEG)) >= P.seg_steps) {
+          const long long slot = __double_as_longlong(lds1(CS(C_SLOT)));
+          const double cw = lds1(CS(C_COUNTS)), sw = lds1(CS(C_STATE));
+          Monitors mo;
+          mo.h_max = lds1(CS(C_HMAX)); mo.q_drift = h; mo.Q0 = 0.0; mo.iQ0 = 0.0;
+          mo.sin_min = lds1(CS(C_SINMIN)); mo.err_margin = lds1(CS(C_MARGIN));
+          store_record(P.rays + slot, lds1(CS(C_T)), r, th, lds1(CS(C_PH)), pr, pth, lam, pt, pph, mo, kRayParked,
+                       n_acc, n_rej, (unsigned)__double2loint(cw), (unsigned)__double2hiint(sw),
+                       (unsigned)__double2hiint(cw));
+          P.list_out[atomicAdd(P.list_out_count, 1ull)] = slot;
+          mode = MODE_IDLE;
+        }
       }
 
       if (finished) {
@@ -391,7 +430,7 @@ trace_dp54(const __grid_constant__ TraceParams P) {
         sts1(CS(C_TOT_STEPS), lds1(CS(C_TOT_STEPS)) + (double)attempts);
         sts1(CS(C_TOT_RHS), lds1(CS(C_TOT_RHS)) + (double)n_rhs);
         mode = MODE_IDLE;
-      } else {
+      } else if (!SEG || mode != MODE_IDLE) {
         // ---- C: stages 2..6 of the next attempt from (y_n, k1) ----
         // step and reciprocal selector: ordinary step s = h, divisor 1; landing s = target - y_w,
         // divisor F_w (w = r or theta).  A landing step never returns to (y_n, k1) — the ray ends

@@ -858,3 +858,31 @@ def test_mixed_precision_variant_against_the_fp64_oracle(gp, O, name, cfgo, sel)
     assert np.array_equal(rays["r"][landed], orc["r"][landed])       # the exit surface is exact
     print(name, "mixed: smooth", int(smooth.sum()), "median", float(np.median(err)), "99 %", float(np.percentile(err, 99)),
           "max", float(err.max()), "status mismatches", int(mism.sum()))
+
+
+def test_segmented_tracing_changes_nothing_but_the_balance(gp):
+    """cfg.segment_steps (Manko-Novikov, scheme 2): parking a long ray's state in its record and resuming it in
+    a later launch leaves every record identical bit for bit — with the thin disk and the ring as well."""
+    for extra in ({}, dict(max_crossings=3, disk_r_in=4.0, disk_r_out=20.0), dict(ring_half_angle=0.05, disk_r_in=5.0, disk_r_out=14.0)):
+        w = W.workload("C4", width=192, height=192, theta_obs=math.radians(82.0))
+        w["cfg"].update(max_steps=30000, **extra)
+        ref = None
+        for seg in (0, -1, 2500, 7):
+            if seg == 7:
+                w["cfg"]["max_steps"] = 600        # 86 rounds of 7 steps: the bookkeeping under stress
+                w["cfg"]["segment_steps"] = 0
+                ref = gp.api.trace_workload(w)
+            w["cfg"]["segment_steps"] = seg
+            rays, disk, counters = gp.api.trace_workload(w)
+            assert counters[1] == len(rays) and (rays["status"] <= 5).all()
+            if ref is None:
+                ref = (rays, disk, counters)
+                assert (rays["status"] == 2).sum() > 500 and (rays["status"] == 0).sum() > 20000
+                continue
+            assert rays.tobytes() == ref[0].tobytes(), (extra, seg)
+            if disk is not None:
+                assert disk.tobytes() == ref[1].tobytes(), (extra, seg)
+            assert np.array_equal(counters[1:4], ref[2][1:4])
+    w["cfg"]["segment_steps"] = -2
+    with pytest.raises(gp.api.GpError):
+        gp.api.trace_workload(w, 0, 10, 1)
