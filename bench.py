@@ -44,7 +44,12 @@ F_STEP_BUILDER = {0: 56.0, 1: 57.0, 2: 324.0}
 # per launch, of the SAME kernel build on the SAME workload, each with the profiles/ file it comes from.
 # Workloads without a capture report null and say so.
 PROFILED = {
-    ("headline", "fp64"): {"hw_fp64_frac": 0.488, "traffic": 8.41e7, "source": "profiles/trace_dp54_r02b.md"},
+    ("headline", "fp64"): {"hw_fp64_frac": 0.487, "traffic": 8.35e7, "source": "profiles/trace_dp54_r02c.md"},
+    ("headline_rk4", "fp64"): {"hw_fp64_frac": 0.489, "traffic": 8.34e7, "source": "profiles/kernels_r02.md"},
+    ("headline_rk4", "fp32"): {"hw_fp64_frac": None, "hw_fp32_frac": 0.349, "traffic": 8.16e7,
+                               "source": "profiles/kernels_r02.md"},
+    ("headline_rk4", "mixed"): {"hw_fp64_frac": 0.101, "hw_fp32_frac": 0.242, "traffic": 8.20e7,
+                                "source": "profiles/kernels_r02.md"},
 }
 # nominal FP64 FMA peak: 148 SMs x 64 FP64 FMA lanes x 2 flop x 1.965 GHz
 FP64_LANES_PER_SM = 64
@@ -406,7 +411,8 @@ def run_b200(args):
                      # not measurable inside a timed run: from the ncu --set full capture named in `profile`
                      # (dram__bytes_read.sum + dram__bytes_write.sum per launch; (2 DFMA + DMUL + DADD) / cycle
                      # over 148 SMs x 128 flop / cycle)
-                     "traffic": prof["traffic"], "hw_fp64_frac": prof["hw_fp64_frac"], "profile": prof["source"],
+                     "traffic": prof["traffic"], "hw_fp64_frac": prof["hw_fp64_frac"],
+                     "hw_fp32_frac": prof.get("hw_fp32_frac"), "profile": prof["source"],
                      "peak_kind": f"nominal {'FP32' if fp32 else 'FP64'} FMA: {props.multi_processor_count} SMs x "
                                   f"{lanes} lanes x 2 x {sm_max:.0f} MHz",
                      "peak_probe": None if fp32 else peak_probe,

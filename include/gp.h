@@ -271,7 +271,8 @@ int gp_probe_fp64_fma(int64_t iters, void *scratch, size_t scratch_bytes, double
  *     of SplitMix64(tex_seed * 0x9E3779B97F4A7C15 + j * tex_width + i) / 255; sample at
  *     u = ph/(2pi)*tex_width - 0.5 (wrapping), v = th/pi*tex_height - 0.5 (clamped).
  *   mode 2 (exit-time bands, L430): PALETTE6[floor(|t| / time_period) mod 6].
- *   disk overlay (L735; needs `disk`; takes precedence over everything above, the disk is opaque):
+ *   disk overlay (L735; needs `disk`; takes precedence over everything above, the disk is opaque; a ray that
+ *     ended on the solid ring, status HIT_RING, carries its hit in the same slot and is coloured the same way):
  *     if the first recorded crossing exists (r_cross[0] is not NaN), the colour is
  *     g < 1: blue (0.1,0.2,1) -> white by (g - g_lo)/(1 - g_lo);  g >= 1: white -> red (1,0.1,0.1)
  *     by (g - 1)/(g_hi - 1), both parameters clamped to [0, 1].
