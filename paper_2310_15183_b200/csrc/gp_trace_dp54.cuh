@@ -30,11 +30,17 @@ enum { C_T = 0, C_PH, C_LAM, C_HMAX, C_QDRIFT, C_Q0, C_IQ0, C_SINMIN, C_MARGIN, 
        C_COUNTS,    // n_equator_crossings (low word) and landing steps taken (high word)
        C_STATE,     // status of the ray once decided (low word) and disk crossings recorded (high word)
        C_SEG,       // attempted steps at the start of this segment (segmented tracing)
+       C_NREJ,      // rejected steps (touched on a rejection only; a register holds the attempts)
        kColdSlots };
 constexpr int kKSlots2 = 11;   // + (sin, cos) of theta_n
 constexpr int kParkSlotsDp54 = 17;
-constexpr size_t dp54_smem_bytes(bool disk) {
-  return sizeof(double) * kBlock * (2 * kKSlots2 + kColdSlots + (disk ? kParkSlotsDp54 : 0));
+// Every area is laid out [pair][lane] with 16 bytes per lane, so that ONE per-lane base address (plus
+// compile-time offsets) reaches everything: a double slot j of the cold or park area is half (j & 1) of
+// pair j / 2.  (With separate 8- and 16-byte strides the compiler rebuilt two or three base addresses from
+// %tid and the shared window several times per step.)
+constexpr int kColdPairs = (kColdSlots + 1) / 2, kParkPairs = (kParkSlotsDp54 + 1) / 2;
+constexpr size_t dp54_smem_bytes(bool parked) {
+  return 16 * (size_t)kBlock * (kKSlots2 + kColdPairs + (parked ? kParkPairs : 0));
 }
 // Resident blocks per SM the register allocation is held to (4 -> <= 128 registers, no spills for
 // Schwarzschild and Kerr; the Manko-Novikov duals need 2 -> <= 255).  Measured on B200 (headline):
@@ -76,12 +82,10 @@ trace_dp54(const __grid_constant__ TraceParams P) {
   extern __shared__ double2 smem2[];
   const MetricConst &mc = P.mc;
   const int tid = threadIdx.x;
-  const unsigned sm_k = (unsigned)__cvta_generic_to_shared(smem2) + 16u * tid;                  // + 16 kBlock slot
-  const unsigned sm_c = (unsigned)__cvta_generic_to_shared(smem2 + kKSlots2 * kBlock) + 8u * tid;  // + 8 kBlock slot
-  const unsigned sm_p = sm_c + 8u * kBlock * kColdSlots;
+  const unsigned sm_k = (unsigned)__cvta_generic_to_shared(smem2) + 16u * tid;   // + 16 kBlock per pair
 #define KS(slot) (sm_k + 16u * kBlock * (slot))
-#define CS(slot) (sm_c + 8u * kBlock * (slot))
-#define PS(slot) (sm_p + 8u * kBlock * (slot))
+#define CS(slot) (sm_k + 16u * kBlock * (kKSlots2 + (slot) / 2) + 8u * ((slot) & 1))
+#define PS(slot) (sm_k + 16u * kBlock * (kKSlots2 + kColdPairs + (slot) / 2) + 8u * ((slot) & 1))
 
   // ---- per-lane ray state (registers) ----
   int mode = MODE_IDLE;
@@ -94,7 +98,8 @@ trace_dp54(const __grid_constant__ TraceParams P) {
   // pending (trial) state and the error sums that still lack the e7 k7 term
   double nt = 0.0, nr = 0.0, nth = 0.0, nph = 0.0, npr = 0.0, npth = 0.0, nlam = 0.0;
   double et = 0.0, er = 0.0, eth = 0.0, eph = 0.0, epr = 0.0, epth = 0.0;
-  unsigned n_acc = 0, n_rej = 0;   // n_cross, n_land: cold slot C_COUNTS; status, n_rec: C_STATE
+  unsigned n_att = 0;   // attempted steps; n_rej: cold slot C_NREJ; n_cross, n_land: C_COUNTS; status, n_rec: C_STATE
+#define GP_BUMP_REJ() sts1(CS(C_NREJ), __hiloint2double(0, __double2loint(lds1(CS(C_NREJ))) + 1));
 #define GP_SET_STATUS(code_)                                                                   \
   {                                                                                            \
     double w_ = lds1(CS(C_STATE));                                                             \
@@ -146,21 +151,22 @@ trace_dp54(const __grid_constant__ TraceParams P) {
           pt = rec[8]; pph = rec[9];
           h = rec[11];
           const double w0 = rec[5], w1 = rec[14], w2 = rec[15];
-          n_acc = (unsigned)__double2hiint(w0);
-          n_rej = (unsigned)__double2loint(w1);
+          n_att = (unsigned)__double2hiint(w0) + (unsigned)__double2loint(w1);
+          sts1(CS(C_NREJ), __hiloint2double(0, __double2loint(w1)));
           sts1(CS(C_HMAX), rec[10]); sts1(CS(C_QDRIFT), 0.0); sts1(CS(C_Q0), 0.0); sts1(CS(C_IQ0), 1.0);
           sts1(CS(C_SINMIN), rec[12]); sts1(CS(C_MARGIN), rec[13]);
           sts1(CS(C_SLOT), __longlong_as_double(slot));
           sts1(CS(C_COUNTS), __hiloint2double(__double2hiint(w2), __double2hiint(w1)));   // n_land | n_cross
           sts1(CS(C_STATE), __hiloint2double(__double2loint(w2), 0));                      // n_rec | status
-          sts1(CS(C_SEG), (double)(n_acc + n_rej));
+          sts1(CS(C_SEG), (double)n_att);
           mode = MODE_RESUME;
         } else {
           // a2 + a3
           ray_birth(P.cc, mc, P.cc.ray_begin + slot * P.cc.ray_stride, nr, nth, nph, pt, npr, npth, pph);
           nt = 0.0; nlam = 0.0;
           mode = MODE_FRESH;
-          n_acc = n_rej = 0;
+          n_att = 0;
+          sts1(CS(C_NREJ), __longlong_as_double(0LL));
           sts1(CS(C_SLOT), __longlong_as_double(slot)); sts1(CS(C_COUNTS), __longlong_as_double(0LL));
           sts1(CS(C_STATE), __longlong_as_double(0LL));
           if (SEG) sts1(CS(C_SEG), 0.0);
@@ -191,6 +197,12 @@ trace_dp54(const __grid_constant__ TraceParams P) {
         sts1(CS(C_K1T), o7.dt); sts1(CS(C_K1PH), o7.dph);
         if (!SEG || mode == MODE_FRESH) h = P.h_cap_rel * nr;   // R10 item 4: h0 = cap x the start radius (r_obs for the pinhole); a resumed ray keeps its proposal
         monH = fabs(0.5 * o7.H2); monQ = carter_q<METRIC>(mc, pt, pph, npth, o7); monS = fabs(o7.s);
+        if (METRIC != METRIC_MN && mode == MODE_FRESH) {
+          // the reference value of the Carter monitor (R23) is set here, once per ray, so that the per-step
+          // monitor below carries no "first step" instructions
+          sts1(CS(C_Q0), monQ);
+          sts1(CS(C_IQ0), rcp_nr(dmax(1.0, fabs(monQ))));
+        }
         mode = MODE_NORMAL;
         moved = true;
       } else if (mode == MODE_NORMAL) {
@@ -225,7 +237,8 @@ trace_dp54(const __grid_constant__ TraceParams P) {
         // finite test on the sums: any inf/NaN term makes them non-finite (numerators are >= 0)
         double err = div_nr(nm, dn, rcp_nr(dn));
         if (!finite_d(nsum) || !finite_d(err)) {
-          ++n_rej;
+          ++n_att;
+          GP_BUMP_REJ()
           h *= dp.fac_min;
         } else {
           sts1(CS(C_MARGIN), dmin(lds1(CS(C_MARGIN)), fabs(err - 1.0)));
@@ -234,10 +247,11 @@ trace_dp54(const __grid_constant__ TraceParams P) {
           double fac = dp.safety * pow_m1_5_clamped(err);
           fac = dmin(dmax(dp.fac_min, fac), dp.fac_max);
           if (err > 1.0) {
-            ++n_rej;
+            ++n_att;
+            GP_BUMP_REJ()
             h *= fac;
           } else {
-            ++n_acc;
+            ++n_att;
             double hnext = dmin(h * fac, P.h_cap_rel * nr);
             if (nr > P.r_esc || nr < P.r_cap) {
               // O8: discard the step, land on the surface from y_n
@@ -372,26 +386,25 @@ trace_dp54(const __grid_constant__ TraceParams P) {
       // stop tests in the oracle's order (R18, R10 item 5), then the monitors of the new state (R22)
       if (mode == MODE_NORMAL) {
         // max_steps <= 5e8 (validated by the host) fits the 32-bit counters; lambda_max is +inf when off
-        if (n_acc + n_rej >= (unsigned)P.max_steps || lam >= P.lambda_max) {
+        if (n_att >= (unsigned)P.max_steps || lam >= P.lambda_max) {
           GP_SET_STATUS(GP_RAY_MAXSTEPS)
           finished = true;
-        } else if (h < dp.h_floor || h < dp.h_floor * fabs(lam)) {   // h < h_floor max(1, |lambda|)
+        } else if (h < dp.h_floor * dmax(1.0, fabs(lam))) {   // R10 item 5 (compare + select, no fmax)
           GP_SET_STATUS(GP_RAY_STEP_UNDERFLOW)
           finished = true;
         } else if (moved) {
           Monitors mo;
           mo.h_max = lds1(CS(C_HMAX)); mo.q_drift = lds1(CS(C_QDRIFT)); mo.Q0 = lds1(CS(C_Q0));
           mo.iQ0 = lds1(CS(C_IQ0)); mo.sin_min = lds1(CS(C_SINMIN)); mo.err_margin = 0.0;
-          monitor_apply<METRIC>(mo, monH, monQ, monS, n_acc == 0 && n_rej == 0);
+          monitor_apply<METRIC>(mo, monH, monQ, monS, false);
           sts1(CS(C_HMAX), mo.h_max); sts1(CS(C_SINMIN), mo.sin_min);
-          if (METRIC != METRIC_MN) {
-            sts1(CS(C_QDRIFT), mo.q_drift); sts1(CS(C_Q0), mo.Q0); sts1(CS(C_IQ0), mo.iQ0);
-          }
+          if (METRIC != METRIC_MN) sts1(CS(C_QDRIFT), mo.q_drift);
         }
         // Segmented tracing: a ray that has used up its segment parks (y_n, constants, monitors, counters, step
         // proposal) in its own record and hands its slot to the next round; any lane picks it up there.
         if (SEG && P.seg_steps > 0 && !finished &&
-            (long long)(n_acc + n_rej) - (long long)lds1(CS(C_SEG)) >= P.seg_steps) {
+            (long long)n_att - (long long)lds1(CS(C_SEG)) >= P.seg_steps) {
+          const unsigned n_rej = (unsigned)__double2loint(lds1(CS(C_NREJ))), n_acc = n_att - n_rej;
           const long long slot = __double_as_longlong(lds1(CS(C_SLOT)));
           const double cw = lds1(CS(C_COUNTS)), sw = lds1(CS(C_STATE));
           Monitors mo;
@@ -406,7 +419,8 @@ trace_dp54(const __grid_constant__ TraceParams P) {
       }
 
       if (finished) {
-        unsigned attempts = n_acc + n_rej;
+        const unsigned attempts = n_att;
+        const unsigned n_rej = (unsigned)__double2loint(lds1(CS(C_NREJ))), n_acc = n_att - n_rej;
         const long long slot = __double_as_longlong(lds1(CS(C_SLOT)));
         const double cw = lds1(CS(C_COUNTS));
         const unsigned n_cross = (unsigned)__double2loint(cw), n_land = (unsigned)__double2hiint(cw);
