@@ -82,7 +82,10 @@ trace_dp54(const __grid_constant__ TraceParams P) {
   extern __shared__ double2 smem2[];
   const MetricConst &mc = P.mc;
   const int tid = threadIdx.x;
-  const unsigned sm_k = (unsigned)__cvta_generic_to_shared(smem2) + 16u * tid;   // + 16 kBlock per pair
+  // the one per-lane base address, produced by an asm volatile so that ptxas keeps it in a register
+  // instead of rebuilding it from %tid and the shared window two or three times per step
+  unsigned sm_k;
+  asm volatile("mad.lo.u32 %0, %1, 16, %2;" : "=r"(sm_k) : "r"(tid), "r"((unsigned)__cvta_generic_to_shared(smem2)));
 #define KS(slot) (sm_k + 16u * kBlock * (slot))
 #define CS(slot) (sm_k + 16u * kBlock * (kKSlots2 + (slot) / 2) + 8u * ((slot) & 1))
 #define PS(slot) (sm_k + 16u * kBlock * (kKSlots2 + kColdPairs + (slot) / 2) + 8u * ((slot) & 1))
