@@ -248,7 +248,7 @@ trace_dp54(const __grid_constant__ TraceParams P) {
           // fac = 0.9 err^(-1/5), clamped to [0.2, 5] (err = 0 gives 5); the clamp of err keeps the
           // FP32 seed of pow_m1_5 in range and changes nothing: 0.9 (1e-5)^-0.2 = 9 > 5, 0.9 (1e4)^-0.2 = 0.14 < 0.2
           double fac = dp.safety * pow_m1_5_clamped(err);
-          fac = dmin(dmax(dp.fac_min, fac), dp.fac_max);
+          fac = dmin(dmax(dp.fac_min, fac), 5.0);   // R10 item 3 (5.0 as an immediate)
           if (err > 1.0) {
             ++n_att;
             GP_BUMP_REJ()
