@@ -22,9 +22,9 @@ namespace gp {
 constexpr int kParkSlotsRk4 = 7;  // trial state (r, th, pr, pth, t, ph, lambda) across an equator landing
 
 // (the disk variant of the FP64 Kerr kernel needs a few registers more than the 128 that four resident
-// blocks allow: it is held to three)
+// blocks allow: it is held to three; the FP64 Manko-Novikov duals need up to 255: two blocks)
 template <int METRIC, bool DISK, class T, class S = T>
-__global__ void __launch_bounds__(kBlock, (DISK && sizeof(T) == 8 && METRIC == METRIC_KERR) ? 3 : 0) trace_rk4(const __grid_constant__ TraceParams P) {
+__global__ void __launch_bounds__(kBlock, (sizeof(T) == 8 && METRIC == METRIC_MN) ? 2 : ((DISK && sizeof(T) == 8 && METRIC == METRIC_KERR) ? 3 : 0)) trace_rk4(const __grid_constant__ TraceParams P) {
   extern __shared__ double park_raw[];  // [kParkSlotsRk4][kBlock] of S when DISK
   S *park = reinterpret_cast<S *>(park_raw);
   const MetricConst &mc = P.mc;
