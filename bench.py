@@ -44,11 +44,11 @@ F_STEP_BUILDER = {0: 56.0, 1: 57.0, 2: 324.0}
 # per launch, of the SAME kernel build on the SAME workload, each with the profiles/ file it comes from.
 # Workloads without a capture report null and say so.
 PROFILED = {
-    ("headline", "fp64"): {"hw_fp64_frac": 0.487, "traffic": 8.35e7, "source": "profiles/trace_dp54_r02c.md"},
-    ("headline_rk4", "fp64"): {"hw_fp64_frac": 0.489, "traffic": 8.34e7, "source": "profiles/kernels_r02.md"},
-    ("headline_rk4", "fp32"): {"hw_fp64_frac": None, "hw_fp32_frac": 0.349, "traffic": 8.16e7,
+    ("headline", "fp64"): {"hw_fp64_frac": 0.510, "traffic": 8.25e7, "source": "profiles/trace_dp54_r02e.md"},
+    ("headline_rk4", "fp64"): {"hw_fp64_frac": 0.494, "traffic": 8.35e7, "source": "profiles/kernels_r02.md"},
+    ("headline_rk4", "fp32"): {"hw_fp64_frac": None, "hw_fp32_frac": 0.349, "traffic": 8.28e7,
                                "source": "profiles/kernels_r02.md"},
-    ("headline_rk4", "mixed"): {"hw_fp64_frac": 0.101, "hw_fp32_frac": 0.242, "traffic": 8.20e7,
+    ("headline_rk4", "mixed"): {"hw_fp64_frac": 0.096, "hw_fp32_frac": 0.230, "traffic": 8.17e7,
                                 "source": "profiles/kernels_r02.md"},
 }
 # nominal FP64 FMA peak: 148 SMs x 64 FP64 FMA lanes x 2 flop x 1.965 GHz

@@ -16,14 +16,18 @@ namespace gp {
 #if defined(__CUDACC__)
 
 // Shared-memory plan, per lane.  Registers hold only what every stage
-// touches; the rest lives in shared memory so that five blocks (20 warps) fit per SM:
-//   K area   8 x double2   stage slopes K2..K5 of (r, th) and (p_r, p_th); K1 and the newest K stay
-//                          in registers.  128-bit accesses, [slot][lane] layout: conflict-free.
-//   cold     kColdSlots x double   state the stages never read: t, phi, lambda, the monitors, the
-//                          landing target, k1 of the two quadratures, the per-lane totals.
-//   park     17 x double   (DISK only) what a ray resumes from after an equator landing step:
-//                          trial state (r, th, pr, pth, t, ph, lambda), next step, raw k7 (6) and
-//                          its monitor triple.
+// touches; the rest lives in shared memory so that four blocks (16 warps) fit per SM in 128 registers.
+// Everything is laid out [pair][lane], 16 bytes per lane, behind ONE per-lane base address:
+//   K area   11 x double2  stage slopes K2..K5 of (r, th) and (p_r, p_th) (pairs 0-7), the RAW k1 = F(y_n)
+//                          of the same four components (pairs 8, 9; read once per attempt, so that a
+//                          rejected step retries from it) and (sin, cos) theta_n (pair 10).  128-bit
+//                          accesses, conflict-free.
+//   cold     kColdSlots x double (two per pair)   state the stages never read: t, phi, lambda, the monitors,
+//                          the landing target, k1 of the two quadratures, the per-lane totals, the output
+//                          slot, the rare counters, status, segment start.
+//   park     17 x double   (disk and ring variants) what a ray resumes from after a landing step located
+//                          something on the way: trial state (r, th, pr, pth, t, ph, lambda), next step,
+//                          raw k7 (6) and its monitor triple.
 enum { C_T = 0, C_PH, C_LAM, C_HMAX, C_QDRIFT, C_Q0, C_IQ0, C_SINMIN, C_MARGIN, C_TARGET, C_K1T, C_K1PH,
        C_TOT_RAYS, C_TOT_STEPS, C_TOT_RHS,
        C_SLOT,      // output slot of the ray in flight (64-bit integer bits)
