@@ -243,22 +243,21 @@ trace_dp54(const __grid_constant__ TraceParams P) {
 #undef GP_SCALE
         // finite test on the sums: any inf/NaN term makes them non-finite (numerators are >= 0)
         double err = div_nr(nm, dn, rcp_nr(dn));
-        if (!finite_d(nsum) || !finite_d(err)) {
-          ++n_att;
-          GP_BUMP_REJ()
-          h *= dp.fac_min;
-        } else {
-          sts1(CS(C_MARGIN), dmin(lds1(CS(C_MARGIN)), fabs(err - 1.0)));
-          // fac = 0.9 err^(-1/5), clamped to [0.2, 5] (err = 0 gives 5); the clamp of err keeps the
-          // FP32 seed of pow_m1_5 in range and changes nothing: 0.9 (1e-5)^-0.2 = 9 > 5, 0.9 (1e4)^-0.2 = 0.14 < 0.2
-          double fac = dp.safety * pow_m1_5_clamped(err);
-          fac = dmin(dmax(dp.fac_min, fac), 5.0);   // R10 item 3 (5.0 as an immediate)
-          if (err > 1.0) {
-            ++n_att;
+        // R10 item 2: a non-finite estimate or trial state is a rejection with the factor 0.2.  The two kinds of
+        // rejection share one (rare) block, so that neither is if-converted into predicated instructions that
+        // every step would issue.
+        const bool bad = !finite_d(nsum) || !finite_d(err);
+        if (!bad) sts1(CS(C_MARGIN), dmin(lds1(CS(C_MARGIN)), fabs(err - 1.0)));
+        // fac = 0.9 err^(-1/5), clamped to [0.2, 5] (err = 0 gives 5); the range clamp sits on the FP32 seed
+        // of the fifth root and changes nothing: 0.9 (1e-5)^-0.2 = 9 > 5, 0.9 (1e4)^-0.2 = 0.14 < 0.2
+        double fac = dp.safety * pow_m1_5_clamped(err);
+        fac = dmin(dmax(dp.fac_min, fac), 5.0);   // R10 item 3 (5.0 as an immediate)
+        ++n_att;
+        {
+          if (bad || err > 1.0) {
             GP_BUMP_REJ()
-            h *= fac;
+            h *= bad ? dp.fac_min : fac;
           } else {
-            ++n_att;
             double hnext = dmin(h * fac, P.h_cap_rel * nr);
             if (nr > P.r_esc || nr < P.r_cap) {
               // O8: discard the step, land on the surface from y_n
@@ -393,11 +392,10 @@ trace_dp54(const __grid_constant__ TraceParams P) {
       // stop tests in the oracle's order (R18, R10 item 5), then the monitors of the new state (R22)
       if (mode == MODE_NORMAL) {
         // max_steps <= 5e8 (validated by the host) fits the 32-bit counters; lambda_max is +inf when off
-        if (n_att >= (unsigned)P.max_steps || lam >= P.lambda_max) {
-          GP_SET_STATUS(GP_RAY_MAXSTEPS)
-          finished = true;
-        } else if (h < dp.h_floor * dmax(1.0, fabs(lam))) {   // R10 item 5 (compare + select, no fmax)
-          GP_SET_STATUS(GP_RAY_STEP_UNDERFLOW)
+        const bool budget = n_att >= (unsigned)P.max_steps || lam >= P.lambda_max;
+        const bool underflow = h < dp.h_floor * dmax(1.0, fabs(lam));   // R10 item 5 (compare + select, no fmax)
+        if (budget || underflow) {            // one rare block for both
+          GP_SET_STATUS(budget ? GP_RAY_MAXSTEPS : GP_RAY_STEP_UNDERFLOW)
           finished = true;
         } else if (moved) {
           Monitors mo;
