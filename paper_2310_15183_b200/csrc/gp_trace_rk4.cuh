@@ -59,7 +59,18 @@ __global__ void __launch_bounds__(kBlock, (sizeof(T) == 8 && METRIC == METRIC_MN
           t = S(0); r = (S)dr0; th = (S)dth0; ph = (S)dph0; lam = S(0);
           mode = MODE_NORMAL;
           n_acc = n_cross = n_rec = n_land = 0;
-          mo.h_max = T(0); mo.q_drift = T(0); mo.Q0 = T(0);
+          mo.h_max = T(0); mo.q_drift = T(0); mo.Q0 = T(0); mo.iQ0 = T(1);
+          if (METRIC != METRIC_MN) {
+            // Reference value of the Carter monitor (R23), once per ray, from the initial state (H = 0 there
+            // by construction, so the term in H is left out: a 1e-16 relative difference to the value taken
+            // at the first step) — the per-step monitor then carries no "first step" instructions.
+            double s0, c0;
+            sincos(dth0, &s0, &c0);
+            const double a2 = (METRIC == METRIC_KERR) ? mc.a2 : 0.0;
+            const double q0 = dpth * dpth + c0 * c0 * (dpph * dpph / (s0 * s0) - a2 * dpt * dpt);
+            mo.Q0 = (T)q0;
+            mo.iQ0 = (T)(1.0 / fmax(1.0, fabs(q0)));
+          }
           mo.sin_min = (T)__longlong_as_double(0x7ff0000000000000LL);
           mo.err_margin = (T)__longlong_as_double(0x7ff0000000000000LL);
         }
@@ -94,7 +105,7 @@ __global__ void __launch_bounds__(kBlock, (sizeof(T) == 8 && METRIC == METRIC_MN
         rhs_eval<METRIC>(mc, pt, pph, (T)r, (T)th, (T)pr, (T)pth, o);
         if (normal)
           monitor_apply<METRIC>(mo, (T)fabs(T(0.5) * o.H2), carter_q<METRIC>(mc, pt, pph, (T)pth, o), (T)fabs(o.s),
-                                n_acc == 0);
+                                false);
         GP_HENON(1.0, true)
         // Stage angles (Schwarzschild, Kerr): sin, cos of theta_n + d from (sin, cos) theta_n — by-products of
         // k1 — through the addition theorems: no range reduction or quadrant logic in stages 2-4.  A fixed
