@@ -587,14 +587,19 @@ def test_no_write_outside_the_callers_buffers(gp):
     ragged ray counts, both kernels, the disk variant and the image-formation kernel."""
     import torch
     G = 4096
-    for name, count in (("C2", 1), ("C2", 1000), ("C3", 777), ("C1", 4096), ("C5a", 333)):
+    for name, count, extra in (("C2", 1, {}), ("C2", 1000, {}), ("C3", 777, {}), ("C1", 4096, {}), ("C5a", 333, {}),
+                               ("C3", 555, dict(max_crossings=0, ring_half_angle=0.05, disk_r_in=0.0)),      # solid ring
+                               ("C5a", 333, dict(precision=2)), ("C2", 333, dict(precision=2, rtol=1e-7, atol=1e-7)),
+                               ("C4", 200, dict(max_steps=3000, segment_steps=500))):                         # segmented
         w = W.workload(name)
+        w["cfg"].update(extra)
         w["cfg"]["max_steps"] = min(w["cfg"]["max_steps"], 20000)
         b, c, s = W.ray_selection(w, 17, count, 5)
         cam = gp.api.camera_struct(w["camera"], b, c, s)
         cfg = gp.api.cfg_struct(w["cfg"])
         bufs = {}
-        for key, nbytes in (("rays", c * 128), ("disk", c * 48 if cfg.max_crossings else 0), ("counters", 64)):
+        for key, nbytes in (("rays", c * 128), ("disk", c * 48 if (cfg.max_crossings or cfg.ring_half_angle > 0) else 0),
+                            ("counters", 64)):
             if nbytes == 0:
                 bufs[key] = (None, None)
                 continue
@@ -610,7 +615,7 @@ def test_no_write_outside_the_callers_buffers(gp):
         cnt = bufs["counters"][1].cpu().numpy().view("<u8")
         assert cnt[1] == c
         rec = bufs["rays"][1].cpu().numpy().view(gp.api.RAY_DTYPE)
-        assert (rec["status"] <= 4).all() and np.isfinite(rec["lambda"]).all()
+        assert (rec["status"] <= 5).all() and np.isfinite(rec["lambda"]).all()
     # image formation
     w = W.workload("C2", width=50, height=30, supersample=2)
     rays, _, _ = gp.api.trace_workload(w)
