@@ -6,13 +6,19 @@
  * paper_2310_15183_b200/csrc); its structs are declared here independently.  Only tests/,
  * __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may use it.
  *
- * Pins (tests/test_oracle_*.py, all `-m "not gpu"`): flat-space closed form, Schwarzschild
- * critical impact parameter and deflection quadrature, Kerr radial-potential classifier and
- * Bardeen's critical curve, Carter constant, photon-orbit and ISCO radii, Manko-Novikov ->
- * Kerr at q = 0, Manko-Novikov vacuum (Ernst) equations, equatorial mirror symmetry,
- * Dormand-Prince order conditions, scipy DOP853 trajectories.
- * Parity unpinned: exit angles inside Manko-Novikov chaotic sets and any state of a
- * MAXSTEPS ray (statistical comparison only, R21).
+ * Pins (tests/test_oracle_*.py, tests/test_golden_closed_forms.py, all `-m "not gpu"`): flat-space closed
+ * form, Schwarzschild critical impact parameter and deflection quadrature, Kerr radial-potential classifier
+ * and Bardeen's critical curve, Carter constant, photon-orbit and ISCO radii, Manko-Novikov -> Kerr at
+ * q = 0, Manko-Novikov vacuum (Ernst) equations, the Manko-Novikov inverse metric against a 50-digit mpmath
+ * evaluation of eq 20-39, equatorial mirror symmetry, Dormand-Prince order conditions, the step-size
+ * controller and error norm re-enacted from the published tableau (test_oracle_controller_pin.py), scipy
+ * DOP853 trajectories, eq 56 against the closed-form Keplerian emitter and a dynamic circular-orbit check,
+ * the solid ring against a brute-force straight-line entry search in flat space, its thin limit and mirror
+ * symmetry (test_oracle_ring_pins.py), the image-formation oracle against a vectorised restatement of
+ * the contract text (test_oracle_shade_contract.py).
+ * Parity unpinned: exit angles inside Manko-Novikov chaotic sets, any state of a MAXSTEPS ray, and the exit
+ * state of Manko-Novikov CAPTURED rays that the rounding probe flags (statistical / status-only comparison;
+ * DESIGN.md section 5, R21, R24).
  */
 #ifndef GP_ORACLE_H_
 #define GP_ORACLE_H_
