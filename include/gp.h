@@ -119,13 +119,14 @@ typedef struct gp_integrator_cfg {
    * r, theta).  Opaque: the ray ends with status GP_RAY_HIT_RING at the point where it ENTERS the
    * volume.  An accepted, non-terminal step y_n -> y_{n+1} is examined when every coordinate (r, theta)
    * that starts outside its interval ends inside it or beyond it; the entry is located from y_n by the
-   * landing step of scheme 2 on the theta-face on y_n's side (a hit if the landed radius is in range),
+   * landing step (R14) on the theta-face on y_n's side (a hit if the landed radius is in range),
    * else on the radial face on y_n's side (a hit if the landed theta is in the slab); otherwise the ray
    * goes on from y_{n+1} (reading R39).  The record holds the state at the hit; disk record
    * slot 0 holds the hit radius and g of the circular equatorial emitter at that radius (eq 56-57), the
-   * other slots NaN.  Requires scheme 2, max_crossings = 0, a disk buffer; Manko-Novikov needs an explicit
-   * disk_r_in.  0 = no ring.  Values < 0 or >= 1.5 -> GP_E_BAD_PARAM; with scheme 0 / 1 or
-   * max_crossings > 0 -> GP_E_UNSUPPORTED.                                                              */
+   * other slots NaN.  Every scheme and precision except the mixed adaptive kernel (the landing steps use the
+   * scheme's own formula).  Requires max_crossings = 0 and a disk buffer; Manko-Novikov needs an explicit
+   * disk_r_in.  0 = no ring.  Values < 0 or >= 1.5 -> GP_E_BAD_PARAM; with max_crossings > 0 ->
+   * GP_E_UNSUPPORTED.                                                              */
   double ring_half_angle;
 } gp_integrator_cfg;
 

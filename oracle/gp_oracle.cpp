@@ -961,8 +961,8 @@ static int valid_run(const orc_metric *m, const orc_camera *cam, const orc_cfg *
   if (cfg->scheme < 0 || cfg->scheme > 2) return 0;
   if (cfg->max_crossings < 0 || cfg->max_crossings > 3) return 0;
   if (!(cfg->ring_half_angle >= 0.0) || cfg->ring_half_angle >= 1.5) return 0;
-  if (cfg->ring_half_angle > 0.0 && (cfg->max_crossings > 0 || cfg->scheme != 2 || !(cfg->disk_r_out >= cfg->disk_r_in)))
-    return 0;   // the ring replaces the thin disk; located hits are built for the adaptive scheme
+  if (cfg->ring_half_angle > 0.0 && (cfg->max_crossings > 0 || !(cfg->disk_r_out >= cfg->disk_r_in)))
+    return 0;   // the ring replaces the thin disk
   if (cfg->ring_half_angle > 0.0 && m->id == 2 && !(cfg->disk_r_in > 0.0)) return 0;
   if (cfg->max_crossings > 0 && m->id == 2 && !(cfg->disk_r_in > 0.0)) return 0;  // no ISCO formula for Manko-Novikov
   if (cam->width <= 0 || cam->height <= 0 || cam->supersample <= 0) return 0;

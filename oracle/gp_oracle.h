@@ -61,7 +61,8 @@ typedef struct orc_cfg {
    * thickness", hit when "the ray propagat[es] to a point inside the volume"): the set
    * disk_r_in <= r <= disk_r_out, |theta - pi/2| <= ring_half_angle.  Opaque: the ray ends there with
    * status 5, located on the face it entered through (see trace_ray); disk_r[0], disk_g[0] = hit radius
-   * and redshift factor of the circular equatorial emitter at that radius.  Needs max_crossings = 0. */
+   * and redshift factor of the circular equatorial emitter at that radius.  Needs max_crossings = 0;
+   * every scheme (the landing steps use the scheme's own formula, R14). */
   double ring_half_angle;
 } orc_cfg;
 

@@ -189,7 +189,7 @@ int make_params(int metric_id, const gp_metric_params *m, const gp_camera *cam, 
   // solid ring (gp.h): replaces the thin disk, located hits exist for the adaptive scheme
   if (!(cfg->ring_half_angle >= 0.0) || !(cfg->ring_half_angle < 1.5)) return GP_E_BAD_PARAM;
   const bool ring = cfg->ring_half_angle > 0.0;
-  if (ring && (cfg->scheme != 2 || cfg->max_crossings > 0)) return GP_E_UNSUPPORTED;
+  if (ring && cfg->max_crossings > 0) return GP_E_UNSUPPORTED;
   if (ring && metric_id == GP_MANKO_NOVIKOV && !(cfg->disk_r_in > 0.0)) return GP_E_BAD_PARAM;
   P->scheme = cfg->scheme;
   P->precision = cfg->precision;
@@ -270,12 +270,11 @@ int launch_info(Kernel kernel, size_t smem, LaunchInfo *slot, LaunchInfo *out) {
 // OBJ: 0 no object, 1 thin disk with recorded crossings, 2 solid ring (scheme 2 only)
 template <int METRIC, int OBJ>
 int launch_one(const TraceParams &P, cudaStream_t stream) {
-  constexpr bool DISK = (OBJ == 1);
   static LaunchInfo cache[kMaxDevices][5];   // per device: dp54, rk4 FP64 / FP32 / mixed, dp54 mixed (zero-initialised)
   const bool dp54 = (P.scheme == 2);
   const int prec = P.precision;   // 0 FP64, 1 FP32, 2 FP32 equations + FP64 state
   const size_t smem = dp54 ? dp54_smem_bytes(OBJ != 0)
-                           : (DISK ? (prec == 1 ? sizeof(float) : sizeof(double)) * kBlock * kParkSlotsRk4 : 0);
+                           : (OBJ != 0 ? (prec == 1 ? sizeof(float) : sizeof(double)) * kBlock * kParkSlotsRk4 : 0);
   int dev = 0;
   GP_CUDA(cudaGetDevice(&dev));
   if (dev < 0 || dev >= kMaxDevices) return GP_E_UNSUPPORTED;
@@ -301,11 +300,11 @@ int launch_one(const TraceParams &P, cudaStream_t stream) {
       GP_GO((trace_dp54<METRIC, OBJ>))
     }
   } else if (prec == 1) {
-    GP_GO((trace_rk4<METRIC, DISK, float>))
+    GP_GO((trace_rk4<METRIC, OBJ, float>))
   } else if (prec == 2) {
-    GP_GO((trace_rk4<METRIC, DISK, float, double>))
+    GP_GO((trace_rk4<METRIC, OBJ, float, double>))
   } else {
-    GP_GO((trace_rk4<METRIC, DISK, double>))
+    GP_GO((trace_rk4<METRIC, OBJ, double>))
   }
 #undef GP_GO
   GP_CUDA(cudaGetLastError());

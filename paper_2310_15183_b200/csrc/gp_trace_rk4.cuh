@@ -23,9 +23,12 @@ constexpr int kParkSlotsRk4 = 7;  // trial state (r, th, pr, pth, t, ph, lambda)
 
 // (the disk variant of the FP64 Kerr kernel needs a few registers more than the 128 that four resident
 // blocks allow: it is held to three; the FP64 Manko-Novikov duals need up to 255: two blocks)
-template <int METRIC, bool DISK, class T, class S = T>
-__global__ void __launch_bounds__(kBlock, (sizeof(T) == 8 && METRIC == METRIC_MN) ? 2 : ((DISK && sizeof(T) == 8 && METRIC == METRIC_KERR) ? 3 : 0)) trace_rk4(const __grid_constant__ TraceParams P) {
-  extern __shared__ double park_raw[];  // [kParkSlotsRk4][kBlock] of S when DISK
+// OBJ: 0 no object; 1 thin disk, crossings located and recorded (R19); 2 solid ring, the ray ends where it
+// enters the volume (R39).  Both objects use the park area.
+template <int METRIC, int OBJ, class T, class S = T>
+__global__ void __launch_bounds__(kBlock, (sizeof(T) == 8 && METRIC == METRIC_MN) ? 2 : ((OBJ != 0 && sizeof(T) == 8 && METRIC == METRIC_KERR) ? 3 : 0)) trace_rk4(const __grid_constant__ TraceParams P) {
+  constexpr bool DISK = (OBJ == 1), RING = (OBJ == 2);
+  extern __shared__ double park_raw[];  // [kParkSlotsRk4][kBlock] of S when OBJ != 0
   S *park = reinterpret_cast<S *>(park_raw);
   const MetricConst &mc = P.mc;
   const int tid = threadIdx.x;
@@ -40,6 +43,16 @@ __global__ void __launch_bounds__(kBlock, (sizeof(T) == 8 && METRIC == METRIC_MN
   unsigned n_acc = 0, n_cross = 0, n_rec = 0, n_land = 0, status = 0;
   bool exhausted = false;
   unsigned long long tot_rays = 0, tot_steps = 0, tot_rhs = 0;
+// the ray goes on from the trial state parked before a landing step (thin disk: always; ring: no hit); the
+// ring variant counts the equator crossing of that step here, as the oracle does after its ring test
+#define GP_RESUME_PARKED()                                                                    \
+  {                                                                                           \
+    const S *pk = park + tid;                                                                 \
+    if (RING && (th - half_pi) * (pk[1 * kBlock] - half_pi) < S(0)) ++n_cross;                \
+    r = pk[0 * kBlock]; th = pk[1 * kBlock]; pr = pk[2 * kBlock]; pth = pk[3 * kBlock];       \
+    t = pk[4 * kBlock]; ph = pk[5 * kBlock]; lam = pk[6 * kBlock];                            \
+    mode = MODE_NORMAL;                                                                       \
+  }
   stamp_start(P.counters);
 
   for (;;) {
@@ -164,27 +177,89 @@ __global__ void __launch_bounds__(kBlock, (sizeof(T) == 8 && METRIC == METRIC_MN
             mode = MODE_LAND_R;
           } else {
             bool commit = true;
-            if ((th - half_pi) * (nth - half_pi) < S(0)) {
+#define GP_PARK()                                                                                      \
+  {                                                                                                    \
+    S *pk = park + tid;                                                                                \
+    pk[0 * kBlock] = nr; pk[1 * kBlock] = nth; pk[2 * kBlock] = npr; pk[3 * kBlock] = npth;            \
+    pk[4 * kBlock] = nt; pk[5 * kBlock] = nph; pk[6 * kBlock] = lam + s;                               \
+  }
+            bool ring_try = false;
+            if (RING) {
+              // R39: the step can meet the box r_in..r_out x |theta - pi/2| <= d only if every coordinate that
+              // starts outside its interval ends inside it or beyond it (see gp_trace_dp54.cuh, gp.h)
+              const S rin = (S)P.disk_r_in, rout = (S)P.disk_r_out, rd = (S)P.ring_d;
+              const S un = th - half_pi, un1 = nth - half_pi;
+              const bool th_out = fabs(un) > rd;
+              const bool r_out_n = !(r >= rin && r <= rout);
+              const bool th_enters = fabs(un1) <= rd || un * un1 < S(0);
+              const bool r_enters = (nr >= rin && nr <= rout) || ((r < rin) != (nr < rin));
+              ring_try = (th_out || r_out_n) && (!th_out || th_enters) && (!r_out_n || r_enters);
+              if (ring_try) {
+                GP_PARK()
+                if (th_out) {
+                  target = half_pi + (un > S(0) ? rd : -rd);
+                  mode = MODE_LAND_TH;
+                } else {
+                  status = GP_RAY_HIT_RING;
+                  target = (r < rin) ? rin : rout;
+                  mode = MODE_LAND_R;
+                }
+                commit = false;
+              }
+            }
+            if (!ring_try && (th - half_pi) * (nth - half_pi) < S(0)) {
               ++n_cross;
               if (DISK && n_rec < (unsigned)P.max_crossings) {
-                S *pk = park + tid;
-                pk[0 * kBlock] = nr; pk[1 * kBlock] = nth; pk[2 * kBlock] = npr; pk[3 * kBlock] = npth;
-                pk[4 * kBlock] = nt; pk[5 * kBlock] = nph; pk[6 * kBlock] = lam + s;
+                GP_PARK()
                 target = half_pi;
                 mode = MODE_LAND_TH;
                 commit = false;
               }
             }
+#undef GP_PARK
             if (commit) {
               t = nt; r = nr; th = nth; ph = nph; pr = npr; pth = npth; lam += s;
             }
           }
         } else if (land_r) {
-          t = nt; r = target; th = nth; ph = nph; pr = npr; pth = npth; lam = lam + w * sl;
           ++n_land;
-          finished = true;
+          bool resume = false;
+          if (RING && status == GP_RAY_HIT_RING) {
+            // radial face of the ring: a hit if the landed theta is inside the slab, else the ray goes on
+            if (fabs(nth - half_pi) <= (S)P.ring_d) {
+              P.disk[slot].r_cross[0] = (double)target;
+              P.disk[slot].g[0] = kepler_g<METRIC>(mc, (double)target, (double)pt, (double)pph);
+              n_rec = 1;
+            } else {
+              status = 0;
+              resume = true;
+            }
+          }
+          if (!resume) {
+            t = nt; r = target; th = nth; ph = nph; pr = npr; pth = npth; lam = lam + w * sl;
+            finished = true;
+          } else {
+            GP_RESUME_PARKED()
+          }
         } else {  // MODE_LAND_TH
           ++n_land;
+          if (RING) {
+            const S rin = (S)P.disk_r_in, rout = (S)P.disk_r_out;
+            if (nr >= rin && nr <= rout) {          // theta-face hit: the record is the landed state
+              P.disk[slot].r_cross[0] = (double)nr;
+              P.disk[slot].g[0] = kepler_g<METRIC>(mc, (double)nr, (double)pt, (double)pph);
+              n_rec = 1;
+              status = GP_RAY_HIT_RING;
+              t = nt; r = nr; th = target; ph = nph; pr = npr; pth = npth; lam = lam + w * sl;
+              finished = true;
+            } else if (!(r >= rin && r <= rout)) {  // try the radial face on y_n's side
+              status = GP_RAY_HIT_RING;
+              target = (r < rin) ? rin : rout;
+              mode = MODE_LAND_R;
+            } else {
+              GP_RESUME_PARKED()
+            }
+          }
           if (DISK) {
             const double rc = (double)nr;
             if (rc >= P.disk_r_in && rc <= P.disk_r_out) {
@@ -192,11 +267,9 @@ __global__ void __launch_bounds__(kBlock, (sizeof(T) == 8 && METRIC == METRIC_MN
               P.disk[slot].g[n_rec] = kepler_g<METRIC>(mc, rc, (double)pt, (double)pph);
               ++n_rec;
             }
-            const S *pk = park + tid;
-            r = pk[0 * kBlock]; th = pk[1 * kBlock]; pr = pk[2 * kBlock]; pth = pk[3 * kBlock];
-            t = pk[4 * kBlock]; ph = pk[5 * kBlock]; lam = pk[6 * kBlock];
+            GP_RESUME_PARKED()
           }
-          mode = MODE_NORMAL;
+          if (OBJ == 0) mode = MODE_NORMAL;
         }
       }
 
@@ -204,10 +277,11 @@ __global__ void __launch_bounds__(kBlock, (sizeof(T) == 8 && METRIC == METRIC_MN
         const unsigned n_rhs = 4u * n_acc + 3u * n_land;
         Monitors mod = {(double)mo.h_max, (double)mo.q_drift, 0.0, 0.0, (double)mo.sin_min, (double)mo.err_margin};
         // the exit surface is exact in the record whatever the arithmetic type
+        // (a ring hit on a radial face has r = that face, exact in S already)
         const double r_rec = (status == GP_RAY_ESCAPED) ? P.r_esc : (status == GP_RAY_CAPTURED ? P.r_cap : (double)r);
         store_record(P.rays + slot, (double)t, r_rec, (double)th, (double)ph, (double)pr, (double)pth, (double)lam,
                      (double)pt, (double)pph, mod, status, n_acc, 0u, n_cross, n_rec, n_rhs);
-        if (DISK) {
+        if (OBJ != 0) {
           const double qnan = __longlong_as_double(0x7ff8000000000000LL);
           for (unsigned i = n_rec; i < 3u; ++i) {
             P.disk[slot].r_cross[i] = qnan;

@@ -109,8 +109,6 @@ BAD = [
     ("4 crossings", lambda m, c, g: setattr(g, "max_crossings", 4), None, api.GP_E_BAD_PARAM),
     ("ring with the thin disk", lambda m, c, g: (setattr(g, "ring_half_angle", 0.05), setattr(g, "max_crossings", 1)),
      None, api.GP_E_UNSUPPORTED),
-    ("ring with a fixed-step scheme", lambda m, c, g: (setattr(g, "ring_half_angle", 0.05), setattr(g, "scheme", 1),
-                                                       setattr(g, "h_rel", 0.02)), None, api.GP_E_UNSUPPORTED),
     ("negative ring angle", lambda m, c, g: setattr(g, "ring_half_angle", -1.0), None, api.GP_E_BAD_PARAM),
     ("FP32 with the adaptive scheme", lambda m, c, g: setattr(g, "precision", 1), None, api.GP_E_UNSUPPORTED),
     ("precision 3", lambda m, c, g: setattr(g, "precision", 3), None, api.GP_E_UNSUPPORTED),

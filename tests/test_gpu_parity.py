@@ -795,6 +795,52 @@ def test_solid_ring_hits_match_the_oracle(gp, O, label, metric, r_in, incl):
           "status mismatches (excused)", int(mism.sum()))
 
 
+@pytest.mark.parametrize("precision", [0, 2])
+def test_solid_ring_with_the_fixed_step_scheme(gp, O, precision):
+    """The ring in trace_rk4 (RK4 h = 0.02 r, the paper's own kind of integrator): FP64 against the oracle under
+    the same rules as the adaptive kernel; the mixed-precision variant (FP32 equations, FP64 state) to 1e-4 on
+    the hit state, same face."""
+    metric = dict(id=W.KERR, M=1.0, a=0.98, q=0.0)
+    w = _ring("C3", metric, 0.05, 0.0, 14.0, width=256, height=256, alpha_min=-18.0, alpha_max=18.0, beta_min=-18.0,
+              beta_max=18.0)
+    w["cfg"].update(scheme=1, h_rel=0.02, max_steps=20000)
+    b, c, s = W.ray_selection(w, 3, None, 5)
+    orc, _ = O.trace(w, b, c, s)
+    probe, _ = O.trace(w, b, c, s, rounding_probe=True)
+    w["cfg"]["precision"] = precision
+    rays, disk, counters = gp.api.trace_workload(w, b, c, s)
+    assert counters[1] == c
+    from parity_rules import SENSITIVE_AT, flags, rel_err as re_
+    fl = flags(orc, probe)
+    gs, os_ = rays["status"].astype(np.int64), orc["status"]
+    for f in ("r", "p_r", "p_theta"):
+        fl["sensitive"] = fl["sensitive"] | ((os_ == 5) & (probe["status"] == 5) & (re_(probe[f], orc[f]) > SENSITIVE_AT))
+    tol = TOL if precision == 0 else 1e-4
+    if precision == 2:
+        fl["sensitive"] = fl["sensitive"] | (fl["spread"] > 1e-13)
+    mism = gs != os_
+    assert not (mism & ~(fl["marginal"] | fl["sensitive"])).any(), int((mism & ~fl["sensitive"]).sum())
+    hit = (gs == 5) & (os_ == 5)
+    smooth = hit & ~(fl["marginal"] | fl["near_axis"] | fl["sensitive"])
+    assert hit.sum() > 1500 and smooth.sum() >= 0.95 * hit.sum()
+    # (the stated tolerance of the mixed variant is on theta, phi, lambda, t; the hit radius is held to it too)
+    for f in FIELDS + (("r", "p_r", "p_theta") if precision == 0 else ("r",)):
+        assert re_(rays[f], orc[f])[smooth].max() <= tol, f
+    on_th = np.abs(np.abs(orc["theta"] - math.pi / 2) - 0.05) <= 1e-15
+    assert np.array_equal(rays["theta"][smooth & on_th], orc["theta"][smooth & on_th])     # the face, exactly
+    assert np.array_equal(rays["r"][smooth & ~on_th], orc["r"][smooth & ~on_th])
+    assert (smooth & ~on_th).sum() >= 5
+    assert re_(disk["g"][smooth, 0], orc["disk_g"][smooth, 0]).max() <= tol
+    assert np.array_equal(disk["r_cross"][smooth, 0], rays["r"][smooth])
+    if precision == 0:
+        for f in ("n_accepted", "n_equator_crossings", "n_rhs"):
+            d_ = rays[f][smooth].astype(np.int64) != orc[f][smooth]
+            assert d_.sum() <= max(1.0, 1e-4 * d_.size), (f, int(d_.sum()))
+        miss = (os_ != 5) & (gs != 5)
+        check_parity(w, rays[miss], orc[miss], probe[miss], "RK4 ring (rays that miss)", max_flagged_fraction=0.05)
+    print("RK4 ring precision", precision, "hits", int(hit.sum()), "smooth", int(smooth.sum()))
+
+
 def test_solid_ring_thin_limit_on_the_gpu(gp):
     """A property that needs no oracle: as the half angle -> 0 the ring hit becomes the first thin-disk
     crossing inside [r_in, r_out] recorded by the disk variant of the same kernel."""
@@ -816,7 +862,8 @@ def test_solid_ring_thin_limit_on_the_gpu(gp):
 
 def test_ring_validation_on_the_gpu(gp):
     w = _ring("C3", dict(id=W.KERR, M=1.0, a=0.9, q=0.0), 0.05, 0.0, 14.0)
-    for bad, code in ((dict(max_crossings=2), gp.api.GP_E_UNSUPPORTED), (dict(scheme=1, h_rel=0.02), gp.api.GP_E_UNSUPPORTED),
+    for bad, code in ((dict(max_crossings=2), gp.api.GP_E_UNSUPPORTED),
+                      (dict(precision=2, rtol=1e-6, atol=1e-6), gp.api.GP_E_UNSUPPORTED),      # mixed adaptive: no objects
                       (dict(ring_half_angle=-0.1), gp.api.GP_E_BAD_PARAM), (dict(ring_half_angle=2.0), gp.api.GP_E_BAD_PARAM)):
         wb = copy.deepcopy(w)
         wb["cfg"].update(bad)

@@ -143,6 +143,26 @@ def test_ring_validation():
     w["cfg"]["max_crossings"] = 3
     with pytest.raises(ValueError):
         O.trace(w, 0, 4, 1)
-    w = ring_workload("C5a")      # fixed-step scheme: the located hit is built for the adaptive one
+    w = ring_workload("C3", r_in=9.0, r_out=8.0)      # empty radial range
     with pytest.raises(ValueError):
         O.trace(w, 0, 4, 1)
+
+
+def test_ring_with_the_fixed_step_scheme_converges_to_the_adaptive_hits():
+    """The ring with RK4 h = 0.01 r: same landing rule with the scheme's own step formula (R14).  The hit
+    points agree with the adaptive scheme's to the fixed step's own accuracy, and every hit is on a face."""
+    w2 = ring_workload("C3", d=0.05, r_in=6.0, r_out=14.0)
+    w1 = copy.deepcopy(w2)
+    w1["cfg"].update(scheme=1, h_rel=0.01, max_steps=200000)
+    sel = W.ray_selection(w2, 7, None, 877)
+    a, _ = O.trace(w2, *sel)
+    b, _ = O.trace(w1, *sel)
+    both = (a["status"] == 5) & (b["status"] == 5)
+    assert both.sum() > 60 and (a["status"] == b["status"]).mean() > 0.99
+    same_face = np.isclose(np.abs(a["theta"] - math.pi / 2), 0.05, atol=1e-15) == np.isclose(np.abs(b["theta"] - math.pi / 2), 0.05, atol=1e-15)
+    ok = both & same_face
+    assert ok.sum() >= 0.97 * both.sum()
+    assert np.abs(a["r"] - b["r"])[ok].max() <= 1e-5 and np.abs(a["phi"] - b["phi"])[ok].max() <= 1e-5
+    assert np.abs(a["disk_g"][ok, 0] / b["disk_g"][ok, 0] - 1.0).max() <= 1e-5
+    on_face = np.isclose(np.abs(b["theta"][both] - math.pi / 2), 0.05, atol=1e-15) | (b["r"][both] == 6.0) | (b["r"][both] == 14.0)
+    assert on_face.all()
