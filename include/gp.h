@@ -92,8 +92,8 @@ typedef struct gp_integrator_cfg {
                         2 = mixed: Hamilton's equations in FP32 at the state
                             rounded to FP32, state / Runge-Kutta sums / error norm / controller in FP64;
                             all schemes; with scheme 2 rtol and atol must be >= 1e-7 (the error estimate
-                            carries the 6e-8 noise of an FP32 evaluation; below -> GP_E_BAD_PARAM) and no
-                            disk / ring (-> GP_E_UNSUPPORTED).  Stated tolerance of 1 and 2: DESIGN.md 7.6.
+                            carries the 6e-8 noise of an FP32 evaluation; below -> GP_E_BAD_PARAM).
+                            Stated tolerance of 1 and 2: DESIGN.md 7.6.
                         The ray is born and the record written in FP64 in every case; other values ->
                         GP_E_UNSUPPORTED                                                             */
   double h, h_rel, rtol, atol, h_cap_rel;
@@ -123,8 +123,7 @@ typedef struct gp_integrator_cfg {
    * else on the radial face on y_n's side (a hit if the landed theta is in the slab); otherwise the ray
    * goes on from y_{n+1} (reading R39).  The record holds the state at the hit; disk record
    * slot 0 holds the hit radius and g of the circular equatorial emitter at that radius (eq 56-57), the
-   * other slots NaN.  Every scheme and precision except the mixed adaptive kernel (the landing steps use the
-   * scheme's own formula).  Requires max_crossings = 0 and a disk buffer; Manko-Novikov needs an explicit
+   * other slots NaN.  Every scheme and precision (the landing steps use the scheme's own formula).  Requires max_crossings = 0 and a disk buffer; Manko-Novikov needs an explicit
    * disk_r_in.  0 = no ring.  Values < 0 or >= 1.5 -> GP_E_BAD_PARAM; with max_crossings > 0 ->
    * GP_E_UNSUPPORTED.                                                              */
   double ring_half_angle;

@@ -156,8 +156,6 @@ int make_params(int metric_id, const gp_metric_params *m, const gp_camera *cam, 
   // precision 2 (FP32 equations, FP64 state): every scheme; with the adaptive scheme the tolerances must
   // stay above the noise of an FP32 evaluation of the equations in the error estimate (gp.h)
   if (cfg->precision == 2 && cfg->scheme == 2 && (!(cfg->rtol >= 1e-7) || !(cfg->atol >= 1e-7))) return GP_E_BAD_PARAM;
-  if (cfg->precision == 2 && cfg->scheme == 2 && (cfg->max_crossings > 0 || cfg->ring_half_angle > 0.0))
-    return GP_E_UNSUPPORTED;   // the mixed adaptive kernel is built without objects
   // the single-precision variant exists for the fixed-step schemes only: a 1e-10 tolerance has no
   // meaning in FP32 arithmetic
   if (cfg->precision == 1 && cfg->scheme == 2) return GP_E_UNSUPPORTED;
@@ -294,8 +292,7 @@ int launch_one(const TraceParams &P, cudaStream_t stream) {
   }
   if (dp54) {
     if (prec == 2) {
-      if (OBJ != 0) return GP_E_UNSUPPORTED;
-      GP_GO((trace_dp54<METRIC, 0, float>))
+      GP_GO((trace_dp54<METRIC, OBJ, float>))
     } else {
       GP_GO((trace_dp54<METRIC, OBJ>))
     }

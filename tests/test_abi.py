@@ -113,13 +113,12 @@ BAD = [
     ("FP32 with the adaptive scheme", lambda m, c, g: setattr(g, "precision", 1), None, api.GP_E_UNSUPPORTED),
     ("precision 3", lambda m, c, g: setattr(g, "precision", 3), None, api.GP_E_UNSUPPORTED),
     ("mixed precision below its tolerance floor", lambda m, c, g: setattr(g, "precision", 2), None, api.GP_E_BAD_PARAM),
-    ("mixed adaptive with a disk", lambda m, c, g: (setattr(g, "precision", 2), setattr(g, "rtol", 1e-6), setattr(g, "atol", 1e-6),
-                                                   setattr(g, "max_crossings", 1)), None, api.GP_E_UNSUPPORTED),
     ("projection 2", lambda m, c, g: setattr(c, "projection", 2), None, api.GP_E_UNSUPPORTED),
     ("screen camera reaching past r_escape", lambda m, c, g: (setattr(c, "projection", 1), setattr(c, "alpha_max", 900.0)),
      None, api.GP_E_BAD_PARAM),
     ("negative focal factor", lambda m, c, g: (setattr(c, "projection", 1), setattr(c, "focal_2f_over_d", -1.0)),
      None, api.GP_E_BAD_PARAM),
+    ("segment_steps below -1", lambda m, c, g: setattr(g, "segment_steps", -2), None, api.GP_E_BAD_PARAM),
 ]
 
 

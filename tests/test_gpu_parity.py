@@ -795,15 +795,18 @@ def test_solid_ring_hits_match_the_oracle(gp, O, label, metric, r_in, incl):
           "status mismatches (excused)", int(mism.sum()))
 
 
-@pytest.mark.parametrize("precision", [0, 2])
-def test_solid_ring_with_the_fixed_step_scheme(gp, O, precision):
+@pytest.mark.parametrize("precision,scheme", [(0, 1), (2, 1), (2, 2)])
+def test_solid_ring_with_the_fixed_step_scheme(gp, O, precision, scheme):
     """The ring in trace_rk4 (RK4 h = 0.02 r, the paper's own kind of integrator): FP64 against the oracle under
     the same rules as the adaptive kernel; the mixed-precision variant (FP32 equations, FP64 state) to 1e-4 on
     the hit state, same face."""
     metric = dict(id=W.KERR, M=1.0, a=0.98, q=0.0)
     w = _ring("C3", metric, 0.05, 0.0, 14.0, width=256, height=256, alpha_min=-18.0, alpha_max=18.0, beta_min=-18.0,
               beta_max=18.0)
-    w["cfg"].update(scheme=1, h_rel=0.02, max_steps=20000)
+    if scheme == 1:
+        w["cfg"].update(scheme=1, h_rel=0.02, max_steps=20000)
+    else:                                       # the mixed adaptive kernel with the ring, at its tolerance floor
+        w["cfg"].update(rtol=1e-7, atol=1e-7)
     b, c, s = W.ray_selection(w, 3, None, 5)
     orc, _ = O.trace(w, b, c, s)
     probe, _ = O.trace(w, b, c, s, rounding_probe=True)
@@ -863,7 +866,6 @@ def test_solid_ring_thin_limit_on_the_gpu(gp):
 def test_ring_validation_on_the_gpu(gp):
     w = _ring("C3", dict(id=W.KERR, M=1.0, a=0.9, q=0.0), 0.05, 0.0, 14.0)
     for bad, code in ((dict(max_crossings=2), gp.api.GP_E_UNSUPPORTED),
-                      (dict(precision=2, rtol=1e-6, atol=1e-6), gp.api.GP_E_UNSUPPORTED),      # mixed adaptive: no objects
                       (dict(ring_half_angle=-0.1), gp.api.GP_E_BAD_PARAM), (dict(ring_half_angle=2.0), gp.api.GP_E_BAD_PARAM)):
         wb = copy.deepcopy(w)
         wb["cfg"].update(bad)
