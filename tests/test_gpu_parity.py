@@ -940,3 +940,17 @@ def test_segmented_tracing_changes_nothing_but_the_balance(gp):
     w["cfg"]["segment_steps"] = -2
     with pytest.raises(gp.api.GpError):
         gp.api.trace_workload(w, 0, 10, 1)
+
+
+@pytest.mark.parametrize("scheme", [2, 1])
+def test_generic_parameters_mass_and_retrograde_spin(gp, O, scheme):
+    """Nothing in the kernels may assume M = 1, a > 0 or an observer above the equator: Kerr with M = 1.3,
+    a = -0.9 (counter-rotating), observer at 100 degrees and phi_obs = 2, both integrators, ordinary rules."""
+    w = W.workload("C2", width=300, height=300, theta_obs=math.radians(100.0), phi_obs=2.0,
+                   alpha_min=-16.0, alpha_max=16.0, beta_min=-16.0, beta_max=16.0)
+    w["metric"] = dict(id=W.KERR, M=1.3, a=-0.9, q=0.0)
+    if scheme == 1:
+        w["cfg"].update(scheme=1, h_rel=0.02, max_steps=200000)
+    rays, _, _, orc, probe = run_both(gp, O, w, 2, None, 29)
+    res, smooth = check_parity(w, rays, orc, probe, f"M=1.3 a=-0.9 scheme {scheme}", max_flagged_fraction=0.02)
+    assert (orc["status"] == 1).sum() > 100 and (orc["status"] == 0).sum() > 2000 and res["status_mismatch"] == 0
