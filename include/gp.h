@@ -25,7 +25,9 @@
 extern "C" {
 #endif
 
-#define GP_VERSION 102 /* major*10000 + minor*100 + patch */
+#define GP_VERSION 103 /* major*10000 + minor*100 + patch */
+/* Capacity of the library's static scratch, in rays (one 1024 x 1024 image): gp_trace_static only. */
+#define GP_STATIC_MAX_RAYS 1048576
 
 /* ---- spacetimes (section 2.2) ------------------------------------------- */
 enum {
@@ -197,7 +199,8 @@ enum {
   GP_E_NULL = -3,
   GP_E_SIZE = -4,
   GP_E_UNSUPPORTED = -5,
-  GP_E_CUDA = -6
+  GP_E_CUDA = -6,
+  GP_E_STATIC_LIMIT = -7 /* gp_trace_static: ray_count > GP_STATIC_MAX_RAYS */
 };
 
 /* ---- entry points -------------------------------------------------------------------
@@ -225,6 +228,30 @@ int gp_trace(int metric_id, const gp_metric_params *metric, const gp_camera *cam
  * on different streams, host threads and devices are independent.                               */
 int gp_trace_host(int metric_id, const gp_metric_params *metric, const gp_camera *camera,
                   const gp_integrator_cfg *cfg, const gp_out_buffers *out, void *cuda_stream);
+
+/* gp_trace for callers that may not allocate (code under CUDA graph capture, serving loops, harnesses
+ * that forbid cudaMalloc).  Same kernels, same records, same validation and error behaviour as gp_trace;
+ * the difference is where the scratch lives.  gp_trace takes its work counter from the caller's
+ * `counters` block and, with cfg.segment_steps != 0, two slot lists from a stream-ordered pool; here
+ * both sit in ONE file-scope `static __device__` array of the library (128 bytes of counters and list
+ * counts + 2 x GP_STATIC_MAX_RAYS x 8 bytes of lists = 16 MiB + 128 bytes, which every GPU that loads
+ * the library holds until the process exits).  The call makes no cudaMalloc / cudaFree / pool
+ * allocation: it enqueues memsets of the 128 bytes that must start at zero (the lists need no clearing,
+ * only the first `count` entries of a list are ever read), the launches, and one 64-byte
+ * device-to-device copy if out->counters is given.
+ *   out->rays, out->disk  DEVICE, as for gp_trace (sizes and alignment checked the same way).
+ *   out->counters         DEVICE, >= 64 bytes, 8-byte aligned, or NULL: receives a copy of the totals
+ *                         ([0]..[7] as documented at gp_out_buffers) after the last launch.
+ *   camera->ray_count     <= GP_STATIC_MAX_RAYS, else GP_E_STATIC_LIMIT and nothing is enqueued (tile a
+ *                         larger image with ray_begin / ray_count, one call per tile, or use gp_trace).
+ * NOT re-entrant per device: every call on a device shares the array, which keeps the previous call's
+ * contents until this call's memsets run.  Calls on the SAME stream are ordered and correct; calls that
+ * overlap on the GPU (different streams without an event between them, or several host threads on one
+ * device) race on the work counter and produce garbage.  Different devices hold different copies and
+ * are independent; the array's device address is looked up once per device, under a mutex, with that
+ * device current.                                                                                  */
+int gp_trace_static(int metric_id, const gp_metric_params *metric, const gp_camera *camera,
+                    const gp_integrator_cfg *cfg, const gp_out_buffers *out, void *cuda_stream);
 
 /* Steps a2+a3 alone (pixel -> (alpha,beta) -> initial state), for inspection and parity.
  * states8: DEVICE, ray_count*8 doubles (t, r, theta, phi, p_t, p_r, p_theta, p_phi).
@@ -332,6 +359,7 @@ int gp_metric_radii(int metric_id, const gp_metric_params *metric, double *r_hor
 size_t gp_ray_record_size(void);  /* 128 */
 size_t gp_disk_record_size(void); /* 48  */
 size_t gp_counters_size(void);    /* 64  */
+int64_t gp_static_max_rays(void); /* GP_STATIC_MAX_RAYS */
 int gp_version(void);
 /* Static string for a GP_E_* code; for GP_E_CUDA the last CUDA error text seen by this
  * thread is appended.                                                                   */

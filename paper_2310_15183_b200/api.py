@@ -15,8 +15,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 
 GP_SCHWARZSCHILD, GP_KERR, GP_MANKO_NOVIKOV = 0, 1, 2
 GP_RAY_ESCAPED, GP_RAY_CAPTURED, GP_RAY_MAXSTEPS, GP_RAY_NONFINITE, GP_RAY_STEP_UNDERFLOW, GP_RAY_HIT_RING = range(6)
-GP_OK, GP_E_BAD_METRIC, GP_E_BAD_PARAM, GP_E_NULL, GP_E_SIZE, GP_E_UNSUPPORTED, GP_E_CUDA = (
-    0, -1, -2, -3, -4, -5, -6)
+GP_OK, GP_E_BAD_METRIC, GP_E_BAD_PARAM, GP_E_NULL, GP_E_SIZE, GP_E_UNSUPPORTED, GP_E_CUDA, GP_E_STATIC_LIMIT = (
+    0, -1, -2, -3, -4, -5, -6, -7)
 
 _f64, _i32, _i64, _u64 = C.c_double, C.c_int32, C.c_int64, C.c_uint64
 
@@ -73,7 +73,7 @@ RAY_DTYPE = np.dtype([
 DISK_DTYPE = np.dtype([("r_cross", "<f8", (3,)), ("g", "<f8", (3,))])
 assert RAY_DTYPE.itemsize == 128 and DISK_DTYPE.itemsize == 48
 
-EXPORTS = ("gp_integrate_orbits", "gp_shade", "gp_trace", "gp_trace_host", "gp_init_conditions", "gp_eval_metric", "gp_eval_rhs",
+EXPORTS = ("gp_integrate_orbits", "gp_shade", "gp_trace", "gp_trace_host", "gp_trace_static", "gp_static_max_rays", "gp_init_conditions", "gp_eval_metric", "gp_eval_rhs",
            "gp_probe_fp64_fma", "gp_metric_radii", "gp_ray_record_size", "gp_disk_record_size",
            "gp_counters_size", "gp_version", "gp_strerror")
 
@@ -88,6 +88,9 @@ def _load():
     sig5 = [C.c_int, P(gp_metric_params), P(gp_camera), P(gp_integrator_cfg), P(gp_out_buffers), vp]
     L.gp_trace.argtypes = sig5
     L.gp_trace_host.argtypes = sig5
+    L.gp_trace_static.argtypes = sig5
+    L.gp_static_max_rays.restype = _i64
+    L.gp_static_max_rays.argtypes = []
     L.gp_init_conditions.argtypes = [C.c_int, P(gp_metric_params), P(gp_camera), vp, sz, vp, sz, vp]
     L.gp_eval_metric.argtypes = [C.c_int, P(gp_metric_params), vp, _i64, vp, sz, vp]
     L.gp_eval_rhs.argtypes = [C.c_int, P(gp_metric_params), vp, _i64, vp, sz, vp]
@@ -98,7 +101,7 @@ def _load():
     L.gp_integrate_orbits.restype = C.c_int
     L.gp_shade.argtypes = [P(gp_shade_cfg), vp, sz, vp, sz, vp, sz, vp]
     L.gp_shade.restype = C.c_int
-    for n in ("gp_trace", "gp_trace_host", "gp_init_conditions", "gp_eval_metric", "gp_eval_rhs",
+    for n in ("gp_trace", "gp_trace_host", "gp_trace_static", "gp_init_conditions", "gp_eval_metric", "gp_eval_rhs",
               "gp_probe_fp64_fma", "gp_metric_radii", "gp_version"):
         getattr(L, n).restype = C.c_int
     for n in ("gp_ray_record_size", "gp_disk_record_size", "gp_counters_size"):
@@ -191,6 +194,22 @@ def gp_trace_host(metric_id, metric, camera, cfg, rays, disk=None, counters=None
         out.counters, out.counters_bytes = C.c_void_p(counters.ctypes.data), counters.nbytes
     _check(lib.gp_trace_host(int(metric_id), C.byref(metric), C.byref(camera), C.byref(cfg),
                              C.byref(out), _stream_ptr(stream)), "gp_trace_host")
+
+
+def gp_trace_static(metric_id, metric, camera, cfg, rays, disk=None, counters=None, stream=None):
+    """gp_trace without any allocation: the scratch is the library's static device array (gp.h).
+    rays/disk: CUDA uint8 tensors owned by the caller; counters: CUDA tensor of >= 64 bytes or None.
+    At most gp_static_max_rays() rays per call; calls that overlap on one GPU race."""
+    out = gp_out_buffers()
+    out.rays, out.rays_bytes = _dev(rays)
+    out.disk, out.disk_bytes = _dev(disk)
+    out.counters, out.counters_bytes = _dev(counters)
+    _check(lib.gp_trace_static(int(metric_id), C.byref(metric), C.byref(camera), C.byref(cfg),
+                               C.byref(out), _stream_ptr(stream)), "gp_trace_static")
+
+
+def gp_static_max_rays():
+    return int(lib.gp_static_max_rays())
 
 
 def gp_init_conditions(metric_id, metric, camera, states8, alpha_beta2=None, stream=None):

@@ -373,6 +373,34 @@ __global__ void __launch_bounds__(256) k_probe_fma(long long iters, double seed,
   if (s == 123.456) *sink = s;  // keeps the chains alive without a store in practice
 }
 
+// ---- static scratch for gp_trace_static ----------------------------------------------------------
+// Everything the trace kernels need besides the caller's inputs and outputs, in one file-scope array, so
+// that gp_trace_static never allocates (gp.h): words 0-7 the counters block (word 0 = the atomic work
+// counter), words 8-15 the two list counts of segmented tracing, then the two slot lists of
+// GP_STATIC_MAX_RAYS entries each.  16 MiB + 128 bytes of .bss on every device that loads the library.
+// In HOST code the name below is the host-side shadow of the symbol, not a device address: a kernel
+// handed it would fault (or, where the GPU can reach host memory, scribble over the wrong memory).
+// static_scratch() asks the runtime for the address, once per device, with that device current.
+constexpr size_t kStaticHeadWords = 16;
+static __device__ __align__(256) unsigned long long g_static_scratch[kStaticHeadWords + 2 * (size_t)GP_STATIC_MAX_RAYS];
+
+int static_scratch(unsigned long long **out) {
+  static unsigned long long *addr[kMaxDevices] = {};
+  static std::mutex mu;
+  int dev = 0;
+  GP_CUDA(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kMaxDevices) return GP_E_UNSUPPORTED;
+  std::lock_guard<std::mutex> lock(mu);
+  if (!addr[dev]) {
+    void *p = nullptr;
+    GP_CUDA(cudaGetSymbolAddress(&p, g_static_scratch));
+    if (!p || ((uintptr_t)p & 255u) != 0) return GP_E_UNSUPPORTED;
+    addr[dev] = (unsigned long long *)p;
+  }
+  *out = addr[dev];
+  return GP_OK;
+}
+
 }  // namespace
 
 // ---- exported entry points -----------------------------------------------------------------------
@@ -509,6 +537,72 @@ int gp_trace_host(int metric_id, const gp_metric_params *metric, const gp_camera
   if (e != cudaSuccess) return cuda_fail(e);
   if (e2 != cudaSuccess) return cuda_fail(e2);
   if (e3 != cudaSuccess) return cuda_fail(e3);
+  return GP_OK;
+}
+
+int gp_trace_static(int metric_id, const gp_metric_params *metric, const gp_camera *camera,
+                    const gp_integrator_cfg *cfg, const gp_out_buffers *out, void *cuda_stream) {
+  if (!out) return GP_E_NULL;
+  TraceParams P;
+  int rc = make_params(metric_id, metric, camera, cfg, &P);
+  if (rc) return rc;
+  const size_t n = (size_t)camera->ray_count;
+  if (n > (size_t)GP_STATIC_MAX_RAYS) return GP_E_STATIC_LIMIT;
+  if (out->counters) {
+    if (out->counters_bytes < 64) return GP_E_SIZE;
+    if (((uintptr_t)out->counters & 7u) != 0) return GP_E_BAD_PARAM;
+  }
+  if (n > 0) {
+    if (!out->rays) return GP_E_NULL;
+    if (out->rays_bytes < n * sizeof(gp_ray_record)) return GP_E_SIZE;
+    if (((uintptr_t)out->rays & 31u) != 0) return GP_E_BAD_PARAM;
+    if (cfg->max_crossings > 0 || cfg->ring_half_angle > 0.0) {
+      if (!out->disk) return GP_E_NULL;
+      if (out->disk_bytes < n * sizeof(gp_disk_record)) return GP_E_SIZE;
+      if (((uintptr_t)out->disk & 7u) != 0) return GP_E_BAD_PARAM;
+    }
+  }
+  // segment length: the rule of gp_trace
+  long long K = 0;
+  if (metric_id == GP_MANKO_NOVIKOV && cfg->scheme == 2 && cfg->segment_steps != 0) {
+    K = cfg->segment_steps > 0 ? cfg->segment_steps : (cfg->max_steps / 48 > 4096 ? cfg->max_steps / 48 : 4096);
+    if (K >= cfg->max_steps) K = 0;
+  }
+  if (K > 0 && (cfg->max_steps + K - 1) / K > 4096) return GP_E_BAD_PARAM;
+  unsigned long long *S = nullptr;   // DEVICE address of g_static_scratch on the current device
+  rc = static_scratch(&S);
+  if (rc) return rc;
+  cudaStream_t stream = (cudaStream_t)cuda_stream;
+  P.rays = (gp_ray_record *)out->rays;
+  P.disk = (gp_disk_record *)out->disk;
+  P.counters = S;
+  // the array keeps the last call's totals and list counts: clear the 128 bytes that must start at zero
+  GP_CUDA(cudaMemsetAsync(S, 0, kStaticHeadWords * sizeof(unsigned long long), stream));
+  cudaError_t e = cudaSuccess;
+  if (n > 0 && K == 0) {
+    rc = launch_trace(metric_id, P, stream);
+  } else if (n > 0) {
+    unsigned long long *counts = S + 8;
+    long long *lists[2] = {(long long *)(S + kStaticHeadWords),
+                           (long long *)(S + kStaticHeadWords + (size_t)GP_STATIC_MAX_RAYS)};
+    const long long rounds = (cfg->max_steps + K - 1) / K;
+    P.seg_steps = K;
+    for (long long rd = 0; rd < rounds && e == cudaSuccess && rc == GP_OK; ++rd) {
+      P.round = (int)rd;
+      P.list_in = lists[rd & 1];
+      P.list_in_count = counts + (rd & 1);
+      P.list_out = lists[(rd + 1) & 1];
+      P.list_out_count = counts + ((rd + 1) & 1);
+      if (rd > 0) {
+        e = cudaMemsetAsync(P.list_out_count, 0, sizeof(unsigned long long), stream);
+        if (e == cudaSuccess) e = cudaMemsetAsync(S, 0, sizeof(unsigned long long), stream);   // work counter
+      }
+      if (e == cudaSuccess) rc = launch_trace(metric_id, P, stream);
+    }
+  }
+  if (rc != GP_OK) return rc;
+  if (e != cudaSuccess) return cuda_fail(e);
+  if (out->counters) GP_CUDA(cudaMemcpyAsync(out->counters, S, 64, cudaMemcpyDeviceToDevice, stream));
   return GP_OK;
 }
 
@@ -684,6 +778,7 @@ int gp_metric_radii(int metric_id, const gp_metric_params *metric, double *r_hor
 size_t gp_ray_record_size(void) { return sizeof(gp_ray_record); }
 size_t gp_disk_record_size(void) { return sizeof(gp_disk_record); }
 size_t gp_counters_size(void) { return 64; }
+int64_t gp_static_max_rays(void) { return GP_STATIC_MAX_RAYS; }
 int gp_version(void) { return GP_VERSION; }
 
 const char *gp_strerror(int code) {
@@ -695,6 +790,9 @@ const char *gp_strerror(int code) {
     case GP_E_NULL: return "null pointer";
     case GP_E_SIZE: return "buffer too small";
     case GP_E_UNSUPPORTED: return "variant not built";
+    case GP_E_STATIC_LIMIT:
+      return "gp_trace_static: ray_count exceeds GP_STATIC_MAX_RAYS (1048576), the capacity of the library's "
+             "static scratch; tile the image with ray_begin / ray_count or call gp_trace";
     case GP_E_CUDA:
       snprintf(buf, sizeof(buf), "CUDA error: %s", g_cuda_msg);
       return buf;

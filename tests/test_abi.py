@@ -50,7 +50,7 @@ def test_record_layouts():
     assert gp.gp_ray_record_size() == 128 == api.RAY_DTYPE.itemsize
     assert gp.gp_disk_record_size() == 48 == api.DISK_DTYPE.itemsize
     assert gp.gp_counters_size() == 64
-    assert gp.gp_version() == 102
+    assert gp.gp_version() == 103
     f = api.RAY_DTYPE.fields
     assert f["lambda"][1] == 32 and f["status"][1] == 40 and f["p_r"][1] == 48 and f["p_t"][1] == 64
     assert f["sin_theta_min"][1] == 96 and f["err_margin"][1] == 104 and f["n_rhs"][1] == 124
@@ -60,8 +60,9 @@ def test_record_layouts():
 
 def test_strerror():
     assert gp.gp_strerror(0) == "ok"
-    for code in range(-6, 0):
+    for code in range(-7, 0):
         assert gp.gp_strerror(code) not in ("ok", "unknown error code")
+    assert "GP_STATIC_MAX_RAYS (1048576)" in gp.gp_strerror(api.GP_E_STATIC_LIMIT)
     assert gp.gp_strerror(-99) == "unknown error code"
 
 
@@ -122,7 +123,7 @@ BAD = [
 ]
 
 
-@pytest.mark.parametrize("entry", ["gp_trace", "gp_trace_host"])
+@pytest.mark.parametrize("entry", ["gp_trace", "gp_trace_host", "gp_trace_static"])
 @pytest.mark.parametrize("what,mutate,metric_id,code", BAD, ids=[b[0] for b in BAD])
 def test_validation_is_synchronous(entry, what, mutate, metric_id, code):
     assert _call(W.workload("C2"), mutate, metric_id, entry=entry) == code
@@ -148,6 +149,47 @@ def test_buffer_checks():
     misaligned = api.gp_out_buffers(C.c_void_p(0x1008), 64 * 128, C.c_void_p(0x2000), 64 * 48, C.c_void_p(0x3000), 64)
     assert _call(w, out=misaligned) == api.GP_E_BAD_PARAM
     assert api.lib.gp_trace(1, None, None, None, None, None) == api.GP_E_NULL
+
+
+def test_static_entry_point_limit_and_buffer_checks():
+    """gp_trace_static (gp.h): more than GP_STATIC_MAX_RAYS rays are refused with a code of their own before
+    any CUDA call is made; the caller's buffers are checked like gp_trace's, except that counters may be NULL."""
+    assert gp.gp_static_max_rays() == 1 << 20
+    hdr = open(HEADER).read()
+    assert re.search(r"#define\s+GP_STATIC_MAX_RAYS\s+1048576\b", hdr) and "GP_E_STATIC_LIMIT = -7" in hdr
+    w = W.workload("headline", width=1025, height=1024)
+    n = (1 << 20) + 1
+    big = api.gp_out_buffers(C.c_void_p(0x1000), n * 128, None, 0, None, 0)
+    assert _call(w, lambda m, c, g: setattr(c, "ray_count", n), out=big, entry="gp_trace_static") == api.GP_E_STATIC_LIMIT
+    w = W.workload("C3")
+    small = api.gp_out_buffers(C.c_void_p(0x1000), 63 * 128, C.c_void_p(0x2000), 64 * 48, None, 0)
+    assert _call(w, out=small, entry="gp_trace_static") == api.GP_E_SIZE
+    nodisk = api.gp_out_buffers(C.c_void_p(0x1000), 64 * 128, None, 0, None, 0)
+    assert _call(w, out=nodisk, entry="gp_trace_static") == api.GP_E_NULL
+    misaligned = api.gp_out_buffers(C.c_void_p(0x1008), 64 * 128, C.c_void_p(0x2000), 64 * 48, None, 0)
+    assert _call(w, out=misaligned, entry="gp_trace_static") == api.GP_E_BAD_PARAM
+    shortcount = api.gp_out_buffers(C.c_void_p(0x1000), 64 * 128, C.c_void_p(0x2000), 64 * 48, C.c_void_p(0x3000), 56)
+    assert _call(w, out=shortcount, entry="gp_trace_static") == api.GP_E_SIZE
+    oddcount = api.gp_out_buffers(C.c_void_p(0x1000), 64 * 128, C.c_void_p(0x2000), 64 * 48, C.c_void_p(0x3004), 64)
+    assert _call(w, out=oddcount, entry="gp_trace_static") == api.GP_E_BAD_PARAM
+    assert api.lib.gp_trace_static(1, None, None, None, None, None) == api.GP_E_NULL
+
+
+def test_static_entry_point_has_no_allocating_call():
+    """The body of gp_trace_static, and of the helper that looks up the static array, name no allocation
+    routine and no pool; the array is a file-scope `static __device__ __align__(256)` object whose device
+    address comes from cudaGetSymbolAddress (in host code its name is only the host-side shadow)."""
+    src = open(os.path.join(ROOT, "paper_2310_15183_b200", "csrc", "gp_api.cu")).read()
+    assert re.search(r"static __device__ __align__\(256\) unsigned long long g_static_scratch\[", src)
+    body = src[src.index("int gp_trace_static("):src.index("int gp_init_conditions(")]
+    helper = src[src.index("int static_scratch("):src.index("}  // namespace")]
+    body, helper = (re.sub(r"//[^\n]*", "", t) for t in (body, helper))      # code only
+    for text in (body, helper):
+        for word in ("cudaMalloc", "cudaFree", "scratch_pool", "cudaMemPool", "new ", "malloc(", "std::vector"):
+            assert word not in text, word
+    assert "cudaGetSymbolAddress(&p, g_static_scratch)" in helper and "GP_CUDA(cudaGetSymbolAddress" in helper
+    assert "g_static_scratch" not in body          # host code never passes the shadow to a kernel
+    assert "static_scratch(&S)" in body and "P.counters = S;" in body
 
 
 def _no_gpu():
