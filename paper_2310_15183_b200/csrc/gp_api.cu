@@ -199,6 +199,11 @@ int make_params(int metric_id, const gp_metric_params *m, const gp_camera *cam, 
   P->h_cap_rel = cfg->h_cap_rel;
   P->max_steps = cfg->max_steps;
   P->lambda_max = cfg->lambda_max > 0.0 ? cfg->lambda_max : (double)INFINITY;  // <= 0 = no affine budget
+  P->h_f = (float)cfg->h;
+  P->h_rel_f = (float)cfg->h_rel;
+  P->lambda_max_f = (float)P->lambda_max;
+  if ((double)P->lambda_max_f < P->lambda_max) P->lambda_max_f = nextafterf(P->lambda_max_f, INFINITY);
+  P->pad_f_ = 0.0f;
   P->r_cap = P->mc.r_horizon * (1.0 + cfg->eps_capture);
   P->r_esc = cfg->r_escape;
   P->ring_d = cfg->ring_half_angle;
@@ -272,7 +277,7 @@ int launch_one(const TraceParams &P, cudaStream_t stream) {
   const bool dp54 = (P.scheme == 2);
   const int prec = P.precision;   // 0 FP64, 1 FP32, 2 FP32 equations + FP64 state
   const size_t smem = dp54 ? dp54_smem_bytes(OBJ != 0)
-                           : (OBJ != 0 ? (prec == 1 ? sizeof(float) : sizeof(double)) * kBlock * kParkSlotsRk4 : 0);
+                           : (OBJ != 0 ? (prec == 1 ? sizeof(float) : sizeof(double)) * kBlock * kParkSlotsRk4 : 0) + kBirthQueueBytes;
   int dev = 0;
   GP_CUDA(cudaGetDevice(&dev));
   if (dev < 0 || dev >= kMaxDevices) return GP_E_UNSUPPORTED;

@@ -28,6 +28,9 @@ struct TraceParams {
   double h, h_rel, rtol, atol, h_cap_rel;
   long long max_steps;
   double lambda_max;   // +inf when the configuration has no affine budget (cfg.lambda_max <= 0)
+  float h_f, h_rel_f;  // h and h_rel rounded to FP32, lambda_max rounded UP to FP32 (for any float x:
+  float lambda_max_f;  // x >= lambda_max_f <=> (double)x >= lambda_max): the FP32 kernels' operands
+  float pad_f_;
   double r_cap, r_esc;              // r_H (1 + eps_capture), r_escape
   double disk_r_in, disk_r_out;
   double ring_d;                    // half opening angle of the solid ring (> 0: object kind 2)

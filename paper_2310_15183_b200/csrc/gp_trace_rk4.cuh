@@ -20,19 +20,63 @@ namespace gp {
 #if defined(__CUDACC__)
 
 constexpr int kParkSlotsRk4 = 7;  // trial state (r, th, pr, pth, t, ph, lambda) across an equator landing
+constexpr int kBirthQueueDoubles = 9;   // per queued ray (see the kernel)
+constexpr size_t kBirthQueueBytes = (size_t)(kBlock / 32) * kBirthQueueDoubles * 32 * sizeof(double);
 
-// (the disk variant of the FP64 Kerr kernel needs a few registers more than the 128 that four resident
-// blocks allow: it is held to three; the FP64 Manko-Novikov duals need up to 255: two blocks)
+// Rows a2 + a3 and the reference value of the Carter monitor for one queued ray; e[k * 32], k = 0..8.
+// Out of line on purpose: it runs once per 32 rays with every lane's ray state live around it, and inlined its
+// FP64 temporaries came on top of that state (158 registers instead of 122 in the FP64 kernel); as a call it
+// costs a few saves and restores around a cold path.
+template <int METRIC>
+__device__ __noinline__ void birth_to_queue(const CameraConst &cc, const MetricConst &mc, long long ray, double *e) {
+  double dr0, dth0, dph0, dpt, dpr, dpth, dpph, q0 = 0.0, iq0 = 1.0;
+  ray_birth(cc, mc, ray, dr0, dth0, dph0, dpt, dpr, dpth, dpph);
+  if (METRIC != METRIC_MN) {
+    // Reference value of the Carter monitor (R23), once per ray, from the initial state (H = 0 there by
+    // construction, so the term in H is left out: a 1e-16 relative difference to the value taken at the
+    // first step) — the per-step monitor then carries no "first step" instructions.
+    double s0, c0;
+    sincos(dth0, &s0, &c0);
+    const double a2 = (METRIC == METRIC_KERR) ? mc.a2 : 0.0;
+    q0 = dpth * dpth + c0 * c0 * (dpph * dpph / (s0 * s0) - a2 * dpt * dpt);
+    iq0 = 1.0 / fmax(1.0, fabs(q0));
+  }
+  e[0 * 32] = dr0; e[1 * 32] = dth0; e[2 * 32] = dph0; e[3 * 32] = dpt; e[4 * 32] = dpr;
+  e[5 * 32] = dpth; e[6 * 32] = dpph; e[7 * 32] = q0; e[8 * 32] = iq0;
+}
+
+template <bool B> struct LandTag { static constexpr bool value = B; };
+
+// Resident blocks per SM asked of ptxas (0 = its own choice), by variant:
+//   FP64 Manko-Novikov                        2  (the duals need up to 255 registers)
+//   FP64 Kerr with an object                  3  (a few registers more than the 128 of four blocks)
+//   other FP64 Schwarzschild / Kerr           4  (128 registers; the out-of-line batch birth is saved around)
+//   FP32 state, no object, Schw. / Kerr       5  (96 registers; measured on B200 at 4096^2: 137.2 ms with four
+//                                                blocks, 129.8 with five, 130.2 with six, 131.3 with eight)
+//   FP32 with an object, FP32 equations + FP64 state (Schwarzschild / Kerr)   4
+template <int METRIC, int OBJ, class T, class S>
+constexpr int rk4_min_blocks() {
+  if (METRIC == METRIC_MN) return sizeof(T) == 8 ? 2 : 0;
+  if (sizeof(T) == 8) return (OBJ != 0 && METRIC == METRIC_KERR) ? 3 : 4;
+  return (sizeof(S) == 4 && OBJ == 0) ? 5 : 4;
+}
+
 // OBJ: 0 no object; 1 thin disk, crossings located and recorded (R19); 2 solid ring, the ray ends where it
 // enters the volume (R39).  Both objects use the park area.
 template <int METRIC, int OBJ, class T, class S = T>
-__global__ void __launch_bounds__(kBlock, (sizeof(T) == 8 && METRIC == METRIC_MN) ? 2 : ((OBJ != 0 && sizeof(T) == 8 && METRIC == METRIC_KERR) ? 3 : 0)) trace_rk4(const __grid_constant__ TraceParams P) {
+__global__ void __launch_bounds__(kBlock, rk4_min_blocks<METRIC, OBJ, T, S>()) trace_rk4(const __grid_constant__ TraceParams P) {
   constexpr bool DISK = (OBJ == 1), RING = (OBJ == 2);
   extern __shared__ double park_raw[];  // [kParkSlotsRk4][kBlock] of S when OBJ != 0
   S *park = reinterpret_cast<S *>(park_raw);
   const MetricConst &mc = P.mc;
   const int tid = threadIdx.x;
   const S r_cap = (S)P.r_cap, r_esc = (S)P.r_esc, half_pi = (S)kHalfPi;
+  // per-launch constants in the state's type: for S = float they are read from the parameter block as FP32
+  // operands (converted once on the host) instead of being converted from double in every step
+  constexpr bool kF32 = (sizeof(S) == 4);
+  const S h_fix = kF32 ? (S)P.h_f : (S)P.h, h_rel = kF32 ? (S)P.h_rel_f : (S)P.h_rel;
+  const S lam_max = kF32 ? (S)P.lambda_max_f : (S)P.lambda_max;   // lambda_max_f: smallest float >= lambda_max
+  const S sixth = kF32 ? S(1.0 / 6.0) : (S)dp.sixth;
 
   int mode = MODE_IDLE;
   long long slot = -1;
@@ -53,62 +97,83 @@ __global__ void __launch_bounds__(kBlock, (sizeof(T) == 8 && METRIC == METRIC_MN
     t = pk[4 * kBlock]; ph = pk[5 * kBlock]; lam = pk[6 * kBlock];                            \
     mode = MODE_NORMAL;                                                                       \
   }
+  // Birth queue: rays are fetched and born (rows a1-a3) 32 at a time by the whole warp and handed to lanes as
+  // they fall idle.  A lane that refilled alone ran the birth — 400 instructions, a quarter of them FP64 — for
+  // the whole warp with 31 lanes masked off: 7 % of the FP32 kernel's issue slots.  Near the end of the image
+  // (fewer than two rays per lane left) a warp fetches only what it needs, so that no ray waits in one warp's
+  // queue while another warp idles.  Entry: r, theta, phi, p_t, p_r, p_theta, p_phi, Q0, 1/max(1,|Q0|).
+  constexpr int kQ = kBirthQueueDoubles;
+  const unsigned lane = (unsigned)tid & 31u;
+  double *bq = park_raw + (OBJ != 0 ? (sizeof(S) * kBlock * kParkSlotsRk4) / 8 : 0) + (tid >> 5) * (kQ * 32);
+  long long q_base = 0;
+  int q_n = 0, q_head = 0;      // warp-uniform: entries in the queue, entries handed out
+  bool drained = false;         // the work counter has passed the end of the image
+  const long long tail_from = P.cc.ray_count - 2LL * (long long)gridDim.x * kBlock;
   stamp_start(P.counters);
 
   for (;;) {
-    // ---- a1: refill idle lanes ----
+    // ---- a1: refill idle lanes, from the warp's birth queue ----
     const bool need = (mode == MODE_IDLE) && !exhausted;
     const unsigned need_mask = __ballot_sync(kFull, need);
     if (need_mask) {
-      const long long got = fetch_slot(need_mask, need, P.counters, P.cc.ray_count);
+      if (q_head == q_n && !drained) {
+        // a1 + a2 + a3 for a batch: one atomic for the warp, the rays born by all lanes at once
+        const int want = (q_base + q_n >= tail_from) ? __popc(need_mask) : 32;
+        unsigned long long base = 0;
+        if (lane == 0u) base = atomicAdd(P.counters, (unsigned long long)want);
+        base = __shfl_sync(kFull, base, 0);
+        const long long left = P.cc.ray_count - (long long)base;
+        q_base = (long long)base;
+        q_n = left >= (long long)want ? want : (left > 0 ? (int)left : 0);
+        q_head = 0;
+        drained = left <= (long long)want;   // the counter is past the image: nothing more will come
+        if ((int)lane < q_n) birth_to_queue<METRIC>(P.cc, mc, P.cc.ray_begin + (q_base + lane) * P.cc.ray_stride, bq + lane);
+        __syncwarp();
+      }
+      const int avail = q_n - q_head;
       if (need) {
-        slot = got;
-        if (slot < 0) {
-          exhausted = true;
-        } else {
-          double dr0, dth0, dph0, dpt, dpr, dpth, dpph;
-          ray_birth(P.cc, mc, P.cc.ray_begin + slot * P.cc.ray_stride, dr0, dth0, dph0, dpt, dpr, dpth, dpph);
-          pt = (T)dpt; pr = (S)dpr; pth = (S)dpth; pph = (T)dpph;
-          t = S(0); r = (S)dr0; th = (S)dth0; ph = (S)dph0; lam = S(0);
+        const int rank = __popc(need_mask & ((1u << lane) - 1u));
+        if (rank < avail) {
+          const double *e = bq + (q_head + rank);
+          slot = q_base + (q_head + rank);
+          r = (S)e[0 * 32]; th = (S)e[1 * 32]; ph = (S)e[2 * 32]; pt = (T)e[3 * 32]; pr = (S)e[4 * 32];
+          pth = (S)e[5 * 32]; pph = (T)e[6 * 32];
+          mo.Q0 = (T)e[7 * 32]; mo.iQ0 = (T)e[8 * 32];
+          t = S(0); lam = S(0);
           mode = MODE_NORMAL;
           n_acc = n_cross = n_rec = n_land = 0;
-          mo.h_max = T(0); mo.q_drift = T(0); mo.Q0 = T(0); mo.iQ0 = T(1);
-          if (METRIC != METRIC_MN) {
-            // Reference value of the Carter monitor (R23), once per ray, from the initial state (H = 0 there
-            // by construction, so the term in H is left out: a 1e-16 relative difference to the value taken
-            // at the first step) — the per-step monitor then carries no "first step" instructions.
-            double s0, c0;
-            sincos(dth0, &s0, &c0);
-            const double a2 = (METRIC == METRIC_KERR) ? mc.a2 : 0.0;
-            const double q0 = dpth * dpth + c0 * c0 * (dpph * dpph / (s0 * s0) - a2 * dpt * dpt);
-            mo.Q0 = (T)q0;
-            mo.iQ0 = (T)(1.0 / fmax(1.0, fabs(q0)));
-          }
+          mo.h_max = T(0); mo.q_drift = T(0);
           mo.sin_min = (T)__longlong_as_double(0x7ff0000000000000LL);
           mo.err_margin = (T)__longlong_as_double(0x7ff0000000000000LL);
-        }
+        } else if (drained) {
+          exhausted = true;
+        }   // else: the queue ran out under this lane; it is refilled in the next trip
       }
+      const int asked = __popc(need_mask);
+      q_head += asked < avail ? asked : avail;
+      __syncwarp();
     }
     if (!__any_sync(kFull, mode != MODE_IDLE)) break;
 
     if (mode != MODE_IDLE) {
       bool finished = false;
       // stop tests at the top of every ordinary step (R18)
-      if (mode == MODE_NORMAL &&
-          (n_acc >= (unsigned)P.max_steps || (double)lam >= P.lambda_max)) {
+      if (mode == MODE_NORMAL && (n_acc >= (unsigned)P.max_steps || lam >= lam_max)) {
         status = GP_RAY_MAXSTEPS;
         finished = true;
       }
-      if (!finished) {
-        const bool normal = (mode == MODE_NORMAL);
-        const bool land_r = (mode == MODE_LAND_R);
-        const S s = normal ? (P.scheme == 0 ? (S)P.h : (S)P.h_rel * r) : (land_r ? (target - r) : (target - th));
-        // Landing steps are 1 in several hundred: their divisor work (Henon's 1/F_w) sits behind a
-        // warp-uniform branch taken only when some lane of this convergence group is landing.
-        const bool any_land = __any_sync(__activemask(), !normal);
+      // Landing steps are 1 in several hundred per lane.  The step is compiled twice: LAND = false is the
+      // ordinary step and nothing else (no Henon divisor, no mode selects, no landing bookkeeping) and runs
+      // whenever no lane of this convergence group is landing — nine warp-steps in ten; LAND = true is the
+      // same instruction stream with the per-lane reciprocal selector (gp_trace.cuh, reading R14).
+      auto step = [&](auto land_tag) {
+        constexpr bool LAND = decltype(land_tag)::value;
+        const bool normal = LAND ? (mode == MODE_NORMAL) : true;
+        const bool land_r = LAND ? (mode == MODE_LAND_R) : false;
+        const S s = normal ? (P.scheme == 0 ? h_fix : h_rel * r) : (land_r ? (target - r) : (target - th));
         S sl = S(1);  // weighted sum of 1/F_w: d(lambda)/ds of a landing step (unused otherwise)
 #define GP_HENON(weight, first)                                                   \
-  if (any_land) {                                                                 \
+  if (LAND) {                                                                     \
     T iv = normal ? T(1) : frcp(land_r ? o.dr : o.dth);                           \
     o.dt *= iv; o.dr *= iv; o.dth *= iv; o.dph *= iv; o.dpr *= iv; o.dpth *= iv;  \
     sl = (first) ? (S)iv : sl + S(weight) * (S)iv;                                \
@@ -159,7 +224,7 @@ __global__ void __launch_bounds__(kBlock, (sizeof(T) == 8 && METRIC == METRIC_MN
         st += (S)o.dt; sr += (S)o.dr; sth += (S)o.dth; sph += (S)o.dph; spr += (S)o.dpr; spth += (S)o.dpth;
 #undef GP_HENON
 #undef GP_STAGE
-        const S w = s * (S)dp.sixth;
+        const S w = s * sixth;
         const S nt = t + w * st, nr = r + w * sr, nth = th + w * sth, nph = ph + w * sph,
                 npr = pr + w * spr, npth = pth + w * spth;
 
@@ -271,6 +336,10 @@ __global__ void __launch_bounds__(kBlock, (sizeof(T) == 8 && METRIC == METRIC_MN
           }
           if (OBJ == 0) mode = MODE_NORMAL;
         }
+      };
+      if (!finished) {
+        if (__any_sync(__activemask(), mode != MODE_NORMAL)) step(LandTag<true>());
+        else step(LandTag<false>());
       }
 
       if (finished) {
