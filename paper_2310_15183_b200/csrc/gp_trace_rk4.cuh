@@ -21,7 +21,8 @@ namespace gp {
 
 constexpr int kParkSlotsRk4 = 7;  // trial state (r, th, pr, pth, t, ph, lambda) across an equator landing
 constexpr int kBirthQueueDoubles = 9;   // per queued ray (see the kernel)
-constexpr size_t kBirthQueueBytes = (size_t)(kBlock / 32) * kBirthQueueDoubles * 32 * sizeof(double);
+constexpr int kBirthQueueStride = kBirthQueueDoubles * 32 + 2;   // + the slot of entry 0 (and a pad), per warp
+constexpr size_t kBirthQueueBytes = (size_t)(kBlock / 32) * kBirthQueueStride * sizeof(double);
 
 // Rows a2 + a3 and the reference value of the Carter monitor for one queued ray; e[k * 32], k = 0..8.
 // Out of line on purpose: it runs once per 32 rays with every lane's ray state live around it, and inlined its
@@ -86,7 +87,7 @@ __global__ void __launch_bounds__(kBlock, rk4_min_blocks<METRIC, OBJ, T, S>()) t
   MonitorsT<T> mo = {T(0), T(0), T(0), T(1), T(0), T(0)};
   unsigned n_acc = 0, n_cross = 0, n_rec = 0, n_land = 0, status = 0;
   bool exhausted = false;
-  unsigned long long tot_rays = 0, tot_steps = 0, tot_rhs = 0;
+  unsigned tot_rays = 0, tot_steps = 0, tot_rhs = 0;   // per lane: < 2^32 (rays per lane x the step budget x 4)
 // the ray goes on from the trial state parked before a landing step (thin disk: always; ring: no hit); the
 // ring variant counts the equator crossing of that step here, as the oracle does after its ring test
 #define GP_RESUME_PARKED()                                                                    \
@@ -104,11 +105,12 @@ __global__ void __launch_bounds__(kBlock, rk4_min_blocks<METRIC, OBJ, T, S>()) t
   // queue while another warp idles.  Entry: r, theta, phi, p_t, p_r, p_theta, p_phi, Q0, 1/max(1,|Q0|).
   constexpr int kQ = kBirthQueueDoubles;
   const unsigned lane = (unsigned)tid & 31u;
-  double *bq = park_raw + (OBJ != 0 ? (sizeof(S) * kBlock * kParkSlotsRk4) / 8 : 0) + (tid >> 5) * (kQ * 32);
-  long long q_base = 0;
+  double *bq = park_raw + (OBJ != 0 ? (sizeof(S) * kBlock * kParkSlotsRk4) / 8 : 0) + (tid >> 5) * kBirthQueueStride;
+  long long *q_base_p = reinterpret_cast<long long *>(bq + kQ * 32);   // slot of entry 0 (read when a lane refills)
+  if (lane == 0u) *q_base_p = 0;
+  __syncwarp();
   int q_n = 0, q_head = 0;      // warp-uniform: entries in the queue, entries handed out
   bool drained = false;         // the work counter has passed the end of the image
-  const long long tail_from = P.cc.ray_count - 2LL * (long long)gridDim.x * kBlock;
   stamp_start(P.counters);
 
   for (;;) {
@@ -118,12 +120,14 @@ __global__ void __launch_bounds__(kBlock, rk4_min_blocks<METRIC, OBJ, T, S>()) t
     if (need_mask) {
       if (q_head == q_n && !drained) {
         // a1 + a2 + a3 for a batch: one atomic for the warp, the rays born by all lanes at once
-        const int want = (q_base + q_n >= tail_from) ? __popc(need_mask) : 32;
+        const bool tail = *q_base_p + q_n >= P.cc.ray_count - 2LL * (long long)gridDim.x * kBlock;
+        const int want = tail ? __popc(need_mask) : 32;
         unsigned long long base = 0;
         if (lane == 0u) base = atomicAdd(P.counters, (unsigned long long)want);
         base = __shfl_sync(kFull, base, 0);
         const long long left = P.cc.ray_count - (long long)base;
-        q_base = (long long)base;
+        const long long q_base = (long long)base;
+        if (lane == 0u) *q_base_p = q_base;
         q_n = left >= (long long)want ? want : (left > 0 ? (int)left : 0);
         q_head = 0;
         drained = left <= (long long)want;   // the counter is past the image: nothing more will come
@@ -135,7 +139,7 @@ __global__ void __launch_bounds__(kBlock, rk4_min_blocks<METRIC, OBJ, T, S>()) t
         const int rank = __popc(need_mask & ((1u << lane) - 1u));
         if (rank < avail) {
           const double *e = bq + (q_head + rank);
-          slot = q_base + (q_head + rank);
+          slot = *q_base_p + (q_head + rank);
           r = (S)e[0 * 32]; th = (S)e[1 * 32]; ph = (S)e[2 * 32]; pt = (T)e[3 * 32]; pr = (S)e[4 * 32];
           pth = (S)e[5 * 32]; pph = (T)e[6 * 32];
           mo.Q0 = (T)e[7 * 32]; mo.iQ0 = (T)e[8 * 32];
@@ -365,9 +369,9 @@ __global__ void __launch_bounds__(kBlock, rk4_min_blocks<METRIC, OBJ, T, S>()) t
   }
 
   if (tot_rays) {
-    atomicAdd(P.counters + 1, tot_rays);
-    atomicAdd(P.counters + 2, tot_steps);
-    atomicAdd(P.counters + 3, tot_rhs);
+    atomicAdd(P.counters + 1, (unsigned long long)tot_rays);
+    atomicAdd(P.counters + 2, (unsigned long long)tot_steps);
+    atomicAdd(P.counters + 3, (unsigned long long)tot_rhs);
   }
   stamp_end(P.counters);
 }
