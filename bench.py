@@ -45,11 +45,13 @@ F_STEP_BUILDER = {0: 56.0, 1: 57.0, 2: 324.0}
 # Workloads without a capture report null and say so.
 PROFILED = {
     ("headline", "fp64"): {"hw_fp64_frac": 0.512, "traffic": 8.37e7, "source": "profiles/trace_dp54_r02e.md"},
-    ("headline_rk4", "fp64"): {"hw_fp64_frac": 0.494, "traffic": 8.35e7, "source": "profiles/kernels_r02.md"},
-    ("headline_rk4", "fp32"): {"hw_fp64_frac": None, "hw_fp32_frac": 0.349, "traffic": 8.28e7,
-                               "source": "profiles/kernels_r02.md"},
-    ("headline_rk4", "mixed"): {"hw_fp64_frac": 0.096, "hw_fp32_frac": 0.230, "traffic": 8.17e7,
-                                "source": "profiles/kernels_r02.md"},
+    ("headline_rk4", "fp64"): {"hw_fp64_frac": 0.523, "traffic": 8.26e7, "source": "profiles/kernels_r02g.md"},
+    ("headline_rk4", "fp32"): {"hw_fp64_frac": None, "hw_fp32_frac": 0.386, "traffic": 8.12e7,
+                               "source": "profiles/kernels_r02g.md"},
+    ("headline_rk4", "mixed"): {"hw_fp64_frac": 0.102, "hw_fp32_frac": 0.246, "traffic": 8.12e7,
+                                "source": "profiles/kernels_r02g.md"},
+    ("C5a", "fp32"): {"hw_fp64_frac": None, "hw_fp32_frac": 0.417, "traffic": 2.12e9,
+                      "source": "profiles/kernels_r02g.md"},
 }
 # nominal FP64 FMA peak: 148 SMs x 64 FP64 FMA lanes x 2 flop x 1.965 GHz
 FP64_LANES_PER_SM = 64
