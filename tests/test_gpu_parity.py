@@ -954,3 +954,31 @@ def test_generic_parameters_mass_and_retrograde_spin(gp, O, scheme):
     rays, _, _, orc, probe = run_both(gp, O, w, 2, None, 29)
     res, smooth = check_parity(w, rays, orc, probe, f"M=1.3 a=-0.9 scheme {scheme}", max_flagged_fraction=0.02)
     assert (orc["status"] == 1).sum() > 100 and (orc["status"] == 0).sum() > 2000 and res["status_mismatch"] == 0
+
+
+@pytest.mark.parametrize("precision,disk", [(0, False), (1, False), (2, False), (0, True), (1, True)])
+def test_birth_queue_changes_no_record(gp, precision, disk):
+    """trace_rk4 fetches and births rays 32 at a time per warp into a shared-memory queue; a selection with fewer
+    than two rays per lane is served by exact fetches instead (the end-of-image rule).  One 640 x 480 image
+    (307 200 rays: the queue is in use for its first half) against the same image traced in chunks of 9973 rays
+    (never enough for the queue; ragged last chunk): every record identical bit for bit, in every precision."""
+    w = W.workload("C5a", width=640, height=480)
+    w["cfg"]["precision"] = precision
+    if disk:
+        w["cfg"].update(max_crossings=3, disk_r_in=0.0, disk_r_out=20.0)
+    n = W.n_rays(w)
+    rays, dsk, counters = gp.api.trace_workload(w)
+    assert counters[1] == n and counters[6] == n and (rays["status"] <= 5).all() and (rays["status"] <= 1).mean() > 0.999
+    parts, dparts, steps = [], [], 0
+    for begin in range(0, n, 9973):
+        r, d, c = gp.api.trace_workload(w, begin, min(9973, n - begin), 1)
+        parts.append(r.tobytes())
+        dparts.append(d.tobytes() if d is not None else b"")
+        steps += int(c[2])
+    assert b"".join(parts) == rays.tobytes()
+    assert steps == int(counters[2])
+    if disk:
+        assert b"".join(dparts) == dsk.tobytes() and (rays["n_disk_recorded"] > 0).sum() > 1000
+    # a strided selection (ray index != output slot) through the queue as well
+    r3, _, c3 = gp.api.trace_workload(w, 1, None, 3)
+    assert r3.tobytes() == rays[1::3].tobytes() and c3[1] == len(r3)
