@@ -276,7 +276,9 @@ int launch_one(const TraceParams &P, cudaStream_t stream) {
   static LaunchInfo cache[kMaxDevices][5];   // per device: dp54, rk4 FP64 / FP32 / mixed, dp54 mixed (zero-initialised)
   const bool dp54 = (P.scheme == 2);
   const int prec = P.precision;   // 0 FP64, 1 FP32, 2 FP32 equations + FP64 state
-  const size_t smem = dp54 ? dp54_smem_bytes(OBJ != 0)
+  // (the mixed adaptive kernels with an object are held to three blocks per SM by asking for the 60 KB their
+  // park area used to need: measured on config 3 at rtol 1e-7, 29.1 ms with three blocks, 32.6 ms with four)
+  const size_t smem = dp54 ? ((prec == 2 && OBJ != 0) ? 16 * (size_t)kBlock * 30 : dp54_smem_bytes(OBJ != 0))
                            : (OBJ != 0 ? (prec == 1 ? sizeof(float) : sizeof(double)) * kBlock * kParkSlotsRk4 : 0) + kBirthQueueBytes;
   int dev = 0;
   GP_CUDA(cudaGetDevice(&dev));

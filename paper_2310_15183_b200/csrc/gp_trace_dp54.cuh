@@ -25,9 +25,12 @@ namespace gp {
 //   cold     kColdSlots x double (two per pair)   state the stages never read: t, phi, lambda, the monitors,
 //                          the landing target, k1 of the two quadratures, the per-lane totals, the output
 //                          slot, the rare counters, status, segment start.
-//   park     17 x double   (disk and ring variants) what a ray resumes from after a landing step located
-//                          something on the way: trial state (r, th, pr, pth, t, ph, lambda), next step,
-//                          raw k7 (6) and its monitor triple.
+//   park     8 x double    (disk and ring variants) what a ray resumes from after a landing step located
+//                          something on the way: the accepted trial state (r, th, pr, pth, t, ph, lambda) and
+//                          the next step.  F there is evaluated again when the ray resumes (MODE_RESUME: one
+//                          evaluation per landing, the same bits) instead of being parked with its monitor
+//                          triple: 17 doubles made the block 60 KB and held these variants to three blocks per
+//                          SM; with 8 it is 50 KB and four fit, like the headline kernel.
 enum { C_T = 0, C_PH, C_LAM, C_HMAX, C_QDRIFT, C_Q0, C_IQ0, C_SINMIN, C_MARGIN, C_TARGET, C_K1T, C_K1PH,
        C_TOT_RAYS, C_TOT_STEPS, C_TOT_RHS,
        C_SLOT,      // output slot of the ray in flight (64-bit integer bits)
@@ -37,7 +40,7 @@ enum { C_T = 0, C_PH, C_LAM, C_HMAX, C_QDRIFT, C_Q0, C_IQ0, C_SINMIN, C_MARGIN, 
        C_NREJ,      // rejected steps (touched on a rejection only; a register holds the attempts)
        kColdSlots };
 constexpr int kKSlots2 = 11;   // + (sin, cos) of theta_n
-constexpr int kParkSlotsDp54 = 17;
+constexpr int kParkSlotsDp54 = 8;
 // Every area is laid out [pair][lane] with 16 bytes per lane, so that ONE per-lane base address (plus
 // compile-time offsets) reaches everything: a double slot j of the cold or park area is half (j & 1) of
 // pair j / 2.  (With separate 8- and 16-byte strides the compiler rebuilt two or three base addresses from
@@ -117,15 +120,9 @@ trace_dp54(const __grid_constant__ TraceParams P) {
 #define GP_RESUME_PARKED()                                                                     \
   {                                                                                            \
     if (RING && (th - kHalfPi) * (lds1(PS(1)) - kHalfPi) < 0.0) GP_BUMP_COUNTS(1, 0)           \
-    r = lds1(PS(0)); th = lds1(PS(1)); pr = lds1(PS(2)); pth = lds1(PS(3));                    \
-    lam = lds1(PS(6)); h = lds1(PS(7));                                                        \
-    sts1(CS(C_T), lds1(PS(4))); sts1(CS(C_PH), lds1(PS(5))); sts1(CS(C_LAM), lam);             \
-    sts1(CS(C_K1T), lds1(PS(8))); sts1(CS(C_K1PH), lds1(PS(11)));                              \
-    GP_SET_K1(lds1(PS(9)), lds1(PS(10)), lds1(PS(12)), lds1(PS(13)))                           \
-    { double rs_, rc_; sincos_fast(th, &rs_, &rc_); GP_SET_SC(rs_, rc_) }                      \
-    monH = lds1(PS(14)); monQ = lds1(PS(15)); monS = lds1(PS(16));                             \
-    mode = MODE_NORMAL;                                                                        \
-    moved = true;                                                                              \
+    nr = lds1(PS(0)); nth = lds1(PS(1)); npr = lds1(PS(2)); npth = lds1(PS(3));                \
+    nt = lds1(PS(4)); nph = lds1(PS(5)); nlam = lds1(PS(6)); h = lds1(PS(7));                  \
+    mode = MODE_RESUME;   /* block A of the next trip evaluates F there, block B takes it as y_n */ \
   }
 #define GP_BUMP_COUNTS(dcross_, dland_)                                                        \
   {                                                                                            \
@@ -196,13 +193,14 @@ trace_dp54(const __grid_constant__ TraceParams P) {
       bool moved = false;   // y_n changed: run the stop tests' monitor on the new state
       double monH = 0.0, monQ = 0.0, monS = 0.0;
       double lam = 0.0;     // lambda of y_n, valid after this block when mode == MODE_NORMAL
-      if (mode == MODE_FRESH || (SEG && mode == MODE_RESUME)) {
+      constexpr bool kResumes = SEG || OBJ != 0;   // MODE_RESUME exists: segmented tracing, or a parked trial state
+      if (mode == MODE_FRESH || (kResumes && mode == MODE_RESUME)) {
         r = nr; th = nth; pr = npr; pth = npth; lam = nlam;
         sts1(CS(C_T), nt); sts1(CS(C_PH), nph); sts1(CS(C_LAM), nlam);
         GP_SET_K1(o7.dr, o7.dth, o7.dpr, o7.dpth)
         GP_SET_SC(o7.s, o7.c)
         sts1(CS(C_K1T), o7.dt); sts1(CS(C_K1PH), o7.dph);
-        if (!SEG || mode == MODE_FRESH) h = P.h_cap_rel * nr;   // R10 item 4: h0 = cap x the start radius (r_obs for the pinhole); a resumed ray keeps its proposal
+        if (!kResumes || mode == MODE_FRESH) h = P.h_cap_rel * nr;   // R10 item 4: h0 = cap x the start radius (r_obs for the pinhole); a resumed ray keeps its proposal
         monH = fabs(0.5 * o7.H2); monQ = carter_q<METRIC>(mc, pt, pph, npth, o7); monS = fabs(o7.s);
         if (METRIC != METRIC_MN && mode == MODE_FRESH) {
           // the reference value of the Carter monitor (R23) is set here, once per ray, so that the per-step
@@ -266,17 +264,12 @@ trace_dp54(const __grid_constant__ TraceParams P) {
               mode = MODE_LAND_R;
             } else {
               bool commit = true;
-              // park the accepted trial state (and F there) so that the ray can resume from it after a
+              // park the accepted trial state and the next step, so that the ray can resume from it after a
               // landing step located something on the way from y_n
 #define GP_PARK()                                                                        \
   {                                                                                      \
     sts1(PS(0), nr); sts1(PS(1), nth); sts1(PS(2), npr); sts1(PS(3), npth);              \
     sts1(PS(4), nt); sts1(PS(5), nph); sts1(PS(6), lam + h); sts1(PS(7), hnext);         \
-    sts1(PS(8), o7.dt); sts1(PS(9), o7.dr); sts1(PS(10), o7.dth);                        \
-    sts1(PS(11), o7.dph); sts1(PS(12), o7.dpr); sts1(PS(13), o7.dpth);                   \
-    sts1(PS(14), fabs(0.5 * o7.H2));                                                     \
-    sts1(PS(15), carter_q<METRIC>(mc, pt, pph, npth, o7));                               \
-    sts1(PS(16), fabs(o7.s));                                                            \
   }
               bool ring_try = false;
               if (RING) {
@@ -383,7 +376,7 @@ trace_dp54(const __grid_constant__ TraceParams P) {
           }
           GP_RESUME_PARKED()
         }
-        if (!RING) {
+        if (OBJ == 0) {
           mode = MODE_NORMAL;
           moved = true;
         }
@@ -449,8 +442,10 @@ trace_dp54(const __grid_constant__ TraceParams P) {
         sts1(CS(C_TOT_STEPS), lds1(CS(C_TOT_STEPS)) + (double)attempts);
         sts1(CS(C_TOT_RHS), lds1(CS(C_TOT_RHS)) + (double)n_rhs);
         mode = MODE_IDLE;
-      } else if (!SEG || mode != MODE_IDLE) {
+      } else if (!kResumes || (mode != MODE_IDLE && mode != MODE_RESUME)) {
         // ---- C: stages 2..6 of the next attempt from (y_n, k1) ----
+        // (a lane that has just parked its segment, or that resumes from a parked trial state and has no k1
+        // yet, sits this block out)
         // step and reciprocal selector: ordinary step s = h, divisor 1; landing s = target - y_w,
         // divisor F_w (w = r or theta).  A landing step never returns to (y_n, k1) — the ray ends
         // (r) or resumes from the parked state (theta) — so k1 is scaled in place.
