@@ -277,7 +277,8 @@ int launch_one(const TraceParams &P, cudaStream_t stream) {
   const bool dp54 = (P.scheme == 2);
   const int prec = P.precision;   // 0 FP64, 1 FP32, 2 FP32 equations + FP64 state
   // (the mixed adaptive kernels with an object are held to three blocks per SM by asking for the 60 KB their
-  // park area used to need: measured on config 3 at rtol 1e-7, 29.1 ms with three blocks, 32.6 ms with four)
+  // park area used to need: measured on config 3 at rtol 1e-7, 29.1 ms with three blocks, 32.6 ms with four;
+  // without an object four are faster for them too: 10.83 against 11.40 ms on the headline at rtol 1e-7)
   const size_t smem = dp54 ? ((prec == 2 && OBJ != 0) ? 16 * (size_t)kBlock * 30 : dp54_smem_bytes(OBJ != 0))
                            : (OBJ != 0 ? (prec == 1 ? sizeof(float) : sizeof(double)) * kBlock * kParkSlotsRk4 : 0) + kBirthQueueBytes;
   int dev = 0;
