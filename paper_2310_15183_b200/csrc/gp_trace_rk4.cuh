@@ -50,6 +50,8 @@ template <bool B> struct LandTag { static constexpr bool value = B; };
 
 // Resident blocks per SM asked of ptxas (0 = its own choice), by variant:
 //   FP64 Manko-Novikov                        2  (the duals need up to 255 registers)
+//   Manko-Novikov with FP32 equations         4  (128 registers, no spill; left to itself ptxas also stops at
+//                                                128 but spills a word in one variant)
 //   FP64 Kerr with an object                  3  (a few registers more than the 128 of four blocks)
 //   other FP64 Schwarzschild / Kerr           4  (128 registers; the out-of-line batch birth is saved around)
 //   FP32 state, no object, Schw. / Kerr       5  (96 registers; measured on B200 at 4096^2: 137.2 ms with four
@@ -57,7 +59,7 @@ template <bool B> struct LandTag { static constexpr bool value = B; };
 //   FP32 with an object, FP32 equations + FP64 state (Schwarzschild / Kerr)   4
 template <int METRIC, int OBJ, class T, class S>
 constexpr int rk4_min_blocks() {
-  if (METRIC == METRIC_MN) return sizeof(T) == 8 ? 2 : 0;
+  if (METRIC == METRIC_MN) return sizeof(T) == 8 ? 2 : 4;
   if (sizeof(T) == 8) return (OBJ != 0 && METRIC == METRIC_KERR) ? 3 : 4;
   return (sizeof(S) == 4 && OBJ == 0) ? 5 : 4;
 }
@@ -84,9 +86,9 @@ __global__ void __launch_bounds__(kBlock, rk4_min_blocks<METRIC, OBJ, T, S>()) t
   T pt = T(0), pph = T(0);
   S t = S(0), r = S(0), th = S(0), ph = S(0), pr = S(0), pth = S(0), lam = S(0);
   S target = S(0);
-  MonitorsT<T> mo = {T(0), T(0), T(0), T(1), T(0), T(0)};
+  // (err_margin belongs to the adaptive scheme: +inf in every fixed-step record, a constant that needs no register)
+  MonitorsT<T> mo = {T(0), T(0), T(0), T(1), T(0), (T)__longlong_as_double(0x7ff0000000000000LL)};
   unsigned n_acc = 0, n_cross = 0, n_rec = 0, n_land = 0, status = 0;
-  bool exhausted = false;
   unsigned tot_rays = 0, tot_steps = 0, tot_rhs = 0;   // per lane: < 2^32 (rays per lane x the step budget x 4)
 // the ray goes on from the trial state parked before a landing step (thin disk: always; ring: no hit); the
 // ring variant counts the equator crossing of that step here, as the oracle does after its ring test
@@ -111,11 +113,12 @@ __global__ void __launch_bounds__(kBlock, rk4_min_blocks<METRIC, OBJ, T, S>()) t
   __syncwarp();
   int q_n = 0, q_head = 0;      // warp-uniform: entries in the queue, entries handed out
   bool drained = false;         // the work counter has passed the end of the image
+  bool none_left = false;       // ... and the queue is empty: idle lanes stay idle (warp-uniform)
   stamp_start(P.counters);
 
   for (;;) {
     // ---- a1: refill idle lanes, from the warp's birth queue ----
-    const bool need = (mode == MODE_IDLE) && !exhausted;
+    const bool need = (mode == MODE_IDLE) && !none_left;
     const unsigned need_mask = __ballot_sync(kFull, need);
     if (need_mask) {
       if (q_head == q_n && !drained) {
@@ -148,13 +151,11 @@ __global__ void __launch_bounds__(kBlock, rk4_min_blocks<METRIC, OBJ, T, S>()) t
           n_acc = n_cross = n_rec = n_land = 0;
           mo.h_max = T(0); mo.q_drift = T(0);
           mo.sin_min = (T)__longlong_as_double(0x7ff0000000000000LL);
-          mo.err_margin = (T)__longlong_as_double(0x7ff0000000000000LL);
-        } else if (drained) {
-          exhausted = true;
-        }   // else: the queue ran out under this lane; it is refilled in the next trip
+        }   // else: the queue ran out under this lane; it is refilled in the next trip (if anything is left)
       }
       const int asked = __popc(need_mask);
       q_head += asked < avail ? asked : avail;
+      none_left = drained && q_head == q_n;
       __syncwarp();
     }
     if (!__any_sync(kFull, mode != MODE_IDLE)) break;
