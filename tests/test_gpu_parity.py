@@ -982,3 +982,40 @@ def test_birth_queue_changes_no_record(gp, precision, disk):
     # a strided selection (ray index != output slot) through the queue as well
     r3, _, c3 = gp.api.trace_workload(w, 1, None, 3)
     assert r3.tobytes() == rays[1::3].tobytes() and c3[1] == len(r3)
+
+
+def test_rk4_sweep_full_image_sampled_parity(gp, O):
+    """The launch bench.py times for the fixed-step sweep (BASELINE.json configs[4]'s setup at 1024 x 1024 and at
+    2048 x 2048: every ray, one persistent launch, rays born in batches through the warp queue), compared record
+    by record with the oracle on a scattered sample the oracle traces one by one — test_c5_fixed_relative_step_
+    subsample traces the sample only, which is a different launch.  The FP32 and mixed launches of the same image
+    are held to north_star's 1e-4 against the FP64 records on the smooth sample."""
+    for side, stride in ((1024, 4099), (2048, 16411)):
+        w = W.workload("headline_rk4", width=side, height=side)
+        n = W.n_rays(w)
+        rays, _, counters = gp.api.trace_workload(w)
+        assert len(rays) == n and counters[1] == n and counters[6] == n
+        b, c, s = W.ray_selection(w, 5, None, stride)
+        orc, _ = O.trace(w, b, c, s)
+        probe, _ = O.trace(w, b, c, s, rounding_probe=True)
+        res, smooth = check_parity(w, rays[b::s][:c], orc, probe, f"headline_rk4 {side} sample", max_flagged_fraction=0.02)
+        assert res["status_mismatch"] == 0 and smooth.sum() > 0.9 * c
+        assert int(counters[2]) == int(rays["n_accepted"].sum())
+        if side != 1024:
+            continue
+        ref = rays[b::s][:c]
+        for precision, tol in ((1, 1e-4), (2, 1e-4)):
+            w32 = W.workload("headline_rk4", width=side, height=side)
+            w32["cfg"]["precision"] = precision
+            r32, _, c32 = gp.api.trace_workload(w32)
+            assert c32[1] == n
+            got = r32[b::s][:c]
+            ok = smooth & (orc["status"] == 0) & (got["status"] == 0) & (orc["sin_theta_min"] >= 0.02)
+            assert ok.sum() > 0.6 * c
+            worst = 0.0
+            for f in ("theta", "phi", "lambda", "t"):
+                d = np.abs(got[f][ok] - ref[f][ok]) / np.maximum(1.0, np.abs(ref[f][ok]))
+                frac_bad = (d > tol).mean()
+                worst = max(worst, float(d.max()))
+                assert frac_bad <= (0.001 if precision == 1 else 0.0) and d.max() <= 1e-3, (precision, f, frac_bad, d.max())
+            print(f"precision {precision}: worst {worst:.2e} on {int(ok.sum())} smooth escaped rays")
