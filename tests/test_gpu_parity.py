@@ -1019,3 +1019,31 @@ def test_rk4_sweep_full_image_sampled_parity(gp, O):
                 worst = max(worst, float(d.max()))
                 assert frac_bad <= (0.001 if precision == 1 else 0.0) and d.max() <= 1e-3, (precision, f, frac_bad, d.max())
             print(f"precision {precision}: worst {worst:.2e} on {int(ok.sum())} smooth escaped rays")
+
+
+def test_c3_full_image_sampled_parity(gp, O):
+    """BASELINE.json configs[2] in the launch bench.py times (1024 x 1024, every ray, one persistent launch of the
+    disk kernel at four blocks per SM, crossings located from a parked trial state that the ray resumes through
+    block A): ray and disk records against the oracle on a scattered sample, and the same records from a launch of
+    the sample alone (a different grid and refill order) bit for bit."""
+    w = W.workload("C3")
+    n = W.n_rays(w)
+    rays, disk, counters = gp.api.trace_workload(w)
+    assert len(rays) == n and counters[1] == n and counters[6] == n
+    b, c, s = W.ray_selection(w, 11, None, 263)
+    orc, _ = O.trace(w, b, c, s)
+    probe, _ = O.trace(w, b, c, s, rounding_probe=True)
+    got, gdisk = rays[b::s][:c], disk[b::s][:c]
+    res, ok = check_parity(w, got, orc, probe, "C3 full image sample", max_flagged_fraction=0.01)
+    n_rec = orc["n_disk_recorded"]
+    assert res["status_mismatch"] == 0 and (n_rec > 0).sum() > 50 and n_rec.max() >= 2
+    assert np.array_equal(got["n_disk_recorded"][ok], n_rec[ok])
+    for k in range(3):
+        have = ok & (n_rec > k)
+        assert np.array_equal(np.isnan(gdisk["r_cross"][ok, k]), np.isnan(orc["disk_r"][ok, k]))
+        if have.any():
+            assert rel_err(gdisk["r_cross"][have, k], orc["disk_r"][have, k]).max() <= TOL
+            assert rel_err(gdisk["g"][have, k], orc["disk_g"][have, k]).max() <= TOL
+    alone, adisk, _ = gp.api.trace_workload(w, b, c, s)
+    assert alone.tobytes() == got.tobytes() and adisk.tobytes() == gdisk.tobytes()
+    assert (rays["n_disk_recorded"] > 0).mean() > 0.05 and (rays["status"] <= 1).all()
