@@ -45,6 +45,7 @@ F_STEP_BUILDER = {0: 56.0, 1: 57.0, 2: 324.0}
 # Workloads without a capture report null and say so.
 PROFILED = {
     ("headline", "fp64"): {"hw_fp64_frac": 0.512, "traffic": 8.37e7, "source": "profiles/trace_dp54_r02e.md"},
+    ("C3", "fp64"): {"hw_fp64_frac": 0.500, "traffic": 1.334e8, "source": "profiles/kernels_r02g.md"},
     ("headline_rk4", "fp64"): {"hw_fp64_frac": 0.523, "traffic": 8.26e7, "source": "profiles/kernels_r02g.md"},
     ("headline_rk4", "fp32"): {"hw_fp64_frac": None, "hw_fp32_frac": 0.386, "traffic": 8.12e7,
                                "source": "profiles/kernels_r02g.md"},
