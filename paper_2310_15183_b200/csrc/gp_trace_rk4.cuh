@@ -50,8 +50,8 @@ template <bool B> struct LandTag { static constexpr bool value = B; };
 
 // Resident blocks per SM asked of ptxas (0 = its own choice), by variant:
 //   FP64 Manko-Novikov                        2  (the duals need up to 255 registers)
-//   Manko-Novikov with FP32 equations         4  (128 registers, no spill; left to itself ptxas also stops at
-//                                                128 but spills a word in one variant)
+//   Manko-Novikov with FP32 equations         4 without an object (128 registers), 3 with one (168; at 128 one
+//                                                of them spills a word)
 //   FP64 Kerr with an object                  3  (a few registers more than the 128 of four blocks)
 //   other FP64 Schwarzschild / Kerr           4  (128 registers; the out-of-line batch birth is saved around)
 //   FP32 state, no object, Schw. / Kerr       5  (96 registers; measured on B200 at 4096^2: 137.2 ms with four
@@ -59,7 +59,7 @@ template <bool B> struct LandTag { static constexpr bool value = B; };
 //   FP32 with an object, FP32 equations + FP64 state (Schwarzschild / Kerr)   4
 template <int METRIC, int OBJ, class T, class S>
 constexpr int rk4_min_blocks() {
-  if (METRIC == METRIC_MN) return sizeof(T) == 8 ? 2 : 4;
+  if (METRIC == METRIC_MN) return sizeof(T) == 8 ? 2 : (OBJ == 0 ? 4 : 3);
   if (sizeof(T) == 8) return (OBJ != 0 && METRIC == METRIC_KERR) ? 3 : 4;
   return (sizeof(S) == 4 && OBJ == 0) ? 5 : 4;
 }
@@ -104,7 +104,8 @@ __global__ void __launch_bounds__(kBlock, rk4_min_blocks<METRIC, OBJ, T, S>()) t
   // they fall idle.  A lane that refilled alone ran the birth — 400 instructions, a quarter of them FP64 — for
   // the whole warp with 31 lanes masked off: 7 % of the FP32 kernel's issue slots.  Near the end of the image
   // (fewer than two rays per lane left) a warp fetches only what it needs, so that no ray waits in one warp's
-  // queue while another warp idles.  Entry: r, theta, phi, p_t, p_r, p_theta, p_phi, Q0, 1/max(1,|Q0|).
+  // queue while another warp idles; the Manko-Novikov kernels, whose ray lengths differ by a factor of 700,
+  // always do.  Entry: r, theta, phi, p_t, p_r, p_theta, p_phi, Q0, 1/max(1,|Q0|).
   constexpr int kQ = kBirthQueueDoubles;
   const unsigned lane = (unsigned)tid & 31u;
   double *bq = park_raw + (OBJ != 0 ? (sizeof(S) * kBlock * kParkSlotsRk4) / 8 : 0) + (tid >> 5) * kBirthQueueStride;
@@ -123,7 +124,11 @@ __global__ void __launch_bounds__(kBlock, rk4_min_blocks<METRIC, OBJ, T, S>()) t
     if (need_mask) {
       if (q_head == q_n && !drained) {
         // a1 + a2 + a3 for a batch: one atomic for the warp, the rays born by all lanes at once
-        const bool tail = *q_base_p + q_n >= P.cc.ray_count - 2LL * (long long)gridDim.x * kBlock;
+        // Manko-Novikov: always exact.  Its shadow rays run to the step budget, 700 x a normal ray, and come
+        // in runs of neighbouring pixels: a batch of them would wait in one warp's queue for that warp's own
+        // lanes, each busy for a second (measured, config 5b at 512^2: 1.90 s with batches, 1.12 s without).
+        const bool tail = METRIC == METRIC_MN ||
+                          *q_base_p + q_n >= P.cc.ray_count - 2LL * (long long)gridDim.x * kBlock;
         const int want = tail ? __popc(need_mask) : 32;
         unsigned long long base = 0;
         if (lane == 0u) base = atomicAdd(P.counters, (unsigned long long)want);
@@ -171,6 +176,7 @@ __global__ void __launch_bounds__(kBlock, rk4_min_blocks<METRIC, OBJ, T, S>()) t
       // ordinary step and nothing else (no Henon divisor, no mode selects, no landing bookkeeping) and runs
       // whenever no lane of this convergence group is landing — nine warp-steps in ten; LAND = true is the
       // same instruction stream with the per-lane reciprocal selector (gp_trace.cuh, reading R14).
+      bool any_land = false;   // some lane of this convergence group is landing (set before the call)
       auto step = [&](auto land_tag) {
         constexpr bool LAND = decltype(land_tag)::value;
         const bool normal = LAND ? (mode == MODE_NORMAL) : true;
@@ -178,7 +184,7 @@ __global__ void __launch_bounds__(kBlock, rk4_min_blocks<METRIC, OBJ, T, S>()) t
         const S s = normal ? (P.scheme == 0 ? h_fix : h_rel * r) : (land_r ? (target - r) : (target - th));
         S sl = S(1);  // weighted sum of 1/F_w: d(lambda)/ds of a landing step (unused otherwise)
 #define GP_HENON(weight, first)                                                   \
-  if (LAND) {                                                                     \
+  if (LAND && any_land) {                                                         \
     T iv = normal ? T(1) : frcp(land_r ? o.dr : o.dth);                           \
     o.dt *= iv; o.dr *= iv; o.dth *= iv; o.dph *= iv; o.dpr *= iv; o.dpth *= iv;  \
     sl = (first) ? (S)iv : sl + S(weight) * (S)iv;                                \
@@ -343,7 +349,10 @@ __global__ void __launch_bounds__(kBlock, rk4_min_blocks<METRIC, OBJ, T, S>()) t
         }
       };
       if (!finished) {
-        if (__any_sync(__activemask(), mode != MODE_NORMAL)) step(LandTag<true>());
+        // (Manko-Novikov: one copy, with the divisor work behind the warp-uniform flag; the rest of the landing
+        // logic is nothing beside its dual-number evaluations)
+        any_land = __any_sync(__activemask(), mode != MODE_NORMAL);
+        if (METRIC == METRIC_MN || any_land) step(LandTag<true>());
         else step(LandTag<false>());
       }
 
