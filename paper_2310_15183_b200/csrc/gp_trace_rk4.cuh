@@ -52,15 +52,16 @@ template <bool B> struct LandTag { static constexpr bool value = B; };
 //   FP64 Manko-Novikov                        2  (the duals need up to 255 registers)
 //   Manko-Novikov with FP32 equations         4 without an object (128 registers), 3 with one (168; at 128 one
 //                                                of them spills a word)
-//   FP64 Kerr with an object                  3  (a few registers more than the 128 of four blocks)
-//   other FP64 Schwarzschild / Kerr           4  (128 registers; the out-of-line batch birth is saved around)
+//   FP64 Schwarzschild / Kerr                 4  (128 registers; the out-of-line batch birth is saved around.  With
+//                                                an object too since the step was split and the birth moved out of
+//                                                line: Kerr + disk at 1024^2 15.00 -> 14.05 ms, + ring 11.52 -> 10.91)
 //   FP32 state, no object, Schw. / Kerr       5  (96 registers; measured on B200 at 4096^2: 137.2 ms with four
 //                                                blocks, 129.8 with five, 130.2 with six, 131.3 with eight)
 //   FP32 with an object, FP32 equations + FP64 state (Schwarzschild / Kerr)   4
 template <int METRIC, int OBJ, class T, class S>
 constexpr int rk4_min_blocks() {
   if (METRIC == METRIC_MN) return sizeof(T) == 8 ? 2 : (OBJ == 0 ? 4 : 3);
-  if (sizeof(T) == 8) return (OBJ != 0 && METRIC == METRIC_KERR) ? 3 : 4;
+  if (sizeof(T) == 8) return 4;
   return (sizeof(S) == 4 && OBJ == 0) ? 5 : 4;
 }
 
