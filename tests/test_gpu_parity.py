@@ -221,6 +221,9 @@ def test_c4_manko_novikov_subsample(gp, O):
     assert np.array_equal((rays["status"] == 0)[~chaotic], (orc["status"] == 0)[~chaotic])
 
 
+_C4_SAMPLE = {}
+
+
 def test_c4_manko_novikov_at_its_own_step_budget(gp, O):
     """BASELINE.json configs[3] as written: <= 2e5 attempted steps per ray.  511 scattered rays of the
     2048 x 2048 image, about 55 of them inside the shadow, where they stall near r = 1.59 M and run to
@@ -229,6 +232,7 @@ def test_c4_manko_novikov_at_its_own_step_budget(gp, O):
     assert w["cfg"]["max_steps"] == 200_000
     sel = W.ray_selection(w, 11, None, 8209)
     rays, _, counters, orc, probe = run_both(gp, O, w, *sel)
+    _C4_SAMPLE["oracle"] = (orc, probe)          # reused by test_c4_full_image_sampled_parity (same selection)
     res, _ = check_parity(w, rays, orc, probe, "C4 (2e5 steps)", max_flagged_fraction=0.03)
     shadow = orc["status"] != 0
     assert len(orc) >= 500 and shadow.sum() >= 40, (len(orc), int(shadow.sum()))
@@ -280,6 +284,9 @@ def test_mn_q0_reproduces_kerr_on_gpu(gp, O):
         assert rel_err(a[f], b[f])[smooth].max() <= TOL, f
 
 
+_C5_SAMPLE = {}
+
+
 @pytest.mark.parametrize("name,stride,flagged", [("C5a", 16411, 0.01), ("C5b", 65521, 0.05)])
 def test_c5_fixed_relative_step_subsample(gp, O, name, stride, flagged):
     """C5b: the Manko-Novikov shadow interior (3.5 % of this sample) ends CAPTURED after winding
@@ -288,6 +295,7 @@ def test_c5_fixed_relative_step_subsample(gp, O, name, stride, flagged):
     w = W.workload(name)
     assert w["cfg"]["max_steps"] == 200_000          # BASELINE.json configs[4] at this build's stated budget
     rays, _, _, orc, probe = run_both(gp, O, w, 1, None, stride)
+    _C5_SAMPLE[name] = (orc, probe, rays)         # reused by test_c5b_full_image_sampled_parity (same selection)
     check_parity(w, rays, orc, probe, name, max_flagged_fraction=flagged)
     steps = orc["n_accepted"]
     print(name, "rays", len(orc), "captured", int((orc["status"] == 1).sum()), "longest ray", int(steps.max()),
@@ -1047,3 +1055,72 @@ def test_c3_full_image_sampled_parity(gp, O):
     alone, adisk, _ = gp.api.trace_workload(w, b, c, s)
     assert alone.tobytes() == got.tobytes() and adisk.tobytes() == gdisk.tobytes()
     assert (rays["n_disk_recorded"] > 0).mean() > 0.05 and (rays["status"] <= 1).all()
+
+
+def test_c4_full_image_sampled_parity(gp, O):
+    """BASELINE.json configs[3] in the launch `bench.py --workload C4` times: all 2048 x 2048 rays at the full
+    2e5-step budget in one persistent launch (about 16 s: 9 % of the pixels run to the budget), the Manko-Novikov
+    kernel with its exact work fetch.  The 511 scattered rays of test_c4_manko_novikov_at_its_own_step_budget are
+    read out of the full image and compared with the oracle's records under the same rules, and with a launch of
+    the sample alone bit for bit (another grid, another refill order: a ray's record depends on the ray only)."""
+    w = W.workload("C4")
+    assert w["cfg"]["max_steps"] == 200_000 and W.n_rays(w) == 2048 * 2048
+    n = W.n_rays(w)
+    rays, _, counters = gp.api.trace_workload(w)
+    assert len(rays) == n and counters[1] == n and counters[6] == n
+    b, c, s = W.ray_selection(w, 11, None, 8209)
+    if "oracle" not in _C4_SAMPLE:
+        _C4_SAMPLE["oracle"] = (O.trace(w, b, c, s)[0], O.trace(w, b, c, s, rounding_probe=True)[0])
+    orc, probe = _C4_SAMPLE["oracle"]
+    got = rays[b::s][:c]
+    assert len(got) == len(orc) == c
+    res, _ = check_parity(w, got, orc, probe, "C4 full image sample", max_flagged_fraction=0.03)
+    alone, _, _ = gp.api.trace_workload(w, b, c, s)
+    assert alone.tobytes() == got.tobytes()
+    # whole-image properties that hold at any size: every ray ended in a defined state, the budget is
+    # never exceeded, the shadow interior (MAXSTEPS or CAPTURED) is the 7-10 % of the pixels the cost model names
+    st = rays["status"]
+    odd = int((st > 2).sum())                      # NONFINITE / STEP_UNDERFLOW at the singular horizon (P:L234)
+    print(f"C4 full image: rays that ended NONFINITE or STEP_UNDERFLOW: {odd} of {n}")
+    assert (st <= 4).all() and odd <= 1e-3 * n      # measured 1359 of 4 194 304 (3.2e-4)
+    attempts = rays["n_accepted"].astype(np.int64) + rays["n_rejected"]
+    assert attempts.max() <= 200_000 and (attempts[st == 2] == 200_000).all()
+    dark = (st != 0).mean()
+    print(f"C4 full image: {dark:.4f} of the pixels do not escape; RHS evaluations {int(counters[3])}")
+    assert 0.05 < dark < 0.12, dark
+
+
+def test_c5b_full_image_sampled_parity(gp, O):
+    """BASELINE.json configs[4], Manko-Novikov half, in the launch `bench.py --workload C5b` times: all 4096 x 4096
+    rays at h = 0.02 r and the 2e5-step budget in one persistent launch of `trace_rk4<MANKO_NOVIKOV, ...>` (about
+    19 s; 2.1 GB of records, which stay on the device).  The scattered sample of
+    test_c5_fixed_relative_step_subsample is read out of the full image and compared with the oracle under the
+    same rules, and with the launch of the sample alone bit for bit."""
+    import torch
+    w = W.workload("C5b")
+    n = W.n_rays(w)
+    assert n == 4096 * 4096 and w["cfg"]["max_steps"] == 200_000
+    rays = torch.empty(n * 128, dtype=torch.uint8, device="cuda")
+    counters = torch.empty(64, dtype=torch.uint8, device="cuda")
+    gp.gp_trace(w["metric"]["id"], gp.api.metric_struct(w["metric"]), gp.api.camera_struct(w["camera"]),
+                gp.api.cfg_struct(w["cfg"]), rays, None, counters)
+    torch.cuda.synchronize()
+    cnt = counters.cpu().numpy().view("<u8")
+    assert cnt[1] == n and cnt[6] == n
+    rec = rays.view(n, 128)
+    status = rec[:, 40:44].contiguous().view(torch.int32).view(n)            # u32 status at byte 40
+    census = torch.bincount(status.to(torch.int64), minlength=6).cpu().numpy()
+    print("C5b full image: status census", census.tolist(), "accepted steps", int(cnt[2]))
+    assert census[0] > 0.9 * n and census[5] == 0 and census[3:5].sum() <= 1e-3 * n    # measured 1.1e-4: NONFINITE at the singular horizon
+    b, c, s = W.ray_selection(w, 1, None, 65521)
+    idx = torch.arange(b, n, s, device="cuda")[:c]
+    got = rec[idx].cpu().numpy().view(gp.api.RAY_DTYPE).reshape(-1)
+    del rays, rec
+    torch.cuda.empty_cache()
+    if "C5b" not in _C5_SAMPLE:
+        alone, _, _ = gp.api.trace_workload(w, b, c, s)
+        _C5_SAMPLE["C5b"] = (O.trace(w, b, c, s)[0], O.trace(w, b, c, s, rounding_probe=True)[0], alone)
+    orc, probe, alone = _C5_SAMPLE["C5b"]
+    assert len(got) == len(orc) == c
+    assert alone.tobytes() == got.tobytes()
+    check_parity(w, got, orc, probe, "C5b full image sample", max_flagged_fraction=0.05)
