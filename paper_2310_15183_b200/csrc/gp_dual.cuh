@@ -56,6 +56,14 @@ template <class S> GP_HD Dual2T<S> dsqrt(const Dual2T<S> &a) {
 }
 GP_HD double dsqrt(double a) { return sqrt(a); }
 GP_HD float dsqrt(float a) { return sqrtf(a); }
+// a^{-1/2}: one reciprocal square root, derivatives -a'/(2 a^{3/2})
+template <class S> GP_HD Dual2T<S> drsqrt(const Dual2T<S> &a) {
+  S i = frsqrt(a.v);
+  S m = S(-0.5) * i * (i * i);
+  return Dual2T<S>(i, a.dx * m, a.dy * m);
+}
+GP_HD double drsqrt(double a) { return frsqrt(a); }
+GP_HD float drsqrt(float a) { return frsqrt(a); }
 template <class S> GP_HD Dual2T<S> dexp(const Dual2T<S> &a) {
   S e = fexp(a.v);
   return Dual2T<S>(e, a.dx * e, a.dy * e);

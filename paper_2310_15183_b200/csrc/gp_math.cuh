@@ -72,6 +72,16 @@ __device__ __forceinline__ double rcp_nr(double x) {
   return fma(y, e, y);
 }
 
+// 1/sqrt(x) to about 1 ulp for normal finite x > 0: MUFU.RSQ64H seed (relative error e0 ~ 2^-22) + one cubic
+// Newton step, y (1 + e/2 + 3 e^2/8) with e = 1 - x y^2: what is left is e0^3 and the rounding of the last FMA.
+__device__ __forceinline__ double rsqrt_nr(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double e = fma(-(x * y), y, 1.0);
+  double p = fma(0.375, e, 0.5);
+  return fma(y * e, p, y);
+}
+
 // a/b to <= 1 ulp given y = rcp_nr(b): one residual correction.
 __device__ __forceinline__ double div_nr(double a, double b, double y) {
   double q = a * y;
@@ -213,6 +223,13 @@ GP_HD double frcp(double x) {
   return 1.0 / x;
 #endif
 }
+GP_HD double frsqrt(double x) {
+#if defined(__CUDA_ARCH__)
+  return rsqrt_nr(x);
+#else
+  return 1.0 / sqrt(x);
+#endif
+}
 GP_HD void fsincos(double x, double *sn, double *cs) {
 #if defined(__CUDA_ARCH__)
   sincos_fast(x, sn, cs);
@@ -274,6 +291,13 @@ GP_HD void fsincos(float x, float *sn, float *cs) {
 #else
   *sn = sinf(x);
   *cs = cosf(x);
+#endif
+}
+GP_HD float frsqrt(float x) {
+#if defined(__CUDA_ARCH__)
+  return rsqrtf(x);
+#else
+  return 1.0f / sqrtf(x);
 #endif
 }
 GP_HD double fexp(double x) { return exp(x); }

@@ -151,9 +151,13 @@ GP_HD void rhs_kerr(const MetricConst &mc, T pt, T pph, T r, T th, T pr, T pth, 
 // rho^2/(x^2-1) in e^{2 gamma} rho^2 = e^{2 gamma'} A k^2 (x^2-y^2) / ((x^2-1)(1-alpha^2)^2),
 // leaving E = k^2 A e^{2 gt}/(1-alpha^2)^2 with gt = gamma' minus that term: no log and no
 // division by x^2-1.
+template <class T> struct scalar_of { typedef T type; };
+template <class S> struct scalar_of<Dual2T<S> > { typedef S type; };
+
 template <class T>
 struct MNCore {
   T f, omega, E;
+  T iF, fE;   // 1/f and f/E as Hamilton's equations use them (see the end of mn_core)
 };
 
 template <class T>
@@ -161,8 +165,18 @@ GP_HD MNCore<T> mn_core(const MetricConst &mc, const T &x, const T &y) {
   const double al = mc.mn_alpha, be = mc.mn_beta, k = mc.mn_k;
   T x2 = sqr(x), y2 = sqr(y);
   T R2 = x2 + y2 - 1.0;            // eq 36
-  T iR2 = recip(R2);
-  T iR = dsqrt(iR2);               // 1/R
+  // FP64: 1/R by one reciprocal square root, and below 1/f from the reciprocals omega needs anyway, so that no
+  // reciprocal waits for f (config 4 -2 to -4 %).  The FP32 instantiations keep the forms their
+  // tolerance was established with (reciprocal then square root, reciprocal of f).
+  constexpr bool kShortChains = sizeof(typename scalar_of<T>::type) == 8;
+  T iR, iR2;
+  if (kShortChains) {
+    iR = drsqrt(R2);               // 1/R
+    iR2 = sqr(iR);
+  } else {
+    iR2 = recip(R2);
+    iR = dsqrt(iR2);
+  }
   T u = x * y * iR;                // eq 37
   T u2 = sqr(u);
   T P2 = 1.5 * u2 - 0.5;           // Legendre P_2
@@ -184,11 +198,23 @@ GP_HD MNCore<T> mn_core(const MetricConst &mc, const T &x, const T &y) {
   T B = sqr((x + 1.0) + (x - 1.0) * ab) + sqr((1.0 + y) * afr + (1.0 - y) * bfr);  // eq 30 (R5)
   T C = xm * opab * (bma - y * (afr + bfr)) + ym * bma * (opab + x * (1.0 - ab));  // eq 31
   T e2psi = dexp(2.0 * psi);
-  T iA = recip(A);
   MNCore<T> o;
-  o.f = e2psi * A * recip(B);                                         // eq 26
-  o.omega = (2.0 * k) * C * iA * recip(e2psi) - mc.mn_w0;             // eq 27
+  if (kShortChains) {
+    T iB = recip(B);
+    T g = recip(A) * recip(e2psi);                                    // 1/(A e^{2 psi}), shared by omega and 1/f
+    o.f = e2psi * A * iB;                                             // eq 26
+    o.omega = (2.0 * k) * C * g - mc.mn_w0;                           // eq 27
+    o.iF = B * g;
+  } else {
+    T iA = recip(A);
+    o.f = e2psi * A * recip(B);                                       // eq 26
+    o.omega = (2.0 * k) * C * iA * recip(e2psi) - mc.mn_w0;           // eq 27
+    o.iF = recip(o.f);
+  }
   o.E = mc.mn_e0 * A * dexp(2.0 * gt);                                // eq 28 x rho^2
+  // f/E keeps its reciprocal of E: the form in which A cancels, e^{2 psi - 2 gt}/(e0 B), stays finite where this
+  // product overflows, and that changes how rays that step onto the singular horizon end.
+  o.fE = o.f * recip(o.E);
   return o;
 }
 
@@ -206,11 +232,10 @@ GP_HD void rhs_manko_novikov(const MetricConst &mc, T pt, T pph, T r, T th, T pr
   D Del = (k * k) * (sqr(x) - T(1));
   D s2(s * s, T(0), T(-2) * c);          // sin^2 = 1 - y^2
   D iDs = recip(Del * s2);
-  D iE = recip(m.E);
-  D iF = recip(m.f);
+  const D &iF = m.iF;
   D L = pph + m.omega * pt;               // p_ph + omega p_t
   D fL = m.f * L * iDs;                   // = dphi/dlambda
-  D fE = m.f * iE;                        // g^{th th}
+  const D &fE = m.fE;                     // g^{th th}
   D K = Del * (pr * pr) + pth * pth;
   D H2 = fL * L + fE * K - (pt * pt) * iF;
   o.dt = -pt * iF.v + m.omega.v * fL.v;
