@@ -89,5 +89,33 @@ def test_chaotic_band_x3_outlier_fraction_is_a_property_of_the_workload():
     assert other_points.mean() <= 0.03
 
 
+def test_fixed_step_ray_onto_the_singular_horizon_ends_by_a_rounding_decision():
+    """The Manko-Novikov disk workload of tests/test_gpu_parity.py under the fixed relative step (256 x 256 at 80
+    degrees, h = 0.02 r, every 7th ray): a ray that steps onto the singular horizon overflows, and
+    whether that leaves an infinity (NONFINITE) or a huge finite radius ("ESCAPED" with a meaningless state) is
+    decided by the rounding of the last step.  Measured on the oracle alone: ray 3643 of the sample ends NONFINITE
+    in the oracle and in its FMA build with identical records (spread 0: the `sensitive` flag cannot see it) and
+    ESCAPED in the x87 build.  This is why a change to the kernel's Manko-Novikov arithmetic that alters which
+    product overflows was not kept; the rules were not widened for it.  What is asserted is that
+    such rays stay a handful: the class of at most 3 of the 9362 rays unflagged by the FMA probe moves under the
+    third rounding sample."""
+    import math
+    w = W.workload("C4", width=256, height=256, theta_obs=math.radians(80.0))
+    w["cfg"].update(max_crossings=3, disk_r_in=4.0, disk_r_out=20.0, scheme=1, h_rel=0.02, max_steps=6000)
+    b, c, s = W.ray_selection(w, 3, None, 7)
+    orc, _ = O.trace(w, b, c, s)
+    fma, _ = O.trace(w, b, c, s, rounding_probe=True)
+    x87, _ = O.trace(w, b, c, s, rounding_probe="x87")
+    unflagged = ~(rounding_spread(orc, fma) > SENSITIVE_AT)
+    moved = unflagged & ((orc["status"] == 0) != (x87["status"] == 0))
+    print("Manko-Novikov disk, fixed step:", c, "rays,", int((~unflagged).sum()), "flagged by the FMA probe; class moved by"
+          " the x87 build on unflagged rays:", np.flatnonzero(moved).tolist(),
+          "their oracle / FMA / x87 status:", orc["status"][moved].tolist(), fma["status"][moved].tolist(),
+          x87["status"][moved].tolist())
+    assert c == 9362 and moved.sum() <= 3
+    # every such ray is one the oracle itself ended off the manifold (NONFINITE) or that the x87 build did
+    assert ((orc["status"][moved] == 3) | (x87["status"][moved] == 3)).all()
+
+
 if __name__ == "__main__":
     print(study(int(sys.argv[1]) if len(sys.argv) > 1 else 1))
