@@ -54,6 +54,11 @@ PROFILED = {
     ("C5a", "fp32"): {"hw_fp64_frac": None, "hw_fp32_frac": 0.417, "traffic": 2.12e9,
                       "source": "profiles/kernels_r02g.md"},
 }
+# captures taken at an overridden image size (--side): the Manko-Novikov configs at a size ncu can replay
+PROFILED_AT_SIDE = {
+    ("C4", "fp64", 512): {"hw_fp64_frac": 0.252, "traffic": 5.07e5,
+                          "source": "profiles/trace_dp54_mn_r02.md (addendum r02b; 17 of 32 lanes live at this size)"},
+}
 # nominal FP64 FMA peak: 148 SMs x 64 FP64 FMA lanes x 2 flop x 1.965 GHz
 FP64_LANES_PER_SM = 64
 FP32_LANES_PER_SM = 128
@@ -385,9 +390,10 @@ def run_b200(args):
     flops = alg_flops(w, attempts, n_rhs)
     achieved = flops / (kern_ms * 1e-3) / 1e12
     achieved_builder = alg_flops(w, attempts, n_rhs, builder=True) / (kern_ms * 1e-3) / 1e12
-    prof = PROFILED.get((args.workload, args.precision),
-                        {"hw_fp64_frac": None, "traffic": None,
-                         "source": "no ncu capture of this workload / precision under profiles/"})
+    none = {"hw_fp64_frac": None, "traffic": None,
+            "source": "no ncu capture of this workload / precision / size under profiles/"}
+    prof = (PROFILED_AT_SIDE.get((args.workload, args.precision, args.side), none) if args.side
+            else PROFILED.get((args.workload, args.precision), none))
     props = torch.cuda.get_device_properties(dev)
     sm_max = (clocks or {}).get("sm_max_mhz") or 1965.0
     lanes = FP32_LANES_PER_SM if fp32 else FP64_LANES_PER_SM
